@@ -122,7 +122,7 @@ def gaussian_random_field(rng, n, slope):
     amp = np.zeros_like(kk)
     nz = kk > 0
     amp[nz] = kk[nz] ** slope
-    g = np.fft.irfftn(wk * amp, s=shape)
+    g = np.fft.irfftn(wk * amp, s=shape, axes=(0, 1, 2))
     g -= g.mean()
     g /= g.std()
     return g
@@ -139,9 +139,9 @@ def solenoidal_field(rng, n, slope):
     nz = kk > 0
     amp[nz] = kk[nz] ** (slope - 1.0)
     A = [np.fft.rfftn(rng.standard_normal(shape)) * amp for _ in range(3)]  # A1, A2, A3
-    v1 = np.fft.irfftn(1j * (k2 * A[2] - k3 * A[1]), s=shape)
-    v2 = np.fft.irfftn(1j * (k3 * A[0] - k1 * A[2]), s=shape)
-    v3 = np.fft.irfftn(1j * (k1 * A[1] - k2 * A[0]), s=shape)
+    v1 = np.fft.irfftn(1j * (k2 * A[2] - k3 * A[1]), s=shape, axes=(0, 1, 2))
+    v2 = np.fft.irfftn(1j * (k3 * A[0] - k1 * A[2]), s=shape, axes=(0, 1, 2))
+    v3 = np.fft.irfftn(1j * (k1 * A[1] - k2 * A[0]), s=shape, axes=(0, 1, 2))
     return v1, v2, v3
 
 
