@@ -1,0 +1,125 @@
+/* include/rt.h — C ABI of the B200-native gray-M1 radiation sub-step library (librt_m1.so).
+ *
+ * What the library computes: one radiation sub-step of the split explicit-implicit scheme of
+ * PAPER.md (arxiv 2606.26268, Scepi & Lesur) Sect. 2.4-2.8, steps 1, 3-8, 10 of L109-120:
+ *   ghost fill -> PLM reconstruction (Eq. 17-18) -> f-preserving fix (Eq. 19-21) -> M1 closure
+ *   (Eq. 11-14) -> wave speeds (Eq. 22-26) -> HLL / GLF flux (L150) -> geometry-weighted flux
+ *   divergence (L117) -> floor/clip -> opacities (L299, L375) -> implicit coupling (Eq. 29-33, 30, 28)
+ *   -> time step (L120).
+ * "R-Gn" = reading Gn of DESIGN.md (points where the paper is silent / ambiguous / garbled).
+ *
+ * Conventions
+ *  - Every call returns an int32 status (RT_OK = 0 ...).  Nothing throws or aborts across the ABI.
+ *    rt_last_error(grid) returns a handle-owned, NUL-terminated description of the last failure.
+ *  - FIELD ARRAYS ARE DEVICE MEMORY OWNED BY THE CALLER: fp64, one contiguous array per field (SoA),
+ *    ghosted, index ((k+g3)*nt2 + (j+g2))*nt1 + (i+g1), x1 fastest, g_d = nghost (= 2) ghosts per
+ *    side on every ACTIVE dimension (n_d > 1) and 0 on inactive ones (n_d == 1); nt_d = n_d + 2 g_d.
+ *    Pointers must be 8-byte aligned (16-byte alignment enables the vectorised / bulk-copy paths).
+ *  - Arguments documented "host" are host pointers; they are copied during the call and may be
+ *    freed on return.  Arrays OF pointers (U_in[4], mom[3] ...) are host arrays of device pointers.
+ *  - The library owns only the handle: metric arrays, opacity tables, the per-cell thick-limit
+ *    scratch array and reduction scratch.  All work is enqueued on the cudaStream_t given at
+ *    rt_grid_create; only the calls documented "synchronises" wait for it.
+ *  - Stored flux variable F is the paper's F_r (it carries the 1/c of Eq. 9: f = |F|/E <= 1;
+ *    free streaming is |F| = E).  All constants are in code units (L95-97).
+ *  - There is no CPU fallback: without a CUDA device rt_grid_create returns RT_ERR_CUDA.
+ */
+#ifndef RT_M1_H
+#define RT_M1_H
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum { RT_OK = 0, RT_ERR_INVALID_ARG = 1, RT_ERR_BAD_STATE = 2, RT_ERR_CUDA = 3, RT_ERR_NOT_FINITE = 4 };
+enum { RT_CARTESIAN = 0, RT_CYLINDRICAL = 1 /* (R,phi,z) */, RT_SPHERICAL = 2 /* (r,theta,phi) */ };
+enum { RT_BC_PERIODIC = 0, RT_BC_OUTFLOW = 1, RT_BC_REFLECT = 2, RT_BC_FIXED = 3 /* ghosts left as the caller wrote them */ };
+enum { RT_SOLVER_HLL = 0, RT_SOLVER_GLF = 1 };
+enum { RT_OPAC_PLANCK = 0, RT_OPAC_ROSSELAND = 1, RT_OPAC_SCATTER = 2 };
+
+typedef struct rt_grid rt_grid; /* opaque */
+
+typedef struct {
+    double chat;    /* reduced speed of light c^ (Sect. 2.7) */
+    double c;       /* speed of light, code units */
+    double a_R;     /* radiation constant (Eq. 15) */
+    double c_v;     /* specific heat: C_v = rho c_v (Eq. 31; R-G12) */
+    double E_floor; /* positivity floor on E_r (L250; R-G11) */
+    int32_t solver;            /* RT_SOLVER_* (L150; R-G5) */
+    int32_t thick_limit;       /* 0/1: optically-thick wave-speed limit, Eq. 25-26 (L171-173; R-G7) */
+    int32_t feedback_momentum; /* 0/1: Eq. 28 (L183) applied to mom[] in rt_implicit_step */
+} rt_params;
+
+typedef struct {
+    int32_t kind; /* 0: kappa = clip(kappa0 (rho/rho0)^a (T/T0)^b, kmin, kmax)               (L299)
+                     1: bilinear table of log10 kappa on a uniform (log10 rho, log10 T) grid (L375; R-G14) */
+    double kappa0, rho0, T0, a, b, kmin, kmax;
+    int32_t n_lrho, n_lT;          /* n_lrho == 1: table in T only (the paper's form, L375) */
+    double lrho_min, lrho_max, lT_min, lT_max;
+    double rho_unit, T_unit;       /* table inputs are rho*rho_unit, T*T_unit (L97) */
+    const double* log10_kappa;     /* HOST, n_lT x n_lrho, lrho fastest; copied to the device */
+} rt_opacity;
+
+/* Grid + metric precompute (a0).  geometry: RT_*; n[3] interior cells; nghost must be 2;
+ * x1f/x2f/x3f: HOST edge coordinates, n[d]+1 strictly increasing values each (n[d] == 1 marks an
+ * inactive dimension; its two edges still give the cell extent); bc[6] = x1lo,x1hi,x2lo,x2hi,x3lo,x3hi.
+ * cuda_stream: a cudaStream_t (NULL = legacy default stream).  Volumes and face areas are the exact
+ * finite-volume integrals of R-G9; they are evaluated by a device kernel into separable 1-D factor
+ * arrays.  Errors: NULL pointer, n < 1, nghost != 2, non-monotone / non-finite edges, r < 0 or theta
+ * outside [0, pi], periodic paired with non-periodic on one axis -> RT_ERR_INVALID_ARG. */
+int32_t rt_grid_create(int32_t geometry, const int32_t n[3], int32_t nghost,
+                       const double* x1f, const double* x2f, const double* x3f,
+                       const int32_t bc[6], void* cuda_stream, rt_grid** out);
+int32_t rt_grid_destroy(rt_grid* g);
+
+/* Test hook: full 3-D metrics to HOST arrays (NULLs allowed): vol[n3][n2][n1]; area_d has n_d + 1
+ * entries along d (lower faces + the last upper face).  Synchronises. */
+int32_t rt_grid_get_metrics(rt_grid* g, double* vol, double* area1, double* area2, double* area3);
+
+int32_t rt_set_params(rt_grid* g, const rt_params* p);
+/* which = RT_OPAC_*; an opacity never set is zero.  chi = kappa_R + sigma (L89). */
+int32_t rt_set_opacity(rt_grid* g, int32_t which, const rt_opacity* o);
+
+/* Step 1 (L111) alone: periodic / outflow / reflect (normal flux negated, L291) / fixed, axis by
+ * axis (x1, then x2 over the x1-extended range, then x3).  U[4] = device pointers E, F1, F2, F3. */
+int32_t rt_fill_ghosts(rt_grid* g, double* const U[4]);
+
+/* Steps 1, 3-7 (L111-117): ghosts of U_in are filled IN PLACE, then
+ *   U_out(interior) = U_in - dt sum_d [A+ F*+ - A- F*-]/V + dt S_geo(U_in)      (unsplit, R-G9, R-G10).
+ * rho, T (device, ghosted layout; ghost values never read) are needed only when thick_limit = 1.
+ * U_out[q] must not alias U_in[q]; ghosts of U_out are not written.  dt <= 0 or non-finite ->
+ * RT_ERR_INVALID_ARG; rt_set_params not called -> RT_ERR_BAD_STATE.  Asynchronous. */
+int32_t rt_explicit_step(rt_grid* g, double dt, const double* rho, const double* T,
+                         double* const U_in[4], double* const U_out[4]);
+
+/* Step 8 (L118) + floor/clip (R-G11), in place on the interior of U, T and (if feedback_momentum
+ * and mom != NULL) mom: E <- max(E, E_floor); |F| <= E; opacities at (rho, T); closed-form solution
+ * of the 2x2 system Eq. 33 (R-G12); F' = F/(1 + dt chat chi rho) (Eq. 30); m' = m - (F' - F)/chat
+ * (Eq. 28).  Asynchronous. */
+int32_t rt_implicit_step(rt_grid* g, double dt, const double* rho, double* T,
+                         double* const mom[3], double* const U[4]);
+
+/* Step 10 (L120; R-G15): dt = cfl / max_cells sum_{d active} chat max(|lam1|,|lam3|)(U; d) / dl_d.
+ * rt_cfl_dt writes a HOST double and synchronises the stream; rt_cfl_dt_async writes a DEVICE
+ * double and does not synchronise (graph-capturable). */
+int32_t rt_cfl_dt(rt_grid* g, const double* const U[4], double cfl, double* dt_host);
+int32_t rt_cfl_dt_async(rt_grid* g, const double* const U[4], double cfl, double* dt_device);
+
+/* Activations of the E floor and of the cell-centre f <= 1 clip in rt_implicit_step since the
+ * last call (then reset).  Synchronises. */
+int32_t rt_get_floor_counts(rt_grid* g, int64_t* n_floor, int64_t* n_clip);
+
+/* Number of kernel launches the library has enqueued on this grid since creation (bench bookkeeping). */
+int64_t rt_get_launch_count(const rt_grid* g);
+
+/* Launch-shape tuning knob, not part of the method: cells marched per thread along the sweep
+ * direction in the x2/x3 sweeps (0 = library default). */
+int32_t rt_set_tuning(rt_grid* g, int32_t march_len, int32_t reserved);
+
+const char* rt_last_error(const rt_grid* g);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -1,0 +1,481 @@
+// rt_api.cu — the C ABI of include/rt.h: argument validation, the handle, kernel launches.
+// No physics here: every step of the path runs in the kernels of rt_kernels_*.cuh.
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdarg.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <new>
+#include <vector>
+
+#include "../../include/rt.h"
+#include "rt_kernels_step.cuh"
+
+using namespace rtm1;
+
+struct rt_grid {
+    GridDev dev;
+    cudaStream_t stream;
+    double* metric_buf;
+    double* lim;  // thick-limit pre-pass array, ntot doubles (lazily allocated)
+    CflScratch* scr;
+    double* dt_dev;
+    double* dt_pinned;
+    unsigned long long* counters;  // device: floor, clip
+    unsigned long long* counters_pinned;
+    rt_params par;
+    int have_par;
+    OpacDev opac[3];
+    double* table_dev[3];
+    std::vector<double> table_host[3];
+    rt_opacity opac_host[3];
+    int same_PR;
+    int march_len;
+    long long launches;
+    char err[256];
+};
+
+static int32_t fail(rt_grid* g, int32_t code, const char* fmt, ...) {
+    if (g) {
+        va_list ap;
+        va_start(ap, fmt);
+        vsnprintf(g->err, sizeof(g->err), fmt, ap);
+        va_end(ap);
+    }
+    return code;
+}
+
+#define RT_CUDA(g, call)                                                                                       \
+    do {                                                                                                       \
+        cudaError_t e_ = (call);                                                                               \
+        if (e_ != cudaSuccess) return fail((g), RT_ERR_CUDA, "%s: %s", #call, cudaGetErrorString(e_));      \
+    } while (0)
+
+#define RT_LAUNCH_CHECK(g)                                                                                     \
+    do {                                                                                                       \
+        (g)->launches += 1;                                                                                    \
+        cudaError_t e_ = cudaGetLastError();                                                                   \
+        if (e_ != cudaSuccess) return fail((g), RT_ERR_CUDA, "kernel launch: %s", cudaGetErrorString(e_));    \
+    } while (0)
+
+static bool aligned8(const void* p) { return p && (reinterpret_cast<uintptr_t>(p) & 7u) == 0; }
+
+extern "C" const char* rt_last_error(const rt_grid* g) { return g ? g->err : "null grid handle"; }
+extern "C" int64_t rt_get_launch_count(const rt_grid* g) { return g ? g->launches : 0; }
+
+extern "C" int32_t rt_set_tuning(rt_grid* g, int32_t march_len, int32_t reserved) {
+    (void)reserved;
+    if (!g || march_len < 0) return fail(g, RT_ERR_INVALID_ARG, "rt_set_tuning: bad argument");
+    g->march_len = march_len;
+    return RT_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+extern "C" int32_t rt_grid_create(int32_t geometry, const int32_t n[3], int32_t nghost, const double* x1f,
+                                  const double* x2f, const double* x3f, const int32_t bc[6], void* cuda_stream,
+                                  rt_grid** out) {
+    if (!n || !x1f || !x2f || !x3f || !bc || !out) return RT_ERR_INVALID_ARG;
+    *out = nullptr;
+    if (geometry < 0 || geometry > 2 || nghost != 2) return RT_ERR_INVALID_ARG;
+    const double* xf[3] = {x1f, x2f, x3f};
+    for (int d = 0; d < 3; ++d) {
+        if (n[d] < 1 || n[d] > (1 << 24)) return RT_ERR_INVALID_ARG;
+        for (int i = 0; i <= n[d]; ++i)
+            if (!isfinite(xf[d][i])) return RT_ERR_INVALID_ARG;
+        for (int i = 0; i < n[d]; ++i)
+            if (!(xf[d][i + 1] > xf[d][i])) return RT_ERR_INVALID_ARG;
+        if (bc[2 * d] < 0 || bc[2 * d] > 3 || bc[2 * d + 1] < 0 || bc[2 * d + 1] > 3) return RT_ERR_INVALID_ARG;
+        if ((bc[2 * d] == RT_BC_PERIODIC) != (bc[2 * d + 1] == RT_BC_PERIODIC)) return RT_ERR_INVALID_ARG;
+    }
+    if (geometry != RT_CARTESIAN && x1f[0] < 0.0) return RT_ERR_INVALID_ARG;
+    if (geometry == RT_SPHERICAL && (x2f[0] < 0.0 || x2f[n[1]] > M_PI)) return RT_ERR_INVALID_ARG;
+    // the geometric sources ride on the x1 sweep: curvilinear grids need an active x1
+    if (geometry != RT_CARTESIAN && n[0] < 2) return RT_ERR_INVALID_ARG;
+
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) return RT_ERR_CUDA;  // no CPU fallback
+
+    rt_grid* g = new (std::nothrow) rt_grid();
+    if (!g) return RT_ERR_CUDA;
+    memset(&g->dev, 0, sizeof(g->dev));
+    g->stream = reinterpret_cast<cudaStream_t>(cuda_stream);
+    g->metric_buf = nullptr;
+    g->lim = nullptr;
+    g->scr = nullptr;
+    g->dt_dev = nullptr;
+    g->dt_pinned = nullptr;
+    g->counters = nullptr;
+    g->counters_pinned = nullptr;
+    g->have_par = 0;
+    g->same_PR = 0;
+    g->march_len = 0;
+    g->launches = 0;
+    g->err[0] = 0;
+    for (int w = 0; w < 3; ++w) {
+        memset(&g->opac[w], 0, sizeof(OpacDev));
+        memset(&g->opac_host[w], 0, sizeof(rt_opacity));
+        g->table_dev[w] = nullptr;
+    }
+    GridDev& D = g->dev;
+    D.geometry = geometry;
+    for (int d = 0; d < 3; ++d) {
+        D.n[d] = n[d];
+        D.gh[d] = n[d] > 1 ? nghost : 0;
+        D.nt[d] = n[d] + 2 * D.gh[d];
+        D.bc[2 * d] = bc[2 * d];
+        D.bc[2 * d + 1] = bc[2 * d + 1];
+    }
+    D.stride[0] = 1;
+    D.stride[1] = D.nt[0];
+    D.stride[2] = (long long)D.nt[0] * D.nt[1];
+    D.ntot = D.stride[2] * D.nt[2];
+
+    // one device buffer for edges and every 1-D factor array: per axis e,
+    //   xf (n+1), wf (n+1), vf (n), and 4 x 3 arrays (af, cg, len, ilen)[d][e] of n; plus invr (n1), cot (n2)
+    size_t total = 0;
+    for (int e = 0; e < 3; ++e) total += 2 * (size_t)(n[e] + 1) + (size_t)n[e] * (1 + 12);
+    total += (size_t)n[0] + (size_t)n[1];
+    cudaError_t ce = cudaMalloc(&g->metric_buf, total * sizeof(double));
+    if (ce == cudaSuccess) ce = cudaMalloc(&g->scr, sizeof(CflScratch));
+    if (ce == cudaSuccess) ce = cudaMalloc(&g->dt_dev, sizeof(double));
+    if (ce == cudaSuccess) ce = cudaMalloc(&g->counters, 2 * sizeof(unsigned long long));
+    if (ce == cudaSuccess) ce = cudaMallocHost(&g->dt_pinned, sizeof(double));
+    if (ce == cudaSuccess) ce = cudaMallocHost(&g->counters_pinned, 2 * sizeof(unsigned long long));
+    if (ce == cudaSuccess) ce = cudaMemsetAsync(g->scr, 0, sizeof(CflScratch), g->stream);
+    if (ce == cudaSuccess) ce = cudaMemsetAsync(g->counters, 0, 2 * sizeof(unsigned long long), g->stream);
+    if (ce != cudaSuccess) {
+        rt_grid_destroy(g);
+        return RT_ERR_CUDA;
+    }
+    MetricOut M;
+    double* p = g->metric_buf;
+    double* xdev[3];
+    for (int e = 0; e < 3; ++e) {
+        xdev[e] = p; D.xf[e] = p; p += n[e] + 1;
+        M.wf[e] = p; D.wf[e] = p; p += n[e] + 1;
+        M.vf[e] = p; D.vf[e] = p; p += n[e];
+    }
+    for (int d = 0; d < 3; ++d)
+        for (int e = 0; e < 3; ++e) {
+            M.af[d][e] = p; D.af[d][e] = p; p += n[e];
+            M.cg[d][e] = p; D.cg[d][e] = p; p += n[e];
+            M.len[d][e] = p; D.len[d][e] = p; p += n[e];
+            M.ilen[d][e] = p; D.ilen[d][e] = p; p += n[e];
+        }
+    M.invr = p; D.invr = p; p += n[0];
+    M.cot = p; D.cot = p; p += n[1];
+    for (int e = 0; e < 3 && ce == cudaSuccess; ++e)
+        ce = cudaMemcpyAsync(xdev[e], xf[e], sizeof(double) * (size_t)(n[e] + 1), cudaMemcpyHostToDevice, g->stream);
+    if (ce == cudaSuccess) ce = cudaMemsetAsync(const_cast<double*>(D.invr), 0, sizeof(double) * (size_t)(n[0] + n[1]), g->stream);
+    if (ce == cudaSuccess) {
+        k_metric_precompute<<<8, 256, 0, g->stream>>>(D, M);
+        g->launches += 1;
+        ce = cudaGetLastError();
+    }
+    // host edge arrays may be freed by the caller on return: wait for the copies
+    if (ce == cudaSuccess) ce = cudaStreamSynchronize(g->stream);
+    if (ce != cudaSuccess) {
+        rt_grid_destroy(g);
+        return RT_ERR_CUDA;
+    }
+    *out = g;
+    return RT_OK;
+}
+
+extern "C" int32_t rt_grid_destroy(rt_grid* g) {
+    if (!g) return RT_ERR_INVALID_ARG;
+    cudaStreamSynchronize(g->stream);
+    cudaFree(g->metric_buf);
+    cudaFree(g->lim);
+    cudaFree(g->scr);
+    cudaFree(g->dt_dev);
+    cudaFree(g->counters);
+    cudaFreeHost(g->dt_pinned);
+    cudaFreeHost(g->counters_pinned);
+    for (int w = 0; w < 3; ++w) cudaFree(g->table_dev[w]);
+    delete g;
+    return RT_OK;
+}
+
+extern "C" int32_t rt_grid_get_metrics(rt_grid* g, double* vol, double* area1, double* area2, double* area3) {
+    if (!g) return RT_ERR_INVALID_ARG;
+    const GridDev& D = g->dev;
+    const size_t n1 = D.n[0], n2 = D.n[1], n3 = D.n[2];
+    const size_t sz[4] = {n1 * n2 * n3, (n1 + 1) * n2 * n3, n1 * (n2 + 1) * n3, n1 * n2 * (n3 + 1)};
+    double* host[4] = {vol, area1, area2, area3};
+    double* dev[4] = {nullptr, nullptr, nullptr, nullptr};
+    int32_t rc = RT_OK;
+    for (int a = 0; a < 4 && rc == RT_OK; ++a)
+        if (host[a] && cudaMalloc(&dev[a], sz[a] * sizeof(double)) != cudaSuccess) rc = fail(g, RT_ERR_CUDA, "cudaMalloc (metrics)");
+    if (rc == RT_OK) {
+        k_metric_expand<<<296, 256, 0, g->stream>>>(D, dev[0], dev[1], dev[2], dev[3]);
+        g->launches += 1;
+        if (cudaGetLastError() != cudaSuccess) rc = fail(g, RT_ERR_CUDA, "k_metric_expand launch failed");
+    }
+    for (int a = 0; a < 4 && rc == RT_OK; ++a)
+        if (host[a] && cudaMemcpyAsync(host[a], dev[a], sz[a] * sizeof(double), cudaMemcpyDeviceToHost, g->stream) != cudaSuccess)
+            rc = fail(g, RT_ERR_CUDA, "cudaMemcpyAsync (metrics)");
+    if (cudaStreamSynchronize(g->stream) != cudaSuccess && rc == RT_OK) rc = fail(g, RT_ERR_CUDA, "stream sync (metrics)");
+    for (int a = 0; a < 4; ++a) cudaFree(dev[a]);
+    return rc;
+}
+
+extern "C" int32_t rt_set_params(rt_grid* g, const rt_params* p) {
+    if (!g || !p) return fail(g, RT_ERR_INVALID_ARG, "rt_set_params: null argument");
+    if (!(p->chat > 0.0) || !(p->c > 0.0) || !(p->a_R >= 0.0) || !(p->c_v > 0.0) || !(p->E_floor >= 0.0) ||
+        !isfinite(p->chat) || !isfinite(p->c) || !isfinite(p->a_R) || !isfinite(p->c_v) || !isfinite(p->E_floor))
+        return fail(g, RT_ERR_INVALID_ARG, "rt_set_params: chat, c, c_v must be > 0 and a_R, E_floor >= 0");
+    if (p->solver != RT_SOLVER_HLL && p->solver != RT_SOLVER_GLF) return fail(g, RT_ERR_INVALID_ARG, "rt_set_params: unknown solver");
+    g->par = *p;
+    g->have_par = 1;
+    return RT_OK;
+}
+
+static int half_int_exponent(double a) {
+    const double t = 2.0 * a;
+    if (t == rint(t) && fabs(t) <= 64.0) return (int)t;
+    return INT_MIN;
+}
+
+static bool same_law(const rt_grid* g, int a, int b) {
+    const rt_opacity &x = g->opac_host[a], &y = g->opac_host[b];
+    if (!g->opac[a].set || !g->opac[b].set || x.kind != y.kind) return false;
+    if (x.kind == 0)
+        return x.kappa0 == y.kappa0 && x.rho0 == y.rho0 && x.T0 == y.T0 && x.a == y.a && x.b == y.b && x.kmin == y.kmin &&
+               x.kmax == y.kmax;
+    return x.n_lrho == y.n_lrho && x.n_lT == y.n_lT && x.lrho_min == y.lrho_min && x.lrho_max == y.lrho_max &&
+           x.lT_min == y.lT_min && x.lT_max == y.lT_max && x.rho_unit == y.rho_unit && x.T_unit == y.T_unit &&
+           g->table_host[a] == g->table_host[b];
+}
+
+extern "C" int32_t rt_set_opacity(rt_grid* g, int32_t which, const rt_opacity* o) {
+    if (!g || !o || which < 0 || which > 2) return fail(g, RT_ERR_INVALID_ARG, "rt_set_opacity: bad argument");
+    OpacDev d;
+    memset(&d, 0, sizeof(d));
+    d.set = 1;
+    d.kind = o->kind;
+    if (o->kind == 0) {
+        if (!(o->rho0 > 0.0) || !(o->T0 > 0.0) || !(o->kmax >= o->kmin) || !(o->kmin >= 0.0) || !(o->kappa0 >= 0.0))
+            return fail(g, RT_ERR_INVALID_ARG, "rt_set_opacity: power law needs rho0, T0 > 0, kappa0 >= 0, 0 <= kmin <= kmax");
+        d.kappa0 = o->kappa0;
+        d.irho0 = 1.0 / o->rho0;
+        d.iT0 = 1.0 / o->T0;
+        d.a = o->a;
+        d.b = o->b;
+        d.kmin = o->kmin;
+        d.kmax = o->kmax;
+        d.n2a = half_int_exponent(o->a);
+        d.n2b = half_int_exponent(o->b);
+    } else if (o->kind == 1) {
+        if (!o->log10_kappa || o->n_lT < 2 || o->n_lrho < 1)
+            return fail(g, RT_ERR_INVALID_ARG, "rt_set_opacity: table needs n_lT >= 2, n_lrho >= 2 (or == 1) and data");
+        if (!(o->lT_max > o->lT_min) || !(o->T_unit > 0.0)) return fail(g, RT_ERR_INVALID_ARG, "rt_set_opacity: bad T axis");
+        if (o->n_lrho > 1 && (!(o->lrho_max > o->lrho_min) || !(o->rho_unit > 0.0)))
+            return fail(g, RT_ERR_INVALID_ARG, "rt_set_opacity: bad rho axis");
+        d.n_lrho = o->n_lrho;
+        d.n_lT = o->n_lT;
+        d.lrho_min = o->lrho_min;
+        d.lrho_max = o->lrho_max;
+        d.lT_min = o->lT_min;
+        d.lT_max = o->lT_max;
+        d.su = o->n_lrho > 1 ? (double)(o->n_lrho - 1) / (o->lrho_max - o->lrho_min) : 0.0;
+        d.sv = (double)(o->n_lT - 1) / (o->lT_max - o->lT_min);
+        d.rho_unit = o->rho_unit;
+        d.T_unit = o->T_unit;
+        const size_t cnt = (size_t)o->n_lT * (size_t)o->n_lrho;
+        g->table_host[which].assign(o->log10_kappa, o->log10_kappa + cnt);
+        RT_CUDA(g, cudaStreamSynchronize(g->stream));  // the old table may still be in use
+        cudaFree(g->table_dev[which]);
+        g->table_dev[which] = nullptr;
+        RT_CUDA(g, cudaMalloc(&g->table_dev[which], cnt * sizeof(double)));
+        RT_CUDA(g, cudaMemcpyAsync(g->table_dev[which], g->table_host[which].data(), cnt * sizeof(double),
+                                   cudaMemcpyHostToDevice, g->stream));
+        RT_CUDA(g, cudaStreamSynchronize(g->stream));
+        d.tab = g->table_dev[which];
+    } else {
+        return fail(g, RT_ERR_INVALID_ARG, "rt_set_opacity: kind must be 0 (power law) or 1 (table)");
+    }
+    g->opac[which] = d;
+    g->opac_host[which] = *o;
+    g->opac_host[which].log10_kappa = nullptr;
+    g->same_PR = same_law(g, RT_OPAC_PLANCK, RT_OPAC_ROSSELAND) ? 1 : 0;
+    return RT_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+static int32_t launch_fill_ghosts(rt_grid* g, double* const U[4]) {
+    const GridDev& D = g->dev;
+    Fields4 F;
+    for (int q = 0; q < 4; ++q) F.q[q] = U[q];
+    for (int d = 0; d < 3; ++d) {
+        if (D.gh[d] == 0) continue;
+        if (D.bc[2 * d] == RT_BC_FIXED && D.bc[2 * d + 1] == RT_BC_FIXED) continue;
+        long long tot = 4;
+        for (int e = 0; e < 3; ++e)
+            if (e != d) tot *= (e < d) ? D.nt[e] : D.n[e];
+        const int nb = (int)((tot + 255) / 256 > 4096 ? 4096 : (tot + 255) / 256);
+        k_fill_ghosts<<<nb, 256, 0, g->stream>>>(D, F, d);
+        RT_LAUNCH_CHECK(g);
+    }
+    return RT_OK;
+}
+
+extern "C" int32_t rt_fill_ghosts(rt_grid* g, double* const U[4]) {
+    if (!g || !U) return fail(g, RT_ERR_INVALID_ARG, "rt_fill_ghosts: null argument");
+    for (int q = 0; q < 4; ++q)
+        if (!aligned8(U[q])) return fail(g, RT_ERR_INVALID_ARG, "rt_fill_ghosts: U[%d] null or misaligned", q);
+    return launch_fill_ghosts(g, U);
+}
+
+template <bool HLL, bool THICK, bool CURVI>
+static void launch_x(rt_grid* g, const SweepArgs& a) {
+    const GridDev& D = g->dev;
+    const int nchunk = (D.n[0] + kXOut - 1) / kXOut;
+    const long long ntask = (long long)nchunk * D.n[1] * D.n[2];
+    const long long nblk = (ntask + 3) / 4;
+    k_sweep_x<HLL, THICK, CURVI><<<(unsigned)nblk, 128, 0, g->stream>>>(D, a, nchunk, ntask);
+}
+
+template <int DIR, bool HLL, bool THICK, bool CURVI>
+static void launch_march(rt_grid* g, const SweepArgs& a) {
+    const GridDev& D = g->dev;
+    constexpr int EO = (DIR == 1) ? 2 : 1;
+    int bx = D.n[0] >= 128 ? 128 : ((D.n[0] + 31) / 32) * 32;
+    int seg = g->march_len > 0 ? g->march_len : 32;
+    if (seg > D.n[DIR]) seg = D.n[DIR];
+    dim3 grid((D.n[0] + bx - 1) / bx, D.n[EO], (D.n[DIR] + seg - 1) / seg);
+    k_sweep_march<DIR, HLL, THICK, CURVI><<<grid, bx, 0, g->stream>>>(D, a, seg);
+}
+
+template <bool HLL, bool THICK, bool CURVI>
+static void launch_dir(rt_grid* g, int d, const SweepArgs& a) {
+    if (d == 0) launch_x<HLL, THICK, CURVI>(g, a);
+    else if (d == 1) launch_march<1, HLL, THICK, CURVI>(g, a);
+    else launch_march<2, HLL, THICK, CURVI>(g, a);
+}
+
+static void launch_sweep(rt_grid* g, int d, bool hll, bool thick, bool curvi, const SweepArgs& a) {
+    const int key = (hll ? 4 : 0) | (thick ? 2 : 0) | (curvi ? 1 : 0);
+    switch (key) {
+        case 0: launch_dir<false, false, false>(g, d, a); break;
+        case 1: launch_dir<false, false, true>(g, d, a); break;
+        case 2: launch_dir<false, true, false>(g, d, a); break;
+        case 3: launch_dir<false, true, true>(g, d, a); break;
+        case 4: launch_dir<true, false, false>(g, d, a); break;
+        case 5: launch_dir<true, false, true>(g, d, a); break;
+        case 6: launch_dir<true, true, false>(g, d, a); break;
+        default: launch_dir<true, true, true>(g, d, a); break;
+    }
+}
+
+extern "C" int32_t rt_explicit_step(rt_grid* g, double dt, const double* rho, const double* T, double* const U_in[4],
+                                    double* const U_out[4]) {
+    if (!g || !U_in || !U_out) return fail(g, RT_ERR_INVALID_ARG, "rt_explicit_step: null argument");
+    if (!g->have_par) return fail(g, RT_ERR_BAD_STATE, "rt_explicit_step: rt_set_params has not been called");
+    if (!(dt > 0.0) || !isfinite(dt)) return fail(g, RT_ERR_INVALID_ARG, "rt_explicit_step: dt must be finite and > 0");
+    for (int q = 0; q < 4; ++q)
+        if (!aligned8(U_in[q]) || !aligned8(U_out[q]) || U_in[q] == U_out[q])
+            return fail(g, RT_ERR_INVALID_ARG, "rt_explicit_step: U_in/U_out[%d] null, misaligned or aliased", q);
+    const bool thick = g->par.thick_limit != 0;
+    if (thick && (!aligned8(rho) || !aligned8(T))) return fail(g, RT_ERR_INVALID_ARG, "rt_explicit_step: thick_limit needs rho and T");
+    const GridDev& D = g->dev;
+
+    int32_t rc = launch_fill_ghosts(g, U_in);
+    if (rc != RT_OK) return rc;
+
+    if (thick) {
+        if (!g->lim) RT_CUDA(g, cudaMalloc(&g->lim, (size_t)D.ntot * sizeof(double)));
+        const int bx = 128;
+        dim3 grid((D.nt[0] + bx - 1) / bx, D.nt[1], D.nt[2]);
+        k_thick_limit<<<grid, bx, 0, g->stream>>>(D, g->opac[RT_OPAC_ROSSELAND], g->opac[RT_OPAC_SCATTER], rho, T, g->lim);
+        RT_LAUNCH_CHECK(g);
+    }
+
+    SweepArgs a;
+    for (int q = 0; q < 4; ++q) {
+        a.uin[q] = U_in[q];
+        a.uout[q] = U_out[q];
+    }
+    a.lim = thick ? g->lim : nullptr;
+    a.dtc = dt * g->par.chat;
+    const bool hll = g->par.solver == RT_SOLVER_HLL;
+    const bool curvi = D.geometry != RT_CARTESIAN;
+    if (D.gh[0] == 0) {
+        // no x1 sweep: start the accumulation from a copy of U^n (rare: grids with n1 == 1)
+        for (int q = 0; q < 4; ++q)
+            RT_CUDA(g, cudaMemcpyAsync(U_out[q], U_in[q], (size_t)D.ntot * sizeof(double), cudaMemcpyDeviceToDevice, g->stream));
+    }
+    for (int d = 0; d < 3; ++d) {
+        if (D.gh[d] == 0) continue;
+        launch_sweep(g, d, hll, thick, curvi, a);
+        RT_LAUNCH_CHECK(g);
+    }
+    return RT_OK;
+}
+
+extern "C" int32_t rt_implicit_step(rt_grid* g, double dt, const double* rho, double* T, double* const mom[3], double* const U[4]) {
+    if (!g || !U || !aligned8(rho) || !aligned8(T)) return fail(g, RT_ERR_INVALID_ARG, "rt_implicit_step: null or misaligned argument");
+    if (!g->have_par) return fail(g, RT_ERR_BAD_STATE, "rt_implicit_step: rt_set_params has not been called");
+    if (!(dt > 0.0) || !isfinite(dt)) return fail(g, RT_ERR_INVALID_ARG, "rt_implicit_step: dt must be finite and > 0");
+    for (int q = 0; q < 4; ++q)
+        if (!aligned8(U[q])) return fail(g, RT_ERR_INVALID_ARG, "rt_implicit_step: U[%d] null or misaligned", q);
+    const bool feedback = g->par.feedback_momentum && mom != nullptr;
+    if (feedback)
+        for (int q = 0; q < 3; ++q)
+            if (!aligned8(mom[q])) return fail(g, RT_ERR_INVALID_ARG, "rt_implicit_step: mom[%d] null or misaligned", q);
+    const GridDev& D = g->dev;
+    ImplicitArgs a;
+    for (int q = 0; q < 4; ++q) a.U[q] = U[q];
+    a.rho = rho;
+    a.T = T;
+    for (int q = 0; q < 3; ++q) a.mom[q] = feedback ? mom[q] : nullptr;
+    a.dt = dt;
+    a.feedback = feedback;
+    a.same_PR = g->same_PR;
+    a.counters = g->counters;
+    ParamsDev P = {g->par.chat, g->par.c, g->par.a_R, g->par.c_v, g->par.E_floor, g->par.solver, g->par.thick_limit,
+                   g->par.feedback_momentum};
+    const int bx = D.n[0] >= 128 ? 128 : ((D.n[0] + 31) / 32) * 32;
+    dim3 grid((D.n[0] + bx - 1) / bx, D.n[1], D.n[2]);
+    if (feedback)
+        k_implicit<true><<<grid, bx, 0, g->stream>>>(D, P, g->opac[0], g->opac[1], g->opac[2], a);
+    else
+        k_implicit<false><<<grid, bx, 0, g->stream>>>(D, P, g->opac[0], g->opac[1], g->opac[2], a);
+    RT_LAUNCH_CHECK(g);
+    return RT_OK;
+}
+
+extern "C" int32_t rt_cfl_dt_async(rt_grid* g, const double* const U[4], double cfl, double* dt_device) {
+    if (!g || !U || !dt_device) return fail(g, RT_ERR_INVALID_ARG, "rt_cfl_dt: null argument");
+    if (!g->have_par) return fail(g, RT_ERR_BAD_STATE, "rt_cfl_dt: rt_set_params has not been called");
+    if (!(cfl > 0.0) || !isfinite(cfl)) return fail(g, RT_ERR_INVALID_ARG, "rt_cfl_dt: cfl must be finite and > 0");
+    for (int q = 0; q < 4; ++q)
+        if (!aligned8(U[q])) return fail(g, RT_ERR_INVALID_ARG, "rt_cfl_dt: U[%d] null or misaligned", q);
+    const GridDev& D = g->dev;
+    const long long nrows = (long long)D.n[1] * D.n[2];
+    const int nb = (int)(nrows < 148 * 8 ? nrows : 148 * 8);
+    k_cfl<<<nb, 256, 0, g->stream>>>(D, g->par.chat, U[0], U[1], U[2], U[3], g->scr, cfl, dt_device);
+    RT_LAUNCH_CHECK(g);
+    return RT_OK;
+}
+
+extern "C" int32_t rt_cfl_dt(rt_grid* g, const double* const U[4], double cfl, double* dt_host) {
+    if (!dt_host) return fail(g, RT_ERR_INVALID_ARG, "rt_cfl_dt: null argument");
+    int32_t rc = rt_cfl_dt_async(g, U, cfl, g ? g->dt_dev : nullptr);
+    if (rc != RT_OK) return rc;
+    RT_CUDA(g, cudaMemcpyAsync(g->dt_pinned, g->dt_dev, sizeof(double), cudaMemcpyDeviceToHost, g->stream));
+    RT_CUDA(g, cudaStreamSynchronize(g->stream));
+    *dt_host = *g->dt_pinned;
+    return RT_OK;
+}
+
+extern "C" int32_t rt_get_floor_counts(rt_grid* g, int64_t* n_floor, int64_t* n_clip) {
+    if (!g) return RT_ERR_INVALID_ARG;
+    RT_CUDA(g, cudaMemcpyAsync(g->counters_pinned, g->counters, 2 * sizeof(unsigned long long), cudaMemcpyDeviceToHost, g->stream));
+    RT_CUDA(g, cudaMemsetAsync(g->counters, 0, 2 * sizeof(unsigned long long), g->stream));
+    RT_CUDA(g, cudaStreamSynchronize(g->stream));
+    if (n_floor) *n_floor = (int64_t)g->counters_pinned[0];
+    if (n_clip) *n_clip = (int64_t)g->counters_pinned[1];
+    return RT_OK;
+}

@@ -1,0 +1,315 @@
+// rt_kernels_aux.cuh — metric precompute (a0), ghost fill (a1), opacity evaluation (a9),
+// thick-limit pre-pass (part of a5) and the CFL reduction (a11).  SURVEY.md Sect. 8(a) row names.
+#pragma once
+#include <limits.h>
+
+#include "rt_math.cuh"
+#include "rt_types.cuh"
+
+namespace rtm1 {
+
+// ------------------------------------------------------------------------------------------------
+// a0: metric precompute.  The paper gives no metric formulas (L15, L409); DESIGN.md R-G9: exact
+// finite-volume integrals, written as separable 1-D factors.
+//   Cartesian   V = dx1 dx2 dx3;                     A_d = prod_{e != d} dx_e
+//   Cylindrical V = 1/2 D(R^2) Dphi Dz;              A_R = R_f Dphi Dz, A_phi = DR Dz, A_z = 1/2 D(R^2) Dphi
+//   Spherical   V = 1/3 D(r^3) D(-cos th) Dphi;      A_r = r_f^2 D(-cos th) Dphi,
+//               A_th = 1/2 D(r^2) sin(th_f) Dphi,    A_phi = 1/2 D(r^2) Dth
+// Lengths (CFL, tau_cell): Cartesian dx_d; cyl DR, R_c Dphi, Dz; sph Dr, r_c Dth, r_c sin(th_c) Dphi.
+// Sources: <1/R> = DR / (1/2 D(R^2)); <1/r> = 1/2 D(r^2) / (1/3 D(r^3)); <cot th> = D(sin th)/D(-cos th).
+// Output pointers are the (writable) aliases of the arrays in GridDev.
+// ------------------------------------------------------------------------------------------------
+struct MetricOut {
+    double* wf[3];
+    double* vf[3];
+    double* af[3][3];
+    double* cg[3][3];
+    double* len[3][3];
+    double* ilen[3][3];
+    double* invr;
+    double* cot;
+};
+
+__global__ void k_metric_precompute(GridDev g, MetricOut m) {
+    const int tid = blockIdx.x * blockDim.x + threadIdx.x;
+    const int nth = gridDim.x * blockDim.x;
+    const int geo = g.geometry;
+    for (int e = 0; e < 3; ++e) {
+        const double* x = g.xf[e];
+        // faces
+        for (int f = tid; f <= g.n[e]; f += nth) {
+            double w = 1.0;
+            if (geo == 1 && e == 0) w = x[f];
+            if (geo == 2 && e == 0) w = x[f] * x[f];
+            if (geo == 2 && e == 1) w = sin(x[f]);
+            m.wf[e][f] = w;
+        }
+        // cells
+        for (int c = tid; c < g.n[e]; c += nth) {
+            const double a0 = x[c], a1 = x[c + 1];
+            const double dx = a1 - a0;
+            double vf = dx;                 // volume factor along e
+            double afe[3] = {dx, dx, dx};   // area factor along e of the face normal to d (d != e)
+            double len_e[3] = {1.0, 1.0, 1.0};  // factor along e of the length along d
+            len_e[e] = dx;
+            if (geo == 1) {  // (R, phi, z)
+                if (e == 0) {
+                    const double hR2 = 0.5 * (a1 * a1 - a0 * a0);
+                    vf = hR2;
+                    afe[1] = dx;   // A_phi = DR Dz
+                    afe[2] = hR2;  // A_z = 1/2 D(R^2) Dphi
+                    len_e[1] = 0.5 * (a0 + a1);  // R_c Dphi
+                    m.invr[c] = dx / hR2;
+                }
+            } else if (geo == 2) {  // (r, theta, phi)
+                if (e == 0) {
+                    const double tr3 = (a1 * a1 * a1 - a0 * a0 * a0) / 3.0;
+                    const double hr2 = 0.5 * (a1 * a1 - a0 * a0);
+                    vf = tr3;
+                    afe[1] = hr2;
+                    afe[2] = hr2;
+                    const double rc = 0.5 * (a0 + a1);
+                    len_e[1] = rc;
+                    len_e[2] = rc;
+                    m.invr[c] = hr2 / tr3;
+                } else if (e == 1) {
+                    const double dmc = cos(a0) - cos(a1);
+                    vf = dmc;
+                    afe[0] = dmc;  // A_r = r_f^2 D(-cos th) Dphi
+                    afe[2] = dx;   // A_phi = 1/2 D(r^2) Dth
+                    len_e[2] = sin(0.5 * (a0 + a1));
+                    m.cot[c] = (sin(a1) - sin(a0)) / dmc;
+                }
+            }
+            m.vf[e][c] = vf;
+            for (int d = 0; d < 3; ++d) {
+                const double a = (d == e) ? 1.0 : afe[d];
+                m.af[d][e][c] = a;
+                m.cg[d][e][c] = (d == e) ? 1.0 / vf : a / vf;
+                m.len[d][e][c] = len_e[d];
+                m.ilen[d][e][c] = 1.0 / len_e[d];
+            }
+        }
+    }
+}
+
+// Test hook behind rt_grid_get_metrics: full 3-D volume and face areas from the separable factors.
+__global__ void k_metric_expand(GridDev g, double* vol, double* a1, double* a2, double* a3) {
+    const int n1 = g.n[0], n2 = g.n[1], n3 = g.n[2];
+    const long long tot = (long long)(n1 + 1) * (n2 + 1) * (n3 + 1);
+    for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < tot; t += (long long)gridDim.x * blockDim.x) {
+        const int i = (int)(t % (n1 + 1));
+        const int j = (int)((t / (n1 + 1)) % (n2 + 1));
+        const int k = (int)(t / ((long long)(n1 + 1) * (n2 + 1)));
+        if (vol && i < n1 && j < n2 && k < n3) vol[((long long)k * n2 + j) * n1 + i] = g.vf[0][i] * g.vf[1][j] * g.vf[2][k];
+        if (a1 && j < n2 && k < n3) a1[((long long)k * n2 + j) * (n1 + 1) + i] = g.wf[0][i] * g.af[0][1][j] * g.af[0][2][k];
+        if (a2 && i < n1 && k < n3) a2[((long long)k * (n2 + 1) + j) * n1 + i] = g.wf[1][j] * g.af[1][0][i] * g.af[1][2][k];
+        if (a3 && i < n1 && j < n2) a3[((long long)k * n2 + j) * n1 + i] = g.wf[2][k] * g.af[2][0][i] * g.af[2][1][j];
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// a1: ghost fill along one axis d (step 1, L111).  periodic: copy from the opposite interior;
+// outflow: nearest interior cell into both ghosts (L260); reflect: mirror, normal flux negated
+// (L291); fixed: untouched (L289).  Axes e < d run over their ghost-extended range.
+// One thread per (ghost layer, side, other-axis position).
+// ------------------------------------------------------------------------------------------------
+__global__ void k_fill_ghosts(GridDev g, Fields4 U, int d) {
+    int lo[3], ext[3];
+    for (int e = 0; e < 3; ++e) {
+        lo[e] = (e < d) ? -g.gh[e] : 0;
+        ext[e] = (e < d) ? g.nt[e] : g.n[e];
+    }
+    const int ea = (d == 0) ? 1 : 0, eb = (d == 2) ? 1 : 2;  // the two other axes, ea < eb
+    const long long na = ext[ea], nb = ext[eb];
+    const long long tot = 4 * na * nb;
+    const int nd = g.n[d];
+    for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < tot; t += (long long)gridDim.x * blockDim.x) {
+        const int a = (int)(t % na);
+        const int b = (int)((t / na) % nb);
+        const int ls = (int)(t / (na * nb));  // 0..3
+        const int gl = ls & 1, side = ls >> 1;
+        const int kind = g.bc[2 * d + side];
+        if (kind == 3) continue;
+        const int dst = side == 0 ? -1 - gl : nd + gl;
+        int src;
+        if (kind == 0) src = side == 0 ? nd - 1 - gl : gl;
+        else if (kind == 1) src = side == 0 ? 0 : nd - 1;
+        else src = side == 0 ? gl : nd - 1 - gl;
+        int c[3];
+        c[ea] = lo[ea] + a;
+        c[eb] = lo[eb] + b;
+        c[d] = 0;
+        const long long base = (c[0] + g.gh[0]) * g.stride[0] + (c[1] + g.gh[1]) * g.stride[1] + (c[2] + g.gh[2]) * g.stride[2];
+        const long long id = base + dst * g.stride[d], is = base + src * g.stride[d];
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            double v = U.q[q][is];
+            if (kind == 2 && q == 1 + d) v = -v;
+            U.q[q][id] = v;
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// a9: opacities.  Power law kappa0 (rho/rho0)^a (T/T0)^b clipped (L299) or bilinear table of
+// log10 kappa on a uniform (log10 rho, log10 T) grid (L375; R-G14).
+// ------------------------------------------------------------------------------------------------
+// x^(n2/2) for integer n2: sqrt for the odd part, binary powering for the rest (uniform control flow).
+__device__ __forceinline__ double pow_half_int(double x, int n2) {
+    int m = n2 < 0 ? -n2 : n2;
+    double r = (m & 1) ? sqrt(x) : 1.0;
+    int k = m >> 1;
+    double base = x;
+    while (k) {
+        if (k & 1) r *= base;
+        base *= base;
+        k >>= 1;
+    }
+    return n2 < 0 ? 1.0 / r : r;
+}
+
+__device__ __forceinline__ double opacity_eval(const OpacDev& o, double rho, double T) {
+    if (!o.set) return 0.0;
+    if (o.kind == 0) {
+        const double xr = rho * o.irho0, xt = T * o.iT0;
+        double pr, pt;
+        if (o.n2a != INT_MIN) pr = pow_half_int(xr, o.n2a); else pr = pow(xr, o.a);
+        if (o.n2b != INT_MIN) pt = pow_half_int(xt, o.n2b); else pt = pow(xt, o.b);
+        double k = o.kappa0 * pr * pt;
+        k = dmax(k, o.kmin);
+        k = dmin(k, o.kmax);
+        return k;
+    }
+    double y = log10(T * o.T_unit);
+    y = dmin(dmax(y, o.lT_min), o.lT_max);
+    const double v = (y - o.lT_min) * o.sv;
+    int j0 = (int)floor(v);
+    j0 = max(0, min(j0, o.n_lT - 2));
+    const double tv = v - (double)j0;
+    double val;
+    if (o.n_lrho == 1) {
+        val = (1.0 - tv) * __ldg(o.tab + j0) + tv * __ldg(o.tab + j0 + 1);
+    } else {
+        double x = log10(rho * o.rho_unit);
+        x = dmin(dmax(x, o.lrho_min), o.lrho_max);
+        const double u = (x - o.lrho_min) * o.su;
+        int i0 = (int)floor(u);
+        i0 = max(0, min(i0, o.n_lrho - 2));
+        const double tu = u - (double)i0;
+        const double* p = o.tab + (long long)j0 * o.n_lrho + i0;
+        const double v00 = __ldg(p), v01 = __ldg(p + 1), v10 = __ldg(p + o.n_lrho), v11 = __ldg(p + o.n_lrho + 1);
+        val = (1.0 - tv) * ((1.0 - tu) * v00 + tu * v01) + tv * ((1.0 - tu) * v10 + tu * v11);
+    }
+    return exp10(val);
+}
+
+// ------------------------------------------------------------------------------------------------
+// Thick-limit pre-pass (Eq. 25-26; R-G7): per ghosted cell
+//   limd = 4 / (3 tau_cell),  tau_cell = rho chi dx,  chi = kappa_R + sigma (L89),
+//   dx = the cell's largest physical extent over the active dimensions.
+// Ghost cells take the value of the periodic image or of the nearest interior cell, so rho and T
+// ghosts are never read.  The sweeps use lim_face = max(limd_a, limd_b) = 4/(3 min(tau_a, tau_b)).
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(128) k_thick_limit(GridDev g, OpacDev oR, OpacDev oS, const double* __restrict__ rho,
+                                                     const double* __restrict__ T, double* __restrict__ lim) {
+    const int ii = blockIdx.x * blockDim.x + threadIdx.x;
+    if (ii >= g.nt[0]) return;
+    const int jj = blockIdx.y, kk = blockIdx.z;
+    int c[3] = {ii - g.gh[0], jj - g.gh[1], kk - g.gh[2]};
+#pragma unroll
+    for (int e = 0; e < 3; ++e) {
+        const int n = g.n[e];
+        if (c[e] < 0) c[e] = (g.bc[2 * e] == 0) ? c[e] + n : 0;
+        else if (c[e] >= n) c[e] = (g.bc[2 * e] == 0) ? c[e] - n : n - 1;
+    }
+    const long long src = (c[0] + g.gh[0]) * g.stride[0] + (c[1] + g.gh[1]) * g.stride[1] + (c[2] + g.gh[2]) * g.stride[2];
+    const long long dst = ii * g.stride[0] + jj * g.stride[1] + kk * g.stride[2];
+    const double r = rho[src], t = T[src];
+    const double chi = opacity_eval(oR, r, t) + opacity_eval(oS, r, t);
+    double dx = 0.0;
+#pragma unroll
+    for (int d = 0; d < 3; ++d)
+        if (g.gh[d] > 0) dx = dmax(dx, g.len[d][0][c[0]] * g.len[d][1][c[1]] * g.len[d][2][c[2]]);
+    const double tau = r * chi * dx;
+    lim[dst] = 4.0 / (3.0 * tau);
+}
+
+// ------------------------------------------------------------------------------------------------
+// a11: CFL (step 10, L120; R-G15).  rate_i = sum_{d active} chat max(|lam1|,|lam3|)/dl_d;
+// max over cells by warp shuffles -> one atomicMax per block on the bit pattern (rates are >= 0,
+// so the unsigned order equals the numeric order); the last block to finish writes
+// dt = cfl / rate and re-arms the scratch words.
+// ------------------------------------------------------------------------------------------------
+struct CflScratch {
+    unsigned long long rate_bits;
+    unsigned int blocks_done;
+    unsigned int pad;
+};
+
+__device__ __forceinline__ double cell_rate(const GridDev& g, double chat, double E, double F1, double F2, double F3, int i,
+                                            int j, int k) {
+    const double E2 = E * E;
+    const double Fq = fma(F3, F3, fma(F2, F2, F1 * F1));
+    const Closure c = closure_of(E, E2, Fq);
+    const double F[3] = {F1, F2, F3};
+    double sum = 0.0;
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+        if (g.gh[d] == 0) continue;
+        const double b = c.gE * F[d];
+        const double z2 = (2.0 * c.dE) * fma(-b, F[d], c.sE);
+        const double z = fsqrt(dmax(z2, kTiny));
+        const double il = g.ilen[d][0][i] * g.ilen[d][1][j] * g.ilen[d][2][k];
+        sum = fma((fabs(F[d]) + z) * c.rsE, il, sum);
+    }
+    return sum * chat;
+}
+
+__device__ __forceinline__ void block_max_to_global(double v, CflScratch* scr, double cfl, double* dt_out, unsigned nblocks) {
+    __shared__ double sred[32];
+    __shared__ bool last;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v = dmax(v, __shfl_xor_sync(0xffffffffu, v, o));
+    const int w = threadIdx.x >> 5, l = threadIdx.x & 31;
+    if (l == 0) sred[w] = v;
+    __syncthreads();
+    if (w == 0) {
+        const int nw = (blockDim.x + 31) >> 5;
+        v = l < nw ? sred[l] : 0.0;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v = dmax(v, __shfl_xor_sync(0xffffffffu, v, o));
+        if (l == 0) {
+            atomicMax(&scr->rate_bits, (unsigned long long)__double_as_longlong(v));
+            __threadfence();
+            const unsigned done = atomicAdd(&scr->blocks_done, 1u);
+            last = (done == nblocks - 1);
+        }
+    }
+    __syncthreads();
+    if (last && threadIdx.x == 0) {
+        __threadfence();
+        const unsigned long long bits = atomicExch(&scr->rate_bits, 0ull);
+        scr->blocks_done = 0;
+        *dt_out = cfl / __longlong_as_double((long long)bits);
+    }
+}
+
+__global__ void __launch_bounds__(256) k_cfl(GridDev g, double chat, const double* __restrict__ E, const double* __restrict__ F1,
+                                             const double* __restrict__ F2, const double* __restrict__ F3, CflScratch* scr,
+                                             double cfl, double* dt_out) {
+    // a persistent-style grid (a few blocks per SM) walks the rows, so that only O(1000) atomics are issued
+    const long long nrows = (long long)g.n[1] * g.n[2];
+    double rate = 0.0;
+    for (long long row = blockIdx.x; row < nrows; row += gridDim.x) {
+        const int j = (int)(row % g.n[1]), k = (int)(row / g.n[1]);
+        const long long rb = g.gh[0] * g.stride[0] + (j + g.gh[1]) * g.stride[1] + (k + g.gh[2]) * g.stride[2];
+        for (int i = threadIdx.x; i < g.n[0]; i += blockDim.x) {
+            const long long id = rb + i;
+            rate = dmax(rate, cell_rate(g, chat, E[id], F1[id], F2[id], F3[id], i, j, k));
+        }
+    }
+    block_max_to_global(rate, scr, cfl, dt_out, gridDim.x);
+}
+
+}  // namespace rtm1

@@ -1,0 +1,278 @@
+// rt_kernels_step.cuh — the fused reconstruct -> f-fix -> closure -> Riemann -> divergence sweeps
+// (a2-a7) and the floor + opacity + implicit coupling kernel (a8-a10).  SURVEY.md Sect. 8(a).
+//
+// Sweep design: face states, face fluxes and wave speeds never touch HBM.
+//  * x1 sweep: one warp owns 32 consecutive cells of one row; every lane builds both face states of
+//    its cell, the upper-face state moves one lane up and the area-weighted face flux one lane down
+//    by warp shuffles, so each closure and each Riemann flux is evaluated once; lanes 1..30 write.
+//  * x2 / x3 sweeps: lanes along x1 (coalesced), each thread marches along the sweep direction and
+//    carries the previous cell's upper-face state and the previous face flux in registers: every
+//    field value is loaded once per sweep, every face quantity is computed once.
+// All directions start from U^n (unsplit, step 7 L117): the x1 sweep writes U_out = U_in - ..., the
+// later sweeps accumulate into U_out while reading the stencil from U_in.
+#pragma once
+#include "rt_kernels_aux.cuh"
+
+namespace rtm1 {
+
+struct SweepArgs {
+    const double* uin[4];
+    double* uout[4];
+    const double* lim;  // thick-limit pre-pass array (ghosted) or nullptr
+    double dtc;         // dt * chat
+};
+
+constexpr double kInf = __builtin_huge_val();
+
+// ------------------------------------------------------------------------------------------------
+// x1 sweep.  Warp task = (chunk of 30 output cells, row).  FIRST: always (x1 is the first active
+// direction whenever n1 > 1).  CURVI: area weights + geometric sources (R-G9) from the
+// cell-centred closure:  cyl: S(F^R) = +chat P^{phiphi}<1/R>, S(F^phi) = -chat P^{Rphi}<1/R>
+//   sph: S(F^r) = chat (P^{thth}+P^{phph})<1/r>, S(F^th) = chat(-P^{rth} + <cot>P^{phph})<1/r>,
+//        S(F^ph) = chat(-P^{rph} - <cot>P^{thph})<1/r>.
+// ------------------------------------------------------------------------------------------------
+constexpr int kXOut = 30;  // output cells per warp
+
+template <bool HLL, bool THICK, bool CURVI>
+__global__ void __launch_bounds__(128) k_sweep_x(const __grid_constant__ GridDev g, const __grid_constant__ SweepArgs a,
+                                                 int nchunk, long long ntask) {
+    const int lane = threadIdx.x & 31;
+    const long long task = (long long)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    if (task >= ntask) return;
+    const int ch = (int)(task % nchunk);
+    const long long row = task / nchunk;
+    const int j = (int)(row % g.n[1]), k = (int)(row / g.n[1]);
+    const int n1 = g.n[0];
+    const int i = ch * kXOut - 1 + lane;      // this lane's cell, -1 .. n1
+    const int ic = i > n1 ? n1 : i;           // clamp idle lanes onto a valid cell
+    const long long id = (ic + g.gh[0]) + (j + g.gh[1]) * g.stride[1] + (k + g.gh[2]) * g.stride[2];
+
+    double q0[4], dm[4], dp[4];
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+        const double* __restrict__ u = a.uin[q];
+        const double um = u[id - 1], uc = u[id], up = u[id + 1];
+        q0[q] = uc;
+        dm[q] = uc - um;
+        dp[q] = up - uc;
+    }
+    double limd = kInf;
+    if (THICK) limd = dmax(a.lim[id - 1], a.lim[id]);
+
+    State lo, hi;
+    cell_faces<0, HLL>(q0, dm, dp, true, true, lo, hi);
+
+    // left state of this lane's lower face = upper-face state of the lane below
+    State L;
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+        L.U[q] = __shfl_up_sync(0xffffffffu, hi.U[q], 1);
+        L.G[q] = __shfl_up_sync(0xffffffffu, hi.G[q], 1);
+    }
+    if (HLL) {
+        L.lm = __shfl_up_sync(0xffffffffu, hi.lm, 1);
+        L.lp = __shfl_up_sync(0xffffffffu, hi.lp, 1);
+    }
+    double fl[4];
+    riemann<HLL>(L, lo, limd, fl);
+    if (CURVI) {
+        const double w = g.wf[0][ic < 0 ? 0 : ic];
+#pragma unroll
+        for (int q = 0; q < 4; ++q) fl[q] *= w;
+    }
+    double fu[4];
+#pragma unroll
+    for (int q = 0; q < 4; ++q) fu[q] = __shfl_down_sync(0xffffffffu, fl[q], 1);
+
+    if (lane >= 1 && lane <= kXOut && i < n1) {
+        const double coef = a.dtc * g.cg[0][0][i] * g.cg[0][1][j] * g.cg[0][2][k];
+        double out[4];
+#pragma unroll
+        for (int q = 0; q < 4; ++q) out[q] = fma(-coef, fu[q] - fl[q], q0[q]);
+        if (CURVI) {
+            const double E2 = q0[0] * q0[0];
+            const double F2 = fma(q0[3], q0[3], fma(q0[2], q0[2], q0[1] * q0[1]));
+            const Closure c = closure_of(q0[0], E2, F2);
+            const double s = a.dtc * g.invr[i];
+            if (g.geometry == 1) {
+                out[1] = fma(s, fma(c.gE * q0[2], q0[2], c.dE), out[1]);
+                out[2] = fma(-s, c.gE * q0[1] * q0[2], out[2]);
+            } else {
+                const double ct = g.cot[j];
+                const double Ptt = fma(c.gE * q0[2], q0[2], c.dE);
+                const double Ppp = fma(c.gE * q0[3], q0[3], c.dE);
+                const double Prt = c.gE * q0[1] * q0[2];
+                const double Prp = c.gE * q0[1] * q0[3];
+                const double Ptp = c.gE * q0[2] * q0[3];
+                out[1] = fma(s, Ptt + Ppp, out[1]);
+                out[2] = fma(s, fma(ct, Ppp, -Prt), out[2]);
+                out[3] = fma(-s, fma(ct, Ptp, Prp), out[3]);
+            }
+        }
+#pragma unroll
+        for (int q = 0; q < 4; ++q) a.uout[q][id] = out[q];
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// x2 / x3 sweeps: marching.  Thread = (i, o, segment); o = the other transverse index (k for D = 1,
+// j for D = 2); the segment covers cells [ca, cb) along D.  Step c in [ca-1, cb] builds the face
+// states of cell c (only the upper one at c = ca-1, only the lower one at c = cb), the flux at the
+// lower face of cell c, and then finishes cell c-1.  Accumulates into U_out (never the first sweep).
+// ------------------------------------------------------------------------------------------------
+template <int D, bool HLL, bool THICK, bool CURVI>
+__global__ void __launch_bounds__(128) k_sweep_march(const __grid_constant__ GridDev g, const __grid_constant__ SweepArgs a,
+                                                     int seglen) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= g.n[0]) return;
+    constexpr int EO = (D == 1) ? 2 : 1;
+    const int o = blockIdx.y;
+    const int nd = g.n[D];
+    const int ca = blockIdx.z * seglen;
+    const int cb = min(ca + seglen, nd);
+    const long long S = g.stride[D];
+    // index of the cell with sweep coordinate 0
+    const long long id0 = (i + g.gh[0]) + (long long)g.gh[D] * S + (long long)(o + g.gh[EO]) * g.stride[EO];
+    const double K = a.dtc * g.cg[D][0][i] * g.cg[D][EO][o];
+    const double* __restrict__ cgd = g.cg[D][D];
+    const double* __restrict__ wfd = g.wf[D];
+
+    long long p = id0 + (long long)(ca - 1) * S;
+    double qc[4], dm[4], qn[4];
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+        const double* __restrict__ u = a.uin[q];
+        qc[q] = u[p];
+        dm[q] = qc[q] - u[p - S];
+        qn[q] = u[p + S];
+    }
+    double limp = kInf, limc = kInf;
+    if (THICK) limc = a.lim[p];
+
+    State hiPrev;
+    double Fprev[4] = {0.0, 0.0, 0.0, 0.0};
+#pragma unroll 1
+    for (int c = ca - 1; c <= cb; ++c, p += S) {
+        // loads issued first: next stencil value, next limiter, accumulation base of cell c-1
+        double qnn[4], base[4], limn = kInf;
+        if (c < cb) {
+#pragma unroll
+            for (int q = 0; q < 4; ++q) qnn[q] = a.uin[q][p + 2 * S];
+            if (THICK) limn = a.lim[p + S];
+        }
+        if (c > ca) {
+#pragma unroll
+            for (int q = 0; q < 4; ++q) base[q] = a.uout[q][p - S];
+        }
+        double dp[4];
+#pragma unroll
+        for (int q = 0; q < 4; ++q) dp[q] = qn[q] - qc[q];
+        State lo, hi;
+        cell_faces<D, HLL>(qc, dm, dp, c >= ca, c < cb, lo, hi);
+        if (c >= ca) {
+            double fl[4];
+            riemann<HLL>(hiPrev, lo, THICK ? dmax(limp, limc) : kInf, fl);
+            if (CURVI) {
+                const double w = wfd[c];
+#pragma unroll
+                for (int q = 0; q < 4; ++q) fl[q] *= w;
+            }
+            if (c > ca) {
+                const double coef = K * cgd[c - 1];
+#pragma unroll
+                for (int q = 0; q < 4; ++q) a.uout[q][p - S] = fma(-coef, fl[q] - Fprev[q], base[q]);
+            }
+#pragma unroll
+            for (int q = 0; q < 4; ++q) Fprev[q] = fl[q];
+        }
+        hiPrev = hi;
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            dm[q] = dp[q];
+            qc[q] = qn[q];
+            qn[q] = qnn[q];
+        }
+        limp = limc;
+        limc = limn;
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// a8-a10: floor / clip (L81, L250; R-G11), opacities, implicit coupling (Eq. 29-33; R-G12):
+//   g_r = dt chat kappa_P rho, g = dt c kappa_P rho, C_v = rho c_v, det = C_v (1 + g_r) + 4 g a_R T^3
+//   E' = [E (C_v + 4 g a_R T^3) + g_r C_v a_R T^4] / det
+//   T' = [(1 + g_r) C_v T + 3 g a_R T^4 + g E] / det
+//   F' = F / (1 + dt chat chi rho) (Eq. 30);   m' = m - (F' - F)/chat (Eq. 28).
+// ------------------------------------------------------------------------------------------------
+struct ImplicitArgs {
+    double* U[4];
+    const double* rho;
+    double* T;
+    double* mom[3];
+    double dt;
+    int feedback;
+    int same_PR;  // kappa_P and kappa_R are the same law: evaluate once
+    unsigned long long* counters;  // [0] floor activations, [1] clip activations
+};
+
+template <bool FEEDBACK>
+__global__ void __launch_bounds__(128) k_implicit(const __grid_constant__ GridDev g, const __grid_constant__ ParamsDev par,
+                                                  const __grid_constant__ OpacDev oP, const __grid_constant__ OpacDev oR,
+                                                  const __grid_constant__ OpacDev oS, const __grid_constant__ ImplicitArgs a) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int j = blockIdx.y, k = blockIdx.z;
+    bool floored = false, clipped = false;
+    if (i < g.n[0]) {
+        const long long id = (i + g.gh[0]) + (j + g.gh[1]) * g.stride[1] + (k + g.gh[2]) * g.stride[2];
+        double E = a.U[0][id];
+        double F[3] = {a.U[1][id], a.U[2][id], a.U[3][id]};
+        const double rho = a.rho[id];
+        const double T0 = a.T[id];
+        double m[3];
+        if (FEEDBACK) {
+#pragma unroll
+            for (int q = 0; q < 3; ++q) m[q] = a.mom[q][id];
+        }
+        if (E < par.E_floor) {
+            E = par.E_floor;
+            floored = true;
+        }
+        const double F2 = fma(F[2], F[2], fma(F[1], F[1], F[0] * F[0]));
+        if (F2 > E * E) {
+            const double sc = E * rsqrt(F2);
+#pragma unroll
+            for (int q = 0; q < 3; ++q) F[q] *= sc;
+            clipped = true;
+        }
+        const double kP = opacity_eval(oP, rho, T0);
+        const double kR = a.same_PR ? kP : opacity_eval(oR, rho, T0);
+        const double chi = kR + opacity_eval(oS, rho, T0);
+        const double gr = a.dt * par.chat * kP * rho;
+        const double gg = a.dt * par.c * kP * rho;
+        const double Cv = rho * par.c_v;
+        const double aT3 = par.a_R * T0 * T0 * T0;
+        const double aT4 = aT3 * T0;
+        const double det = fma(Cv, 1.0 + gr, 4.0 * gg * aT3);
+        const double idet = frcp(det);
+        const double En = fma(E, fma(4.0 * gg, aT3, Cv), gr * Cv * aT4) * idet;
+        const double Tn = fma((1.0 + gr) * Cv, T0, fma(3.0 * gg, aT4, gg * E)) * idet;
+        const double idamp = frcp(fma(a.dt * par.chat * chi, rho, 1.0));
+        a.U[0][id] = En;
+        a.T[id] = Tn;
+        const double ichat = 1.0 / par.chat;
+#pragma unroll
+        for (int q = 0; q < 3; ++q) {
+            const double Fn = F[q] * idamp;
+            if (FEEDBACK) a.mom[q][id] = fma(-(Fn - F[q]), ichat, m[q]);
+            a.U[1 + q][id] = Fn;
+        }
+    }
+    // rare: count floor / clip activations (debug counters, SURVEY.md Sect. 8(d) "Parity")
+    const unsigned mf = __ballot_sync(0xffffffffu, floored), mc = __ballot_sync(0xffffffffu, clipped);
+    if ((mf | mc) && (threadIdx.x & 31) == 0) {
+        if (mf) atomicAdd(&a.counters[0], (unsigned long long)__popc(mf));
+        if (mc) atomicAdd(&a.counters[1], (unsigned long long)__popc(mc));
+    }
+}
+
+}  // namespace rtm1

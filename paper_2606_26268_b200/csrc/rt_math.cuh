@@ -1,0 +1,200 @@
+// rt_math.cuh — fp64 device arithmetic of the gray-M1 sub-step (sm_100a).
+//
+// The sweeps sit at the fp64-pipe ridge of B200, so the formulas of
+// PAPER.md Sect. 2.1/2.6 are restated in a division-lean form.  With s = sqrt(4 - 3 f^2) (Eq. 13,
+// L75) the Levermore factor is xi = (3 + 4f^2)/(5 + 2s) = (5 - 2s)/3, hence
+//     (1 - xi)/2 = (s - 1)/3,     (3 xi - 1)/(2 f^2) = 3/(2 + s),
+//     P^{ij} = (s-1)/3 E delta^{ij} + 3/(2+s) F^i F^j / E                       (Eq. 11-12)
+//     zeta^2 = 2/3 (s - 1)(s - 3 mu^2/(2+s)),  mu = F^d/E,  lambda_{1,3} = (mu -+ zeta)/s   (Eq. 22, 24)
+// and everything is carried multiplied by E ("E-scaled": sE = sqrt(4E^2 - 3|F|^2) = E s) so that no
+// 1/E is needed:  P^{id} = (sE - E)/3 delta^{id} + gE F^i F^d,  gE = 3/(2E + sE),
+//                 zE^2 = 2/3 (sE - E)(sE - gE (F^d)^2),  lambda_{1,3} = (F^d -+ zE)/sE.
+// Reciprocals / square roots are MUFU seeds (rcp.approx / rsqrt.approx, >= 20 bits) plus two
+// Newton steps: <= ~1-2 ulp, no slow path.  Valid for NORMAL-range operands whose squares are
+// normal too (|x| in ~[1e-150, 1e150]); include/rt.h states that as the field range.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace rtm1 {
+
+__device__ __forceinline__ double rcp_seed(double x) {
+    double r;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
+    return r;
+}
+__device__ __forceinline__ double rsqrt_seed(double x) {
+    double r;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
+    return r;
+}
+
+// 1/x: seed + 2 Newton steps (4 DFMA).
+__device__ __forceinline__ double frcp(double x) {
+    double r = rcp_seed(x);
+    double e = fma(-x, r, 1.0);
+    r = fma(r, e, r);
+    e = fma(-x, r, 1.0);
+    r = fma(r, e, r);
+    return r;
+}
+
+// s = sqrt(x) and rs = 1/sqrt(x) together (coupled Newton, 8 fp64 ops + 1 for rs).
+__device__ __forceinline__ void fsqrt_rsqrt(double x, double& s, double& rs) {
+    double y = rsqrt_seed(x);
+    double g = x * y, h = 0.5 * y;
+    double t = fma(-h, g, 0.5);
+    g = fma(g, t, g);
+    h = fma(h, t, h);
+    t = fma(-h, g, 0.5);
+    g = fma(g, t, g);
+    h = fma(h, t, h);
+    s = g;
+    rs = h + h;
+}
+
+// sqrt(x) alone (7 fp64 ops); x must be > 0 (callers clamp at a tiny positive number).
+__device__ __forceinline__ double fsqrt(double x) {
+    double y = rsqrt_seed(x);
+    double g = x * y, h = 0.5 * y;
+    double t = fma(-h, g, 0.5);
+    g = fma(g, t, g);
+    h = fma(h, t, h);
+    double d = fma(-g, g, x);
+    return fma(d, h, g);
+}
+
+__device__ __forceinline__ double dmin(double a, double b) { return a < b ? a : b; }
+__device__ __forceinline__ double dmax(double a, double b) { return a > b ? a : b; }
+
+constexpr double kTiny = 1.0e-200;  // positive clamp under square roots (zeta^2 = 0 at f = 1)
+constexpr double kTinySpeed = 1.0e-30;  // HLL: S_R >= +tiny, S_L <= -tiny  ==> den > 0 always (R-G8)
+
+// One face (or cell) state with what the Riemann solver needs from it.
+struct State {
+    double U[4];   // E, F1, F2, F3
+    double G[4];   // physical flux through direction D divided by chat: (F^D, P^{1D}, P^{2D}, P^{3D})
+    double lm, lp; // lambda_1 (minus) and lambda_3 (plus) along D, in units of chat (HLL only)
+};
+
+// E-scaled closure pieces shared by flux, wave speeds and sources.
+struct Closure {
+    double sE;   // E sqrt(4 - 3 f^2)
+    double rsE;  // 1 / sE
+    double gE;   // 3 / (2E + sE)
+    double dE;   // (sE - E)/3   = (1 - xi)/2 E
+};
+
+// E2 = E*E and F2 = |F|^2 are passed in because the callers have them already.
+// f is capped at 1 (Eq. 14; round-off guard, R-G4): |F|^2 enters as min(F2, E2).
+__device__ __forceinline__ Closure closure_of(double E, double E2, double F2) {
+    Closure c;
+    double m = dmin(F2, E2);
+    double w = fma(-3.0, m, 4.0 * E2);
+    fsqrt_rsqrt(w, c.sE, c.rsE);
+    c.gE = 3.0 * frcp(fma(2.0, E, c.sE));
+    c.dE = (c.sE - E) * (1.0 / 3.0);
+    return c;
+}
+
+// Flux through direction D (Eq. 5-6, without the factor chat) and, for HLL, lambda_{1,3}.
+template <int D, bool WAVES>
+__device__ __forceinline__ void flux_and_speeds(State& st, double E2, double F2) {
+    const double E = st.U[0];
+    const Closure c = closure_of(E, E2, F2);
+    const double Fd = st.U[1 + D];
+    const double b = c.gE * Fd;
+    st.G[0] = Fd;
+    st.G[1] = b * st.U[1];
+    st.G[2] = b * st.U[2];
+    st.G[3] = b * st.U[3];
+    st.G[1 + D] += c.dE;
+    if (WAVES) {
+        double z2 = (2.0 * c.dE) * fma(-b, Fd, c.sE);  // 2/3 (sE - E)(sE - gE Fd^2)
+        double z = fsqrt(dmax(z2, kTiny));
+        st.lm = (Fd - z) * c.rsE;
+        st.lp = (Fd + z) * c.rsE;
+    } else {
+        st.lm = 0.0;
+        st.lp = 0.0;
+    }
+}
+
+// PLM + van Leer limiter (Eq. 17-18; R-G3): HALF slope  h = dm dp/(dm + dp) if dm dp > 0.
+__device__ __forceinline__ double half_slope(double dm, double dp) {
+    double pr = dm * dp;
+    double h = pr * frcp(dm + dp);
+    return pr > 0.0 ? h : 0.0;
+}
+
+// f-preserving face state (Eq. 19-21; R-G4).  Uc = cell value, invEc = 1/E_c,
+// Ec2 = E_c^2, F2c = |F_c|^2; on entry st.U holds the reconstructed R(U); on exit the face state.
+// Returns through E2f/F2f the squares of the final face state.
+__device__ __forceinline__ void fpreserve(State& st, const double Uc[4], double invEc, double Ec2, double F2c,
+                                          double& E2f, double& F2f) {
+    const double Ef = st.U[0];
+    E2f = Ef * Ef;
+    double F2r = fma(st.U[3], st.U[3], fma(st.U[2], st.U[2], st.U[1] * st.U[1]));
+    bool keep = (F2r <= E2f) && (F2r * Ec2 > F2c * E2f);
+    double r = Ef * invEc;
+    st.U[1] = keep ? st.U[1] : Uc[1] * r;
+    st.U[2] = keep ? st.U[2] : Uc[2] * r;
+    st.U[3] = keep ? st.U[3] : Uc[3] * r;
+    F2f = keep ? F2r : F2c * (r * r);
+}
+
+// Riemann flux (L150; R-G5, G6, G8) divided by chat, from left state L and right state R.
+// limd = 4/(3 tau_face) (Eq. 25-26 in units of chat; +inf when the thick limit is off).
+template <bool HLL>
+__device__ __forceinline__ void riemann(const State& L, const State& R, double limd, double flux[4]) {
+    double sR, sL;
+    if (HLL) {
+        sL = dmin(dmin(L.lm, R.lm), 0.0);
+        sR = dmax(dmax(L.lp, R.lp), 0.0);
+        sL = dmax(sL, -limd);
+        sR = dmin(sR, limd);
+        sL = dmin(sL, -kTinySpeed);
+        sR = dmax(sR, kTinySpeed);
+    } else {
+        sR = dmax(dmin(1.0, limd), kTinySpeed);  // GLF: alpha = min(chat, 4 chat/(3 tau))
+        sL = -sR;
+    }
+    const double rden = frcp(sR - sL);
+    const double sRL = sR * sL;
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+        double num = fma(sR, L.G[q], fma(-sL, R.G[q], sRL * (R.U[q] - L.U[q])));
+        flux[q] = num * rden;
+    }
+}
+
+// Both face states of one cell along D from the cell value q0 and the two one-sided differences.
+// lo = state at the cell's lower face (RIGHT state of face c-1/2), hi = state at its upper face
+// (LEFT state of face c+1/2).  WANT_LO / WANT_HI are warp-uniform run-time flags.
+template <int D, bool HLL>
+__device__ __forceinline__ void cell_faces(const double q0[4], const double dm[4], const double dp[4], bool want_lo,
+                                           bool want_hi, State& lo, State& hi) {
+    double h[4];
+#pragma unroll
+    for (int q = 0; q < 4; ++q) h[q] = half_slope(dm[q], dp[q]);
+    const double Ec = q0[0];
+    const double Ec2 = Ec * Ec;
+    const double F2c = fma(q0[3], q0[3], fma(q0[2], q0[2], q0[1] * q0[1]));
+    const double invEc = frcp(Ec);
+    if (want_lo) {
+#pragma unroll
+        for (int q = 0; q < 4; ++q) lo.U[q] = q0[q] - h[q];
+        double E2f, F2f;
+        fpreserve(lo, q0, invEc, Ec2, F2c, E2f, F2f);
+        flux_and_speeds<D, HLL>(lo, E2f, F2f);
+    }
+    if (want_hi) {
+#pragma unroll
+        for (int q = 0; q < 4; ++q) hi.U[q] = q0[q] + h[q];
+        double E2f, F2f;
+        fpreserve(hi, q0, invEc, Ec2, F2c, E2f, F2f);
+        flux_and_speeds<D, HLL>(hi, E2f, F2f);
+    }
+}
+
+}  // namespace rtm1

@@ -1,0 +1,326 @@
+"""Thin ctypes binding of include/rt.h (librt_m1.so).  Argument marshalling only: every step of the
+radiation sub-step runs in the CUDA kernels behind the C ABI.  PyTorch supplies device memory and
+streams; nothing here computes on the CPU and there is no fallback: a missing library or a missing
+GPU raises.
+
+Function names mirror the C ABI (rt_grid_create, rt_set_params, rt_set_opacity, rt_explicit_step,
+rt_implicit_step, rt_cfl_dt, ...); `Grid` is a small handle owner around them.
+"""
+import ctypes as C
+import os
+
+import numpy as np
+import torch
+
+from . import build as _build
+
+CARTESIAN, CYLINDRICAL, SPHERICAL = 0, 1, 2
+BC_PERIODIC, BC_OUTFLOW, BC_REFLECT, BC_FIXED = 0, 1, 2, 3
+SOLVER_HLL, SOLVER_GLF = 0, 1
+OPAC_PLANCK, OPAC_ROSSELAND, OPAC_SCATTER = 0, 1, 2
+OK, ERR_INVALID_ARG, ERR_BAD_STATE, ERR_CUDA, ERR_NOT_FINITE = 0, 1, 2, 3, 4
+NGHOST = 2
+
+_dp = C.POINTER(C.c_double)
+
+
+class Params(C.Structure):
+    _fields_ = [("chat", C.c_double), ("c", C.c_double), ("a_R", C.c_double), ("c_v", C.c_double),
+                ("E_floor", C.c_double), ("solver", C.c_int32), ("thick_limit", C.c_int32),
+                ("feedback_momentum", C.c_int32)]
+
+
+class Opacity(C.Structure):
+    _fields_ = [("kind", C.c_int32), ("kappa0", C.c_double), ("rho0", C.c_double), ("T0", C.c_double),
+                ("a", C.c_double), ("b", C.c_double), ("kmin", C.c_double), ("kmax", C.c_double),
+                ("n_lrho", C.c_int32), ("n_lT", C.c_int32), ("lrho_min", C.c_double), ("lrho_max", C.c_double),
+                ("lT_min", C.c_double), ("lT_max", C.c_double), ("rho_unit", C.c_double), ("T_unit", C.c_double),
+                ("log10_kappa", _dp)]
+
+
+class RtError(RuntimeError):
+    def __init__(self, call, status, message=""):
+        self.status = status
+        super().__init__("%s failed with status %d%s" % (call, status, (": " + message) if message else ""))
+
+
+_lib = None
+
+_SIGNATURES = {
+    "rt_grid_create": (C.c_int32, [C.c_int32, C.POINTER(C.c_int32), C.c_int32, _dp, _dp, _dp, C.POINTER(C.c_int32),
+                                   C.c_void_p, C.POINTER(C.c_void_p)]),
+    "rt_grid_destroy": (C.c_int32, [C.c_void_p]),
+    "rt_grid_get_metrics": (C.c_int32, [C.c_void_p, _dp, _dp, _dp, _dp]),
+    "rt_set_params": (C.c_int32, [C.c_void_p, C.POINTER(Params)]),
+    "rt_set_opacity": (C.c_int32, [C.c_void_p, C.c_int32, C.POINTER(Opacity)]),
+    "rt_fill_ghosts": (C.c_int32, [C.c_void_p, C.POINTER(C.c_void_p)]),
+    "rt_explicit_step": (C.c_int32, [C.c_void_p, C.c_double, C.c_void_p, C.c_void_p, C.POINTER(C.c_void_p),
+                                     C.POINTER(C.c_void_p)]),
+    "rt_implicit_step": (C.c_int32, [C.c_void_p, C.c_double, C.c_void_p, C.c_void_p, C.POINTER(C.c_void_p),
+                                     C.POINTER(C.c_void_p)]),
+    "rt_cfl_dt": (C.c_int32, [C.c_void_p, C.POINTER(C.c_void_p), C.c_double, _dp]),
+    "rt_cfl_dt_async": (C.c_int32, [C.c_void_p, C.POINTER(C.c_void_p), C.c_double, C.c_void_p]),
+    "rt_get_floor_counts": (C.c_int32, [C.c_void_p, C.POINTER(C.c_int64), C.POINTER(C.c_int64)]),
+    "rt_get_launch_count": (C.c_int64, [C.c_void_p]),
+    "rt_set_tuning": (C.c_int32, [C.c_void_p, C.c_int32, C.c_int32]),
+    "rt_last_error": (C.c_char_p, [C.c_void_p]),
+}
+
+
+def exported_symbols():
+    """names the C ABI must export (used by the CPU-side load test)"""
+    return sorted(_SIGNATURES)
+
+
+def lib():
+    """load (building first if needed) librt_m1.so; raises if it cannot be had"""
+    global _lib
+    if _lib is None:
+        path = _build.build()
+        if not os.path.exists(path):
+            raise RuntimeError("librt_m1.so is missing and could not be built")
+        L = C.CDLL(path)
+        for name, (res, args) in _SIGNATURES.items():
+            fn = getattr(L, name)  # AttributeError if the symbol is missing: loud by design
+            fn.restype = res
+            fn.argtypes = args
+        _lib = L
+    return _lib
+
+
+def _check_field(t, shape, name):
+    if not isinstance(t, torch.Tensor):
+        raise TypeError("%s must be a torch.Tensor on the GPU" % name)
+    if not t.is_cuda:
+        raise RuntimeError("%s is not a CUDA tensor: this library has no CPU path" % name)
+    if t.dtype != torch.float64 or not t.is_contiguous() or tuple(t.shape) != tuple(shape):
+        raise ValueError("%s must be contiguous float64 of shape %s (got %s %s)" % (name, tuple(shape), t.dtype,
+                                                                                     tuple(t.shape)))
+
+
+def _ptr_array(tensors):
+    return (C.c_void_p * len(tensors))(*[t.data_ptr() for t in tensors])
+
+
+def make_params(chat=1.0, c=1.0, a_R=1.0, c_v=1.5, E_floor=0.0, solver=SOLVER_HLL, thick_limit=0,
+                feedback_momentum=0):
+    return Params(chat, c, a_R, c_v, E_floor, solver, thick_limit, feedback_momentum)
+
+
+def make_power_law(kappa0, a=0.0, b=0.0, rho0=1.0, T0=1.0, kmin=0.0, kmax=np.inf):
+    o = Opacity()
+    o.kind = 0
+    o.kappa0, o.rho0, o.T0, o.a, o.b, o.kmin, o.kmax = kappa0, rho0, T0, a, b, kmin, kmax
+    o.rho_unit = o.T_unit = 1.0
+    return o
+
+
+def make_table(log10_kappa, lrho_range, lT_range, rho_unit=1.0, T_unit=1.0):
+    tab = np.ascontiguousarray(np.asarray(log10_kappa, dtype=np.float64))
+    if tab.ndim != 2:
+        raise ValueError("table must be 2-D (n_lT, n_lrho)")
+    o = Opacity()
+    o.kind = 1
+    o.n_lT, o.n_lrho = tab.shape
+    o.lrho_min, o.lrho_max = lrho_range
+    o.lT_min, o.lT_max = lT_range
+    o.rho_unit, o.T_unit = rho_unit, T_unit
+    o.rho0 = o.T0 = 1.0
+    o.log10_kappa = tab.ctypes.data_as(_dp)
+    o._keep = tab
+    return o
+
+
+def opacity_from_spec(spec):
+    """translate the plain-Python opacity description of rt_workloads into the C struct"""
+    if spec["kind"] == "power":
+        return make_power_law(spec["kappa0"], spec["a"], spec["b"], spec["rho0"], spec["T0"], spec["kmin"],
+                              spec["kmax"])
+    return make_table(spec["log10_kappa"], spec["lrho_range"], spec["lT_range"], spec["rho_unit"], spec["T_unit"])
+
+
+class Grid:
+    """Owner of one rt_grid handle.  All field arguments are CUDA float64 tensors of shape `self.shape`
+    (ghosted, (nt3, nt2, nt1)); work is enqueued on the stream that was current at construction."""
+
+    def __init__(self, geometry, n, x1f, x2f, x3f, bc, nghost=NGHOST, device="cuda:0", stream=None):
+        if not torch.cuda.is_available():
+            raise RuntimeError("no CUDA device: paper_2606_26268_b200 has no CPU path")
+        self.device = torch.device(device)
+        self.n = tuple(int(v) for v in n)
+        self.gh = tuple(nghost if v > 1 else 0 for v in self.n)
+        self.nt = tuple(v + 2 * g for v, g in zip(self.n, self.gh))
+        self.shape = (self.nt[2], self.nt[1], self.nt[0])
+        self.geometry = int(geometry)
+        self.bc = tuple(int(b) for b in bc)
+        xs = [np.ascontiguousarray(np.asarray(x, dtype=np.float64)) for x in (x1f, x2f, x3f)]
+        for d in range(3):
+            if xs[d].shape != (self.n[d] + 1,):
+                raise ValueError("x%df must have n[%d] + 1 entries" % (d + 1, d))
+        with torch.cuda.device(self.device):
+            self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+            h = C.c_void_p()
+            rc = lib().rt_grid_create(self.geometry, (C.c_int32 * 3)(*self.n), int(nghost),
+                                      xs[0].ctypes.data_as(_dp), xs[1].ctypes.data_as(_dp), xs[2].ctypes.data_as(_dp),
+                                      (C.c_int32 * 6)(*self.bc), C.c_void_p(self.stream.cuda_stream), C.byref(h))
+        if rc != OK:
+            raise RtError("rt_grid_create", rc)
+        self._h = h
+
+    def __del__(self):
+        h = getattr(self, "_h", None)
+        if h and _lib is not None:
+            _lib.rt_grid_destroy(h)
+            self._h = None
+
+    # ------------------------------------------------------------------ helpers
+    def _raise(self, call, rc):
+        msg = lib().rt_last_error(self._h)
+        raise RtError(call, rc, msg.decode() if msg else "")
+
+    @property
+    def interior(self):
+        return tuple(slice(g, g + n) for g, n in zip(self.gh[::-1], self.n[::-1]))
+
+    @property
+    def ncells(self):
+        return self.n[0] * self.n[1] * self.n[2]
+
+    def zeros(self):
+        return torch.zeros(self.shape, dtype=torch.float64, device=self.device)
+
+    def to_device(self, a):
+        return torch.as_tensor(np.ascontiguousarray(a, dtype=np.float64)).to(self.device)
+
+    # ------------------------------------------------------------------ the C ABI, one method per call
+    def set_params(self, params):
+        rc = lib().rt_set_params(self._h, C.byref(params))
+        if rc != OK:
+            self._raise("rt_set_params", rc)
+        self.params = params
+
+    def set_opacity(self, which, o):
+        rc = lib().rt_set_opacity(self._h, int(which), C.byref(o))
+        if rc != OK:
+            self._raise("rt_set_opacity", rc)
+
+    def set_tuning(self, march_len=0):
+        rc = lib().rt_set_tuning(self._h, int(march_len), 0)
+        if rc != OK:
+            self._raise("rt_set_tuning", rc)
+
+    def metrics(self):
+        n1, n2, n3 = self.n
+        vol = np.empty((n3, n2, n1))
+        a1 = np.empty((n3, n2, n1 + 1))
+        a2 = np.empty((n3, n2 + 1, n1))
+        a3 = np.empty((n3 + 1, n2, n1))
+        rc = lib().rt_grid_get_metrics(self._h, *[a.ctypes.data_as(_dp) for a in (vol, a1, a2, a3)])
+        if rc != OK:
+            self._raise("rt_grid_get_metrics", rc)
+        return vol, a1, a2, a3
+
+    def fill_ghosts(self, U):
+        for q, t in enumerate(U):
+            _check_field(t, self.shape, "U[%d]" % q)
+        rc = lib().rt_fill_ghosts(self._h, _ptr_array(U))
+        if rc != OK:
+            self._raise("rt_fill_ghosts", rc)
+
+    def explicit_step(self, dt, rho, T, U_in, U_out):
+        for name, t in (("rho", rho), ("T", T)):
+            if t is not None:
+                _check_field(t, self.shape, name)
+        for q in range(4):
+            _check_field(U_in[q], self.shape, "U_in[%d]" % q)
+            _check_field(U_out[q], self.shape, "U_out[%d]" % q)
+        rc = lib().rt_explicit_step(self._h, float(dt), rho.data_ptr() if rho is not None else None,
+                                    T.data_ptr() if T is not None else None, _ptr_array(U_in), _ptr_array(U_out))
+        if rc != OK:
+            self._raise("rt_explicit_step", rc)
+
+    def implicit_step(self, dt, rho, T, mom, U):
+        _check_field(rho, self.shape, "rho")
+        _check_field(T, self.shape, "T")
+        for q in range(4):
+            _check_field(U[q], self.shape, "U[%d]" % q)
+        if mom is not None:
+            for q in range(3):
+                _check_field(mom[q], self.shape, "mom[%d]" % q)
+        rc = lib().rt_implicit_step(self._h, float(dt), rho.data_ptr(), T.data_ptr(),
+                                    _ptr_array(mom) if mom is not None else None, _ptr_array(U))
+        if rc != OK:
+            self._raise("rt_implicit_step", rc)
+
+    def cfl_dt(self, U, cfl):
+        for q in range(4):
+            _check_field(U[q], self.shape, "U[%d]" % q)
+        out = C.c_double()
+        rc = lib().rt_cfl_dt(self._h, _ptr_array(U), float(cfl), C.byref(out))
+        if rc != OK:
+            self._raise("rt_cfl_dt", rc)
+        return out.value
+
+    def cfl_dt_async(self, U, cfl, dt_device):
+        for q in range(4):
+            _check_field(U[q], self.shape, "U[%d]" % q)
+        if not (dt_device.is_cuda and dt_device.dtype == torch.float64 and dt_device.numel() >= 1):
+            raise ValueError("dt_device must be a CUDA float64 tensor")
+        rc = lib().rt_cfl_dt_async(self._h, _ptr_array(U), float(cfl), dt_device.data_ptr())
+        if rc != OK:
+            self._raise("rt_cfl_dt_async", rc)
+
+    def floor_counts(self):
+        a, b = C.c_int64(), C.c_int64()
+        rc = lib().rt_get_floor_counts(self._h, C.byref(a), C.byref(b))
+        if rc != OK:
+            self._raise("rt_get_floor_counts", rc)
+        return a.value, b.value
+
+    def launch_count(self):
+        return int(lib().rt_get_launch_count(self._h))
+
+
+# ---------------------------------------------------------------------- driving a described workload
+def grid_from_workload(w, device="cuda:0"):
+    g = Grid(w.geometry, w.n, w.xf[0], w.xf[1], w.xf[2], w.bc, device=device)
+    g.set_params(make_params(**w.params))
+    for which, spec in w.opacities.items():
+        g.set_opacity(which, opacity_from_spec(spec))
+    return g
+
+
+class DeviceState:
+    """device-resident copy of a workload's fields: U (two buffers), rho, T, mom"""
+
+    def __init__(self, g, w):
+        self.U = [g.to_device(a) for a in w.U]
+        self.U2 = [t.clone() for t in self.U]  # ghosts of FIXED boundaries must exist in both buffers
+        self.rho = g.to_device(w.rho)
+        self.T = g.to_device(w.T)
+        self.mom = [g.to_device(a) for a in w.mom] if w.mom is not None else None
+
+
+def substep(g, w, st, dt, step_index=0):
+    """one sub-step = rt_explicit_step + rt_implicit_step on the device state (buffers swap)"""
+    if w.solver_schedule:
+        g.set_params(make_params(**dict(w.params, solver=w.solver_at(step_index))))
+    g.explicit_step(dt, st.rho, st.T, st.U, st.U2)
+    g.implicit_step(dt, st.rho, st.T, st.mom, st.U2)
+    st.U, st.U2 = st.U2, st.U
+
+
+def run_substeps(g, w, nsub, dts=None, st=None):
+    """nsub sub-steps of workload w; dts = fixed time steps, else rt_cfl_dt each step.
+    Returns (state, list of dt used)."""
+    st = st if st is not None else DeviceState(g, w)
+    used = []
+    for s in range(nsub):
+        if w.solver_schedule:
+            g.set_params(make_params(**dict(w.params, solver=w.solver_at(s))))
+        dt = float(dts[s]) if dts is not None else g.cfl_dt(st.U, w.cfl)
+        used.append(dt)
+        g.explicit_step(dt, st.rho, st.T, st.U, st.U2)
+        g.implicit_step(dt, st.rho, st.T, st.mom, st.U2)
+        st.U, st.U2 = st.U2, st.U
+    return st, used
