@@ -1,0 +1,370 @@
+"""GPU parity: the CUDA path (through the C ABI of include/rt.h) against the CPU oracle, element by
+element on the same seeded inputs.  Run on the B200 box with `-m gpu`.
+
+Error norm (SURVEY.md Sect. 8(d) "Parity"): per field,
+    err = max_i |gpu - oracle| / max_i |oracle|   over interior cells,
+with the three flux components scaled by max_i E_r (F may be identically ~0) and the three momentum
+components by the largest |m|.  Gates (BASELINE.json north_star): <= 1e-11 after one sub-step,
+<= 1e-8 after 100 sub-steps.  Integer/byte work (ghost fill, floor counters) is bit-exact.
+"""
+import ctypes
+
+import numpy as np
+import pytest
+import torch
+
+import rt_workloads as W
+from oracle import ort
+
+pytestmark = pytest.mark.gpu
+
+TOL1 = 1e-11     # one sub-step
+TOL100 = 1e-8    # 100 sub-steps
+
+
+@pytest.fixture(scope="module")
+def rt():
+    assert torch.cuda.is_available(), "the -m gpu tests need a CUDA device"
+    from paper_2606_26268_b200 import rt as _rt
+    _rt.lib()
+    return _rt
+
+
+def field_errors(w, gpuU, refU, gpuT=None, refT=None, gpum=None, refm=None):
+    """dict name -> scaled max error over interior cells"""
+    it = w.interior
+    out = {}
+    Escale = np.abs(refU[0][it]).max()
+    for q, name in enumerate(("E", "F1", "F2", "F3")):
+        out[name] = np.abs(gpuU[q][it] - refU[q][it]).max() / Escale
+    if refT is not None:
+        out["T"] = np.abs(gpuT[it] - refT[it]).max() / np.abs(refT[it]).max()
+    if refm is not None:
+        ms = max(np.abs(a[it]).max() for a in refm)
+        for q in range(3):
+            out["m%d" % (q + 1)] = np.abs(gpum[q][it] - refm[q][it]).max() / (ms if ms > 0 else 1.0)
+    return out
+
+
+def to_host(ts):
+    return [t.cpu().numpy() for t in ts]
+
+
+def run_both(rt, w, nsub, dts=None):
+    """nsub sub-steps on both sides with one dt sequence (the oracle's CFL unless given)."""
+    og = ort.grid_from_workload(w)
+    if dts is None:
+        refU, refT, refm, dts = ort.run_substeps(og, w, nsub)
+    else:
+        refU, refT, refm, _ = ort.run_substeps(og, w, nsub, dts=dts)
+    g = rt.grid_from_workload(w)
+    st, _ = rt.run_substeps(g, w, nsub, dts=dts)
+    torch.cuda.synchronize()
+    gpuU = to_host(st.U)
+    gpuT = st.T.cpu().numpy()
+    gpum = to_host(st.mom) if st.mom is not None else None
+    errs = field_errors(w, gpuU, refU, gpuT, refT, gpum, refm if w.params["feedback_momentum"] else None)
+    return errs, (og.floor_counts(), g.floor_counts()), dts
+
+
+def assert_below(errs, tol, what):
+    bad = {k: v for k, v in errs.items() if not (v <= tol)}
+    assert not bad, "%s: scaled errors above %.1e: %s (all: %s)" % (what, tol, bad, errs)
+
+
+# ----------------------------------------------------------------------------- a0: metrics
+def stretched_edges(geometry, n, rng):
+    if geometry == W.CARTESIAN:
+        return [np.cumsum(np.concatenate([[0.3], rng.uniform(0.5, 1.5, size=v)])) for v in n]
+    if geometry == W.CYLINDRICAL:
+        return [np.geomspace(0.5, 7.0, n[0] + 1), np.linspace(0.0, 2 * np.pi, n[1] + 1),
+                np.cumsum(np.concatenate([[-1.0], rng.uniform(0.5, 1.5, size=n[2])]))]
+    return [np.geomspace(1.0, 50.0, n[0] + 1), np.linspace(0.4, 2.6, n[1] + 1), np.linspace(0.0, 2 * np.pi, n[2] + 1)]
+
+
+@pytest.mark.parametrize("geometry", [W.CARTESIAN, W.CYLINDRICAL, W.SPHERICAL])
+def test_metric_precompute_matches_oracle(rt, geometry):
+    rng = np.random.default_rng(11 + geometry)
+    n = (37, 19, 11)
+    xf = stretched_edges(geometry, n, rng)
+    bc = (1,) * 6
+    og = ort.Grid(geometry, n, xf[0], xf[1], xf[2], bc)
+    g = rt.Grid(geometry, n, xf[0], xf[1], xf[2], bc)
+    # products of the same 1-D factors in another order: a few ulp.  Spherical: D(-cos th) is a difference of
+    # two cosines of size ~1, each within ~2 ulp of libm's on the device, so the factor itself carries
+    # ~4 eps / min D(-cos th) relative difference.
+    tol = 2e-15
+    if geometry == W.SPHERICAL:
+        tol += 4 * np.finfo(float).eps / np.abs(np.diff(np.cos(xf[1]))).min()
+    for a, b, name in zip(g.metrics(), og.metrics(), ("vol", "area1", "area2", "area3")):
+        assert np.all(np.abs(a - b) <= tol * np.abs(b)), name
+
+
+# ----------------------------------------------------------------------------- a1: ghost fill (bit-exact)
+@pytest.mark.parametrize("n", [(13, 9, 7), (33, 1, 1), (1, 6, 5), (9, 8, 1)])
+@pytest.mark.parametrize("bc", [(0, 0, 0, 0, 0, 0), (1, 1, 2, 2, 0, 0), (2, 1, 1, 2, 2, 2), (3, 1, 0, 0, 1, 3)])
+def test_ghost_fill_is_bit_exact(rt, n, bc):
+    rng = np.random.default_rng(3)
+    xf = [np.linspace(0.0, 1.0, v + 1) for v in n]
+    og = ort.Grid(W.CARTESIAN, n, xf[0], xf[1], xf[2], bc)
+    g = rt.Grid(W.CARTESIAN, n, xf[0], xf[1], xf[2], bc)
+    U = [rng.standard_normal(og.shape) for _ in range(4)]
+    dU = [g.to_device(a) for a in U]
+    og.fill_ghosts(U)
+    g.fill_ghosts(dU)
+    for q in range(4):
+        assert np.array_equal(dU[q].cpu().numpy(), U[q]), "field %d" % q
+
+
+# ----------------------------------------------------------------------------- one sub-step, random states
+def random_workload(geometry, n, solver, thick, seed, fmax=1.0, bc=None, feedback=1, table=False):
+    rng = np.random.default_rng(seed)
+    xf = stretched_edges(geometry, n, rng)
+    for d in range(3):
+        if n[d] == 1:
+            xf[d] = xf[d][:2]
+    if bc is None:
+        bc = (0, 0, 0, 0, 0, 0) if geometry == W.CARTESIAN else (2, 1, 1, 1, 0, 0)
+    shape = W.ghosted_shape(n)
+    U = W.random_state(rng, n, fmax=fmax)
+    rho = np.exp(rng.uniform(np.log(1e-3), np.log(1e2), size=shape))
+    T = np.exp(rng.uniform(np.log(0.3), np.log(3.0), size=shape))
+    mom = [rng.standard_normal(shape) for _ in range(3)]
+    if table:
+        tab = W.smooth_table(rng, 24, 20, (-4.0, 3.0), (-1.0, 1.0), offset=0.0)
+        opac = {W.OPAC_PLANCK: W.table(tab - 0.3, (-4.0, 3.0), (-1.0, 1.0), 2.0, 1.5),
+                W.OPAC_ROSSELAND: W.table(tab, (-4.0, 3.0), (-1.0, 1.0), 2.0, 1.5),
+                W.OPAC_SCATTER: W.power_law(0.05)}
+    else:
+        opac = {W.OPAC_PLANCK: W.power_law(2.0, a=1.0, b=-3.0, kmin=1e-4, kmax=1e6),
+                W.OPAC_ROSSELAND: W.power_law(1.0, a=1.0, b=-3.5, kmin=1e-4, kmax=1e6),
+                W.OPAC_SCATTER: W.power_law(0.3, a=0.37, b=0.21)}   # generic exponents: the pow() path
+    return W.Workload(name="rand", geometry=geometry, n=n, xf=xf, bc=bc,
+                      params=W.default_params(chat=7.0, c=300.0, solver=solver, thick_limit=thick,
+                                              feedback_momentum=feedback, E_floor=1e-30),
+                      opacities=opac, U=U, rho=rho, T=T, mom=mom)
+
+
+# sizes span several tiles of every kernel and leave ragged tails: the x1 sweep owns 30 cells per
+# warp, the marching sweeps 128 x 32 (i x march), the per-cell kernels 128 cells per block
+@pytest.mark.parametrize("geometry", [W.CARTESIAN, W.CYLINDRICAL, W.SPHERICAL])
+@pytest.mark.parametrize("solver", [W.SOLVER_HLL, W.SOLVER_GLF])
+@pytest.mark.parametrize("thick", [0, 1])
+def test_one_substep_random_states_3d(rt, geometry, solver, thick):
+    w = random_workload(geometry, (141, 37, 35), solver, thick, seed=100 + 10 * geometry + 2 * solver + thick)
+    errs, counts, _ = run_both(rt, w, 1)
+    assert_below(errs, TOL1, "3-D one sub-step")
+    assert counts[0] == counts[1]
+
+
+@pytest.mark.parametrize("n", [(257, 1, 1), (5, 1, 1), (2, 2, 2), (1, 40, 1), (1, 9, 33), (64, 1, 7), (31, 65, 1),
+                               (300, 3, 2)])
+@pytest.mark.parametrize("solver", [W.SOLVER_HLL, W.SOLVER_GLF])
+def test_one_substep_degenerate_shapes(rt, n, solver):
+    w = random_workload(W.CARTESIAN, n, solver, 1, seed=7 + sum(n))
+    errs, counts, _ = run_both(rt, w, 1)
+    assert_below(errs, TOL1, "shape %s" % (n,))
+    assert counts[0] == counts[1]
+
+
+@pytest.mark.parametrize("geometry", [W.CYLINDRICAL, W.SPHERICAL])
+def test_one_substep_curvilinear_low_dimensional(rt, geometry):
+    for n in [(65, 1, 1), (40, 33, 1)]:
+        w = random_workload(geometry, n, W.SOLVER_HLL, 1, seed=17 + geometry, bc=(2, 1, 1, 1, 1, 1))
+        errs, _, _ = run_both(rt, w, 1)
+        assert_below(errs, TOL1, "geometry %d shape %s" % (geometry, n))
+
+
+def test_one_substep_table_opacities_and_all_boundary_kinds(rt):
+    w = random_workload(W.SPHERICAL, (50, 34, 20), W.SOLVER_HLL, 1, seed=5, bc=(3, 1, 2, 1, 0, 0), table=True)
+    errs, _, _ = run_both(rt, w, 1)
+    assert_below(errs, TOL1, "table opacities")
+
+
+def streaming_workload(seed, exact):
+    """30 % of the cells free-streaming.  exact=True: f = 1 EXACTLY (|F| = E with F along one axis, the
+    beam of config 2 / the irradiation boundary of config 5) next to vacuum-floor cells.
+    exact=False: F = E n with a random direction n, so |F|/E = 1 +- a few ulp."""
+    w = random_workload(W.CARTESIAN, (70, 33, 9), W.SOLVER_HLL, 0, seed=seed, fmax=0.999)
+    rng = np.random.default_rng(seed + 1)
+    shape = w.U[0].shape
+    beam = rng.uniform(size=shape) < 0.3
+    if exact:
+        axis = rng.integers(0, 3, size=shape)
+        sign = rng.choice([-1.0, 1.0], size=shape)
+        for q in range(3):
+            w.U[1 + q][beam] = np.where(axis == q, sign * w.U[0], 0.0)[beam]   # tangential to the other two sweeps (R-G8)
+    else:
+        nrm = np.sqrt(w.U[1] ** 2 + w.U[2] ** 2 + w.U[3] ** 2)
+        for q in (1, 2, 3):
+            w.U[q][beam] = (w.U[q] * w.U[0] / nrm)[beam]
+    vac = rng.uniform(size=shape) < 0.1
+    w.U[0][vac] = 1e-10
+    for q in (1, 2, 3):
+        w.U[q][vac] = 0.0
+    return w
+
+
+@pytest.mark.parametrize("solver", [W.SOLVER_HLL, W.SOLVER_GLF])
+def test_streaming_limit_states_f_exactly_one(rt, solver):
+    """the degenerate closure limit: s = 1, zeta = 0, lambda_1 = lambda_3 = cos(theta) (L167), S_L = S_R = 0
+    on the faces a beam is tangential to (R-G8)"""
+    w = streaming_workload(9, exact=True)
+    w.params["solver"] = solver
+    errs, counts, _ = run_both(rt, w, 1)
+    assert_below(errs, TOL1, "f = 1 exactly, solver %d" % solver)
+    assert counts[0] == counts[1]
+
+
+def test_streaming_limit_states_f_one_to_roundoff(rt):
+    """1 - f of a few ulp: Eq. 22 is ill-conditioned there in ANY arithmetic, zeta^2 = O(1 - f) so a
+    half-ulp change of f^2 moves zeta = sqrt(.) by ~sqrt(2 eps) = 2e-8 and the HLL flux by that times the
+    jump.  The gate here is that conditioning bound, not the 1e-11 formula-parity gate
+    (DESIGN.md "Tolerances"); GLF has no wave-speed estimate and keeps 1e-11."""
+    w = streaming_workload(9, exact=False)
+    errs, _, _ = run_both(rt, w, 1)
+    assert_below(errs, 2e-7, "f = 1 to round-off, HLL")
+    w.params["solver"] = W.SOLVER_GLF
+    errs, _, _ = run_both(rt, w, 1)
+    assert_below(errs, TOL1, "f = 1 to round-off, GLF")
+
+
+def test_uniform_state_is_preserved_on_the_gpu(rt):
+    n = (70, 9, 6)
+    xf = [np.linspace(0.0, 1.0, v + 1) for v in n]
+    g = rt.Grid(rt.CARTESIAN, n, xf[0], xf[1], xf[2], (0,) * 6)
+    g.set_params(rt.make_params(chat=3.0))
+    U = [torch.full(g.shape, v, dtype=torch.float64, device="cuda") for v in (1.7, 0.3, -0.4, 0.5)]
+    out = [torch.zeros_like(t) for t in U]
+    g.explicit_step(0.01, None, None, U, out)
+    for q in range(4):
+        a, b = out[q][g.interior], U[q][g.interior]
+        assert torch.all((a - b).abs() <= 2e-16 * 1.7), q
+
+
+# ----------------------------------------------------------------------------- a11: CFL
+@pytest.mark.parametrize("geometry,n", [(W.CARTESIAN, (141, 37, 35)), (W.SPHERICAL, (67, 33, 18)), (W.CARTESIAN, (300, 1, 1)),
+                                        (W.CYLINDRICAL, (1 + 32, 7, 1))])
+def test_cfl_dt_matches_oracle(rt, geometry, n):
+    w = random_workload(geometry, n, W.SOLVER_HLL, 0, seed=23)
+    og = ort.grid_from_workload(w)
+    g = rt.grid_from_workload(w)
+    dU = [g.to_device(a) for a in w.U]
+    ref = og.cfl_dt(w.U, 0.4)
+    got = g.cfl_dt(dU, 0.4)
+    assert abs(got - ref) <= 1e-14 * ref
+    dt_dev = torch.zeros(1, dtype=torch.float64, device="cuda")
+    g.cfl_dt_async(dU, 0.4, dt_dev)
+    g.cfl_dt_async(dU, 0.8, dt_dev)       # scratch re-arms itself between calls
+    assert abs(dt_dev.item() - 2 * ref) <= 2e-14 * ref
+
+
+# ----------------------------------------------------------------------------- BASELINE configs
+def test_config1_pulse_and_equilibration_100_substeps(rt):
+    for w in (W.c1a(), W.c1b()):
+        errs1, _, dts = run_both(rt, w, 1)
+        assert_below(errs1, TOL1, w.name + " 1 sub-step")
+        errs, counts, _ = run_both(rt, w, 100)
+        assert_below(errs, TOL100, w.name + " 100 sub-steps")
+        assert counts[0] == counts[1]
+
+
+def test_config2_beam_shadow_reduced_and_full_width(rt):
+    w = W.c2(n1=128, n2=128, nsub=300)
+    errs, counts, _ = run_both(rt, w, 300)
+    assert_below(errs, TOL100, "C2 128^2, 300 sub-steps")
+    # no floor-count comparison here: the vacuum cells sit exactly ON the floor value, so E* = floor -+ 1 ulp
+    # flips the `E < E_floor` predicate without changing the floored result
+    w = W.c2()                                  # full 512^2
+    errs1, _, _ = run_both(rt, w, 1)
+    assert_below(errs1, TOL1, "C2 512^2 1 sub-step")
+    errs, counts, _ = run_both(rt, w, 100)
+    assert_below(errs, TOL100, "C2 512^2 100 sub-steps")
+    assert counts[0][1] == counts[1][1]
+
+
+def test_config3_turbulent_box_128_full_length(rt):
+    w = W.c3()
+    errs1, _, _ = run_both(rt, w, 1)
+    assert_below(errs1, TOL1, "C3 1 sub-step")
+    errs, counts, _ = run_both(rt, w, 100)
+    assert_below(errs, TOL100, "C3 100 sub-steps")
+    assert counts[0] == counts[1]
+
+
+def test_config4_two_opacities_alternating_solvers(rt):
+    w = W.c4(nside=96)
+    errs, counts, _ = run_both(rt, w, 100)       # HLL / GLF alternate every sub-step
+    assert_below(errs, TOL100, "C4 96^3 100 sub-steps")
+    assert counts[0] == counts[1]
+
+
+def test_config5_spherical_disc_reduced_full_length(rt):
+    w = W.c5(n=(128, 64, 128))
+    errs1, _, _ = run_both(rt, w, 1)
+    assert_below(errs1, TOL1, "C5 128x64x128 1 sub-step")
+    errs, counts, _ = run_both(rt, w, 50)
+    assert_below(errs, TOL100, "C5 128x64x128 50 sub-steps")
+    assert counts[0] == counts[1]
+
+
+@pytest.mark.parametrize("name", ["C4", "C5"])
+def test_full_size_configs_in_the_bench_launch_configuration(rt, name):
+    """BASELINE.json's full sizes (256^3, 256x128x256): two sub-steps (HLL then GLF for C4), every cell
+    compared; the same calls bench.py times."""
+    w = W.BY_NAME[name]()
+    errs1, counts, _ = run_both(rt, w, 2)
+    assert_below(errs1, TOL1 * 2, name + " full size, 2 sub-steps")
+    assert counts[0] == counts[1]
+
+
+# ----------------------------------------------------------------------------- conservation on the GPU
+def test_coupled_energy_is_conserved_when_no_floor_fires(rt):
+    w = W.c3(nside=48)
+    g = rt.grid_from_workload(w)
+    st = rt.DeviceState(g, w)
+    it = w.interior
+    p = w.params
+    tot = lambda: float((st.rho[it] * p["c_v"] * st.T[it] + (p["c"] / p["chat"]) * st.U[0][it]).sum().item())
+    e0 = tot()
+    for s in range(20):
+        dt = g.cfl_dt(st.U, w.cfl)
+        rt.substep(g, w, st, dt, s)
+    nf, nc = g.floor_counts()
+    if nf == 0:
+        assert abs(tot() - e0) <= 1e-12 * abs(e0)
+
+
+# ----------------------------------------------------------------------------- argument errors
+def test_argument_errors_are_reported_not_computed(rt):
+    n = (16, 8, 1)
+    xf = [np.linspace(0.0, 1.0, v + 1) for v in n]
+    with pytest.raises(rt.RtError):
+        rt.Grid(rt.CARTESIAN, n, xf[0][::-1].copy(), xf[1], xf[2], (0,) * 6)          # non-monotone edges
+    with pytest.raises(rt.RtError):
+        rt.Grid(rt.CARTESIAN, n, xf[0], xf[1], xf[2], (0, 1, 0, 0, 0, 0))             # periodic paired with outflow
+    with pytest.raises(rt.RtError):
+        rt.Grid(rt.SPHERICAL, n, xf[0] + 1, xf[1] + 3.0, xf[2], (1,) * 6)             # theta > pi
+    g = rt.Grid(rt.CARTESIAN, n, xf[0], xf[1], xf[2], (0,) * 6)
+    U = [g.zeros() + 1.0 for _ in range(4)]
+    V = [g.zeros() for _ in range(4)]
+    with pytest.raises(rt.RtError) as ei:
+        g.explicit_step(0.1, None, None, U, V)                                         # params not set
+    assert ei.value.status == rt.ERR_BAD_STATE
+    g.set_params(rt.make_params(chat=1.0))
+    for bad in (0.0, -1.0, float("nan"), float("inf")):
+        with pytest.raises(rt.RtError) as ei:
+            g.explicit_step(bad, None, None, U, V)
+        assert ei.value.status == rt.ERR_INVALID_ARG
+    with pytest.raises(rt.RtError):
+        g.explicit_step(0.1, None, None, U, U)                                         # aliased
+    g.set_params(rt.make_params(chat=1.0, thick_limit=1))
+    with pytest.raises(rt.RtError):
+        g.explicit_step(0.1, None, None, U, V)                                         # thick limit needs rho, T
+    with pytest.raises(rt.RtError):
+        g.set_params(rt.make_params(chat=-1.0))
+    with pytest.raises(rt.RtError):
+        g.set_opacity(0, rt.make_power_law(1.0, rho0=0.0))
+    with pytest.raises(RuntimeError):
+        g.explicit_step(0.1, None, None, [t.cpu() for t in U], V)                      # host tensors: no CPU path
+    assert all(torch.all(v == 0.0) for v in V), "a rejected call must not enqueue work"
