@@ -113,6 +113,15 @@ int32_t rt_get_floor_counts(rt_grid* g, int64_t* n_floor, int64_t* n_clip);
 /* Number of kernel launches the library has enqueued on this grid since creation (bench bookkeeping). */
 int64_t rt_get_launch_count(const rt_grid* g);
 
+/* Optional per-kernel device timing (measurement support, not part of the method).  While profiling is
+ * on, every kernel launch is bracketed by a cudaEvent pair on the grid's stream.  rt_get_kernel_times
+ * synchronises, returns the summed milliseconds and launch counts per kernel kind since the last call,
+ * and releases the events.  Kinds: */
+enum { RT_K_GHOST = 0, RT_K_THICK = 1, RT_K_SWEEP1 = 2, RT_K_SWEEP2 = 3, RT_K_SWEEP3 = 4, RT_K_IMPLICIT = 5,
+       RT_K_CFL = 6, RT_NKERNEL_KINDS = 8 };
+int32_t rt_set_profiling(rt_grid* g, int32_t on);
+int32_t rt_get_kernel_times(rt_grid* g, double ms[RT_NKERNEL_KINDS], int64_t launches[RT_NKERNEL_KINDS]);
+
 /* Launch-shape tuning knob, not part of the method: cells marched per thread along the sweep
  * direction in the x2/x3 sweeps (0 = library default). */
 int32_t rt_set_tuning(rt_grid* g, int32_t march_len, int32_t reserved);

@@ -33,7 +33,27 @@ struct rt_grid {
     int same_PR;
     int march_len;
     long long launches;
+    // optional per-kernel device timing (rt_set_profiling): one event pair per launch
+    int profiling;
+    struct ProfRec { int kind; cudaEvent_t a, b; };
+    std::vector<ProfRec> prof;
     char err[256];
+};
+
+// RAII around one launch: records an event before and after it when profiling is on
+struct ProfScope {
+    rt_grid* g;
+    cudaEvent_t b;
+    ProfScope(rt_grid* g_, int kind) : g(g_), b(nullptr) {
+        if (!g->profiling) return;
+        cudaEvent_t a = nullptr;
+        if (cudaEventCreate(&a) != cudaSuccess || cudaEventCreate(&b) != cudaSuccess) { b = nullptr; return; }
+        cudaEventRecord(a, g->stream);
+        g->prof.push_back({kind, a, b});
+    }
+    ~ProfScope() {
+        if (b) cudaEventRecord(b, g->stream);
+    }
 };
 
 static int32_t fail(rt_grid* g, int32_t code, const char* fmt, ...) {
@@ -63,6 +83,32 @@ static bool aligned8(const void* p) { return p && (reinterpret_cast<uintptr_t>(p
 
 extern "C" const char* rt_last_error(const rt_grid* g) { return g ? g->err : "null grid handle"; }
 extern "C" int64_t rt_get_launch_count(const rt_grid* g) { return g ? g->launches : 0; }
+
+extern "C" int32_t rt_set_profiling(rt_grid* g, int32_t on) {
+    if (!g) return RT_ERR_INVALID_ARG;
+    g->profiling = on ? 1 : 0;
+    return RT_OK;
+}
+
+extern "C" int32_t rt_get_kernel_times(rt_grid* g, double ms[RT_NKERNEL_KINDS], int64_t launches[RT_NKERNEL_KINDS]) {
+    if (!g || !ms || !launches) return fail(g, RT_ERR_INVALID_ARG, "rt_get_kernel_times: null argument");
+    for (int k = 0; k < RT_NKERNEL_KINDS; ++k) {
+        ms[k] = 0.0;
+        launches[k] = 0;
+    }
+    RT_CUDA(g, cudaStreamSynchronize(g->stream));
+    for (auto& r : g->prof) {
+        float t = 0.f;
+        if (cudaEventElapsedTime(&t, r.a, r.b) == cudaSuccess && r.kind >= 0 && r.kind < RT_NKERNEL_KINDS) {
+            ms[r.kind] += (double)t;
+            launches[r.kind] += 1;
+        }
+        cudaEventDestroy(r.a);
+        cudaEventDestroy(r.b);
+    }
+    g->prof.clear();
+    return RT_OK;
+}
 
 extern "C" int32_t rt_set_tuning(rt_grid* g, int32_t march_len, int32_t reserved) {
     (void)reserved;
@@ -111,6 +157,7 @@ extern "C" int32_t rt_grid_create(int32_t geometry, const int32_t n[3], int32_t 
     g->same_PR = 0;
     g->march_len = 0;
     g->launches = 0;
+    g->profiling = 0;
     g->err[0] = 0;
     for (int w = 0; w < 3; ++w) {
         memset(&g->opac[w], 0, sizeof(OpacDev));
@@ -186,6 +233,10 @@ extern "C" int32_t rt_grid_create(int32_t geometry, const int32_t n[3], int32_t 
 extern "C" int32_t rt_grid_destroy(rt_grid* g) {
     if (!g) return RT_ERR_INVALID_ARG;
     cudaStreamSynchronize(g->stream);
+    for (auto& r : g->prof) {
+        cudaEventDestroy(r.a);
+        cudaEventDestroy(r.b);
+    }
     cudaFree(g->metric_buf);
     cudaFree(g->lim);
     cudaFree(g->scr);
@@ -315,7 +366,10 @@ static int32_t launch_fill_ghosts(rt_grid* g, double* const U[4]) {
         for (int e = 0; e < 3; ++e)
             if (e != d) tot *= (e < d) ? D.nt[e] : D.n[e];
         const int nb = (int)((tot + 255) / 256 > 4096 ? 4096 : (tot + 255) / 256);
-        k_fill_ghosts<<<nb, 256, 0, g->stream>>>(D, F, d);
+        {
+            ProfScope ps(g, RT_K_GHOST);
+            k_fill_ghosts<<<nb, 256, 0, g->stream>>>(D, F, d);
+        }
         RT_LAUNCH_CHECK(g);
     }
     return RT_OK;
@@ -388,7 +442,10 @@ extern "C" int32_t rt_explicit_step(rt_grid* g, double dt, const double* rho, co
         if (!g->lim) RT_CUDA(g, cudaMalloc(&g->lim, (size_t)D.ntot * sizeof(double)));
         const int bx = 128;
         dim3 grid((D.nt[0] + bx - 1) / bx, D.nt[1], D.nt[2]);
-        k_thick_limit<<<grid, bx, 0, g->stream>>>(D, g->opac[RT_OPAC_ROSSELAND], g->opac[RT_OPAC_SCATTER], rho, T, g->lim);
+        {
+            ProfScope ps(g, RT_K_THICK);
+            k_thick_limit<<<grid, bx, 0, g->stream>>>(D, g->opac[RT_OPAC_ROSSELAND], g->opac[RT_OPAC_SCATTER], rho, T, g->lim);
+        }
         RT_LAUNCH_CHECK(g);
     }
 
@@ -408,7 +465,10 @@ extern "C" int32_t rt_explicit_step(rt_grid* g, double dt, const double* rho, co
     }
     for (int d = 0; d < 3; ++d) {
         if (D.gh[d] == 0) continue;
-        launch_sweep(g, d, hll, thick, curvi, a);
+        {
+            ProfScope ps(g, RT_K_SWEEP1 + d);
+            launch_sweep(g, d, hll, thick, curvi, a);
+        }
         RT_LAUNCH_CHECK(g);
     }
     return RT_OK;
@@ -438,10 +498,13 @@ extern "C" int32_t rt_implicit_step(rt_grid* g, double dt, const double* rho, do
                    g->par.feedback_momentum};
     const int bx = D.n[0] >= 128 ? 128 : ((D.n[0] + 31) / 32) * 32;
     dim3 grid((D.n[0] + bx - 1) / bx, D.n[1], D.n[2]);
-    if (feedback)
-        k_implicit<true><<<grid, bx, 0, g->stream>>>(D, P, g->opac[0], g->opac[1], g->opac[2], a);
-    else
-        k_implicit<false><<<grid, bx, 0, g->stream>>>(D, P, g->opac[0], g->opac[1], g->opac[2], a);
+    {
+        ProfScope ps(g, RT_K_IMPLICIT);
+        if (feedback)
+            k_implicit<true><<<grid, bx, 0, g->stream>>>(D, P, g->opac[0], g->opac[1], g->opac[2], a);
+        else
+            k_implicit<false><<<grid, bx, 0, g->stream>>>(D, P, g->opac[0], g->opac[1], g->opac[2], a);
+    }
     RT_LAUNCH_CHECK(g);
     return RT_OK;
 }
@@ -455,7 +518,10 @@ extern "C" int32_t rt_cfl_dt_async(rt_grid* g, const double* const U[4], double 
     const GridDev& D = g->dev;
     const long long nrows = (long long)D.n[1] * D.n[2];
     const int nb = (int)(nrows < 148 * 8 ? nrows : 148 * 8);
-    k_cfl<<<nb, 256, 0, g->stream>>>(D, g->par.chat, U[0], U[1], U[2], U[3], g->scr, cfl, dt_device);
+    {
+        ProfScope ps(g, RT_K_CFL);
+        k_cfl<<<nb, 256, 0, g->stream>>>(D, g->par.chat, U[0], U[1], U[2], U[3], g->scr, cfl, dt_device);
+    }
     RT_LAUNCH_CHECK(g);
     return RT_OK;
 }

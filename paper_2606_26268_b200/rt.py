@@ -20,6 +20,8 @@ SOLVER_HLL, SOLVER_GLF = 0, 1
 OPAC_PLANCK, OPAC_ROSSELAND, OPAC_SCATTER = 0, 1, 2
 OK, ERR_INVALID_ARG, ERR_BAD_STATE, ERR_CUDA, ERR_NOT_FINITE = 0, 1, 2, 3, 4
 NGHOST = 2
+KERNEL_KINDS = ("ghost_fill", "thick_limit", "sweep_x1", "sweep_x2", "sweep_x3", "implicit", "cfl")
+NKERNEL_KINDS = 8
 
 _dp = C.POINTER(C.c_double)
 
@@ -63,6 +65,8 @@ _SIGNATURES = {
     "rt_get_floor_counts": (C.c_int32, [C.c_void_p, C.POINTER(C.c_int64), C.POINTER(C.c_int64)]),
     "rt_get_launch_count": (C.c_int64, [C.c_void_p]),
     "rt_set_tuning": (C.c_int32, [C.c_void_p, C.c_int32, C.c_int32]),
+    "rt_set_profiling": (C.c_int32, [C.c_void_p, C.c_int32]),
+    "rt_get_kernel_times": (C.c_int32, [C.c_void_p, _dp, C.POINTER(C.c_int64)]),
     "rt_last_error": (C.c_char_p, [C.c_void_p]),
 }
 
@@ -276,6 +280,20 @@ class Grid:
         if rc != OK:
             self._raise("rt_get_floor_counts", rc)
         return a.value, b.value
+
+    def set_profiling(self, on):
+        rc = lib().rt_set_profiling(self._h, 1 if on else 0)
+        if rc != OK:
+            self._raise("rt_set_profiling", rc)
+
+    def kernel_times(self):
+        """{kind name: (summed ms, launches)} since the last call (needs set_profiling(True))"""
+        ms = (C.c_double * NKERNEL_KINDS)()
+        cnt = (C.c_int64 * NKERNEL_KINDS)()
+        rc = lib().rt_get_kernel_times(self._h, ms, cnt)
+        if rc != OK:
+            self._raise("rt_get_kernel_times", rc)
+        return {name: (ms[k], cnt[k]) for k, name in enumerate(KERNEL_KINDS)}
 
     def launch_count(self):
         return int(lib().rt_get_launch_count(self._h))

@@ -182,23 +182,31 @@ def test_one_substep_table_opacities_and_all_boundary_kinds(rt):
 
 
 def streaming_workload(seed, exact):
-    """30 % of the cells free-streaming.  exact=True: f = 1 EXACTLY (|F| = E with F along one axis, the
-    beam of config 2 / the irradiation boundary of config 5) next to vacuum-floor cells.
-    exact=False: F = E n with a random direction n, so |F|/E = 1 +- a few ulp."""
+    """30 % free-streaming states.  exact=True: 3x3x3 BLOCKS of identical cells with f = 1 EXACTLY (|F| = E, F
+    along one axis: the beam of config 2 / the irradiation boundary of config 5) and blocks of vacuum floor.
+    Inside a block every cell has an equal neighbour along each direction, so its van Leer slope is 0 and
+    its face states ARE the cell state: f_face = 1 exactly, s = 1, zeta = 0 on both sides, with O(1) jumps
+    to the neighbouring blocks.  exact=False: single cells with F = E n, n random, so |F|/E = 1 +- a few ulp."""
     w = random_workload(W.CARTESIAN, (70, 33, 9), W.SOLVER_HLL, 0, seed=seed, fmax=0.999)
     rng = np.random.default_rng(seed + 1)
     shape = w.U[0].shape
-    beam = rng.uniform(size=shape) < 0.3
     if exact:
-        axis = rng.integers(0, 3, size=shape)
-        sign = rng.choice([-1.0, 1.0], size=shape)
+        cshape = tuple((v + 2) // 3 for v in shape)
+        up = lambda a: np.repeat(np.repeat(np.repeat(a, 3, 0), 3, 1), 3, 2)[:shape[0], :shape[1], :shape[2]]
+        kind = up(rng.uniform(size=cshape))
+        axis = up(rng.integers(0, 3, size=cshape))
+        sign = up(rng.choice([-1.0, 1.0], size=cshape))
+        Eb = up(np.exp(rng.uniform(np.log(0.1), np.log(10.0), size=cshape)))
+        beam, vac = kind < 0.3, kind > 0.9
+        w.U[0][beam] = Eb[beam]
         for q in range(3):
-            w.U[1 + q][beam] = np.where(axis == q, sign * w.U[0], 0.0)[beam]   # tangential to the other two sweeps (R-G8)
+            w.U[1 + q][beam] = np.where(axis == q, sign * Eb, 0.0)[beam]   # tangential to the other two sweeps (R-G8)
     else:
+        beam = rng.uniform(size=shape) < 0.3
+        vac = rng.uniform(size=shape) < 0.1
         nrm = np.sqrt(w.U[1] ** 2 + w.U[2] ** 2 + w.U[3] ** 2)
         for q in (1, 2, 3):
             w.U[q][beam] = (w.U[q] * w.U[0] / nrm)[beam]
-    vac = rng.uniform(size=shape) < 0.1
     w.U[0][vac] = 1e-10
     for q in (1, 2, 3):
         w.U[q][vac] = 0.0
