@@ -39,7 +39,7 @@ __device__ __forceinline__ double frcp(double x) {
     return r;
 }
 
-// s = sqrt(x) and rs = 1/sqrt(x) together (coupled Newton, 8 fp64 ops + 1 for rs).
+// s = sqrt(x) and rs = 1/sqrt(x) together (coupled Newton + residual step, 10 fp64 ops + 1 for rs).
 __device__ __forceinline__ void fsqrt_rsqrt(double x, double& s, double& rs) {
     double y = rsqrt_seed(x);
     double g = x * y, h = 0.5 * y;
@@ -49,7 +49,10 @@ __device__ __forceinline__ void fsqrt_rsqrt(double x, double& s, double& rs) {
     t = fma(-h, g, 0.5);
     g = fma(g, t, g);
     h = fma(h, t, h);
-    s = g;
+    // residual step: makes s exact for perfect squares (x = E^2 at f = 1 gives s = E, hence
+    // (1 - xi)/2 = 0 and zeta = 0 exactly: the lambda -> cos(theta) limit of L167)
+    const double d = fma(-g, g, x);
+    s = fma(d, h, g);
     rs = h + h;
 }
 
@@ -136,7 +139,10 @@ __device__ __forceinline__ void fpreserve(State& st, const double Uc[4], double 
     E2f = Ef * Ef;
     double F2r = fma(st.U[3], st.U[3], fma(st.U[2], st.U[2], st.U[1] * st.U[1]));
     bool keep = (F2r <= E2f) && (F2r * Ec2 > F2c * E2f);
+    // quotient with one residual step: correctly rounded, so E_f = E_c gives r = 1 EXACTLY and a
+    // cell with f = 1 and zero slopes keeps f_face = 1 exactly (the zeta = 0 limit, L167)
     double r = Ef * invEc;
+    r = fma(fma(-Uc[0], r, Ef), invEc, r);
     st.U[1] = keep ? st.U[1] : Uc[1] * r;
     st.U[2] = keep ? st.U[2] : Uc[2] * r;
     st.U[3] = keep ? st.U[3] : Uc[3] * r;
