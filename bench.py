@@ -2,8 +2,10 @@
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C4|C5|C3|CP] [--impl native|reference]
 
-A "step" is one pass of the whole hot path over the resident fields: rt_cfl_dt -> rt_explicit_step
-(ghost fill, thick-limit pre-pass, fused sweeps x1/x2/x3) -> rt_implicit_step.  Default workload: C4,
+A "step" is one pass of the whole hot path over the resident fields, one rt_substep call: ghost fill ->
+thick-limit pre-pass -> fused sweeps x1/x2/x3 -> floor + opacities + implicit coupling with the CFL reduction
+of the updated state fused behind it (the time step stays on the device).  `--api split` times the three-call
+form rt_cfl_dt (8-byte result to the host) -> rt_explicit_step -> rt_implicit_step instead.  Default workload: C4,
 the 256^3 Cartesian config the north_star target is quoted on (C5 = the spherical one).
 Prints ONE JSON line (see DESIGN.md "Measurement" for every key).  `--impl reference` times the CPU
 oracle instead (the only other place oracle/ may be executed besides the cpu_baseline leg).
@@ -24,6 +26,8 @@ if ROOT not in sys.path:
 METRIC = "radiation cell-updates/sec (fp64, 1 B200)"
 UNIT = "cell-updates/s"
 
+FUSED_CFL = True
+
 # Algorithmic bytes per interior cell and launch: 8 B x (fields read + written)
 def bytes_per_cell(kind, thick, feedback):
     return {
@@ -32,7 +36,7 @@ def bytes_per_cell(kind, thick, feedback):
         "sweep_x2": 96.0 + (8.0 if thick else 0.0),            # read U 4 (+ lim) + U_out 4; write U_out 4
         "sweep_x3": 96.0 + (8.0 if thick else 0.0),
         "implicit": 88.0 + (48.0 if feedback else 0.0),        # read E,F,rho,T (+m); write E,F,T (+m)
-        "cfl": 32.0,                                           # read E,F
+        "cfl": 32.0 if not FUSED_CFL else 0.0,                 # split API: read E,F; fused: a one-thread finalise kernel
         "ghost_fill": 0.0,                                     # O(surface)
     }[kind]
 
@@ -45,6 +49,7 @@ def parse_args():
     ap.add_argument("--workload", default="C4")
     ap.add_argument("--impl", default="native", choices=["native", "reference"])
     ap.add_argument("--size", type=int, default=0, help="override the grid side (debug only; marks the line)")
+    ap.add_argument("--api", default="fused", choices=["fused", "split"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     return ap.parse_args()
@@ -64,7 +69,8 @@ def workload_config(w, args):
     n = w.n
     cfg = {"workload": "%s: %s %dx%dx%d, %s" % (w.name, ("cartesian", "cylindrical", "spherical")[w.geometry], n[0], n[1], n[2],
                                                 w.notes),
-           "cells": w.ncells, "substep": "rt_cfl_dt + rt_explicit_step + rt_implicit_step",
+           "cells": w.ncells, "substep": "rt_substep (device-resident dt)" if args.api == "fused" else
+           "rt_cfl_dt + rt_explicit_step + rt_implicit_step",
            "solver": "HLL/GLF alternating" if w.solver_schedule else ("HLL" if w.params["solver"] == 0 else "GLF"),
            "thick_limit": int(w.params["thick_limit"]), "feedback_momentum": int(w.params["feedback_momentum"]),
            "l2": "inputs larger than L2 (%.2f GB resident fields vs 126 MB)" % (13 * 8 * float(__import__("numpy").prod(w.shape)) / 1e9),
@@ -123,9 +129,13 @@ class ClockSampler(threading.Thread):
 
 # ------------------------------------------------------------------------------------------ native arm
 def one_substep(rt, g, w, st, step_index):
-    """the whole hot path once: CFL (8-byte result to the host) -> explicit -> implicit"""
+    """the whole hot path once"""
     if w.solver_schedule:
         g.set_params(rt.make_params(**dict(w.params, solver=w.solver_at(step_index))))
+    if FUSED_CFL:
+        g.substep(st.dt_dev, w.cfl, st.rho, st.T, st.mom, st.U, st.U2)
+        st.U, st.U2 = st.U2, st.U
+        return None
     dt = g.cfl_dt(st.U, w.cfl)
     g.explicit_step(dt, st.rho, st.T, st.U, st.U2)
     g.implicit_step(dt, st.rho, st.T, st.mom, st.U2)
@@ -149,9 +159,13 @@ def run_native(args):
     if world > 1:
         dist.init_process_group("nccl", device_id=dev)
 
+    global FUSED_CFL
+    FUSED_CFL = args.api == "fused"
     w = make_workload(args.workload, args.size)
     g = rt.grid_from_workload(w, device=dev)
     st = rt.DeviceState(g, w)
+    st.dt_dev = torch.zeros(1, dtype=torch.float64, device=dev)
+    g.cfl_dt_async(st.U, w.cfl, st.dt_dev)
     thick, feedback = bool(w.params["thick_limit"]), bool(w.params["feedback_momentum"]) and w.mom is not None
     K, Wm = args.steps, max(args.warmup, 0)
 
@@ -274,9 +288,13 @@ def run_e2e(rt, g, w, st, K, world, dev, barrier):
             d.copy_(h, non_blocking=True)
         if w.solver_schedule:
             g.set_params(rt.make_params(**dict(w.params, solver=w.solver_at(i))))
-        dt = g.cfl_dt(ins[:4], w.cfl)
-        g.explicit_step(dt, st.rho, st.T, ins[:4], st.U2)
-        g.implicit_step(dt, st.rho, st.T, st.mom, st.U2)
+        if FUSED_CFL:   # the input state is new every step: its CFL first, then the whole sub-step, no host sync
+            g.cfl_dt_async(ins[:4], w.cfl, st.dt_dev)
+            g.substep(st.dt_dev, w.cfl, st.rho, st.T, st.mom, ins[:4], st.U2)
+        else:
+            dt = g.cfl_dt(ins[:4], w.cfl)
+            g.explicit_step(dt, st.rho, st.T, ins[:4], st.U2)
+            g.implicit_step(dt, st.rho, st.T, st.mom, st.U2)
         outs = list(st.U2) + [st.T] + (list(st.mom) if st.mom is not None else [])
         for h, d in zip(host_out, outs):
             h.copy_(d, non_blocking=True)

@@ -100,6 +100,21 @@ int32_t rt_explicit_step(rt_grid* g, double dt, const double* rho, const double*
 int32_t rt_implicit_step(rt_grid* g, double dt, const double* rho, double* T,
                          double* const mom[3], double* const U[4]);
 
+/* rt_implicit_step with step 10 (L120; R-G15) fused behind it: the kernel that writes the updated state also
+ * reduces the CFL rate of that state (warp shuffles + filtered atomicMax), and a one-thread kernel writes
+ * *dt_next_device = cfl / max rate (DEVICE double): bit-identical to rt_cfl_dt_async on the updated U, without
+ * reading the four fields again.  Asynchronous, graph-capturable. */
+int32_t rt_implicit_step_cfl(rt_grid* g, double dt, const double* rho, double* T,
+                             double* const mom[3], double* const U[4], double cfl, double* dt_next_device);
+
+/* One WHOLE sub-step (steps 1, 3-8, 10; L111-120) with the time step resident on the device:
+ *   dt = *dt_device  ->  rt_explicit_step(dt, U_in -> U_out)  ->  rt_implicit_step_cfl(dt, U_out)  ->  *dt_device = next dt.
+ * dt_device: DEVICE double, read by the kernels of this sub-step and overwritten at its end (seed it with
+ * rt_cfl_dt_async).  No host synchronisation anywhere: a sequence of sub-steps can be enqueued back to back or
+ * captured in a CUDA graph.  rho and T are required.  Same argument errors as the two halves. */
+int32_t rt_substep(rt_grid* g, double* dt_device, double cfl, const double* rho, double* T,
+                   double* const mom[3], double* const U_in[4], double* const U_out[4]);
+
 /* Step 10 (L120; R-G15): dt = cfl / max_cells sum_{d active} chat max(|lam1|,|lam3|)(U; d) / dl_d.
  * rt_cfl_dt writes a HOST double and synchronises the stream; rt_cfl_dt_async writes a DEVICE
  * double and does not synchronise (graph-capturable). */

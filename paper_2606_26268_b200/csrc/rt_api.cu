@@ -354,6 +354,25 @@ extern "C" int32_t rt_set_opacity(rt_grid* g, int32_t which, const rt_opacity* o
     return RT_OK;
 }
 
+// which table opacities among `members` (RT_OPAC_* indices) can share log10(rho rho_unit), log10(T T_unit)
+static OpacSet opac_set(const rt_grid* g, const int* members, int nm) {
+    OpacSet os = {0, -1};
+    int ntab = 0;
+    for (int a = 0; a < nm; ++a) {
+        const int w = members[a];
+        if (!g->opac[w].set || g->opac[w].kind != 1) continue;
+        ++ntab;
+        if (os.src < 0) {
+            os.src = w;
+            continue;
+        }
+        const OpacDev &x = g->opac[os.src], &y = g->opac[w];
+        if (x.T_unit != y.T_unit || (x.n_lrho > 1) != (y.n_lrho > 1) || (x.n_lrho > 1 && x.rho_unit != y.rho_unit)) return OpacSet{0, -1};
+    }
+    os.share = ntab >= 2 ? 1 : 0;
+    return os;
+}
+
 // ------------------------------------------------------------------------------------------------
 static int32_t launch_fill_ghosts(rt_grid* g, double* const U[4]) {
     const GridDev& D = g->dev;
@@ -423,11 +442,12 @@ static void launch_sweep(rt_grid* g, int d, bool hll, bool thick, bool curvi, co
     }
 }
 
-extern "C" int32_t rt_explicit_step(rt_grid* g, double dt, const double* rho, const double* T, double* const U_in[4],
-                                    double* const U_out[4]) {
+// explicit half; the time step is dt (host) or, when dt_dev != nullptr, the device double *dt_dev
+static int32_t explicit_impl(rt_grid* g, double dt, const double* dt_dev, const double* rho, const double* T,
+                             double* const U_in[4], double* const U_out[4]) {
     if (!g || !U_in || !U_out) return fail(g, RT_ERR_INVALID_ARG, "rt_explicit_step: null argument");
     if (!g->have_par) return fail(g, RT_ERR_BAD_STATE, "rt_explicit_step: rt_set_params has not been called");
-    if (!(dt > 0.0) || !isfinite(dt)) return fail(g, RT_ERR_INVALID_ARG, "rt_explicit_step: dt must be finite and > 0");
+    if (!dt_dev && (!(dt > 0.0) || !isfinite(dt))) return fail(g, RT_ERR_INVALID_ARG, "rt_explicit_step: dt must be finite and > 0");
     for (int q = 0; q < 4; ++q)
         if (!aligned8(U_in[q]) || !aligned8(U_out[q]) || U_in[q] == U_out[q])
             return fail(g, RT_ERR_INVALID_ARG, "rt_explicit_step: U_in/U_out[%d] null, misaligned or aliased", q);
@@ -444,7 +464,9 @@ extern "C" int32_t rt_explicit_step(rt_grid* g, double dt, const double* rho, co
         dim3 grid((D.nt[0] + bx - 1) / bx, D.nt[1], D.nt[2]);
         {
             ProfScope ps(g, RT_K_THICK);
-            k_thick_limit<<<grid, bx, 0, g->stream>>>(D, g->opac[RT_OPAC_ROSSELAND], g->opac[RT_OPAC_SCATTER], rho, T, g->lim);
+            const int members[2] = {RT_OPAC_ROSSELAND, RT_OPAC_SCATTER};
+            k_thick_limit<<<grid, bx, 0, g->stream>>>(D, g->opac[RT_OPAC_ROSSELAND], g->opac[RT_OPAC_SCATTER], opac_set(g, members, 2),
+                                                      rho, T, g->lim);
         }
         RT_LAUNCH_CHECK(g);
     }
@@ -456,6 +478,8 @@ extern "C" int32_t rt_explicit_step(rt_grid* g, double dt, const double* rho, co
     }
     a.lim = thick ? g->lim : nullptr;
     a.dtc = dt * g->par.chat;
+    a.dt_dev = dt_dev;
+    a.chat = g->par.chat;
     const bool hll = g->par.solver == RT_SOLVER_HLL;
     const bool curvi = D.geometry != RT_CARTESIAN;
     if (D.gh[0] == 0) {
@@ -474,10 +498,20 @@ extern "C" int32_t rt_explicit_step(rt_grid* g, double dt, const double* rho, co
     return RT_OK;
 }
 
-extern "C" int32_t rt_implicit_step(rt_grid* g, double dt, const double* rho, double* T, double* const mom[3], double* const U[4]) {
+extern "C" int32_t rt_explicit_step(rt_grid* g, double dt, const double* rho, const double* T, double* const U_in[4],
+                                    double* const U_out[4]) {
+    return explicit_impl(g, dt, nullptr, rho, T, U_in, U_out);
+}
+
+// implicit half; with_cfl: fold the step-10 rate of the updated state into the scratch word and finalise
+// dt_next_dev = cfl / max rate with a one-thread kernel
+static int32_t implicit_impl(rt_grid* g, double dt, const double* dt_dev, const double* rho, double* T, double* const mom[3],
+                             double* const U[4], bool with_cfl, double cfl, double* dt_next_dev) {
     if (!g || !U || !aligned8(rho) || !aligned8(T)) return fail(g, RT_ERR_INVALID_ARG, "rt_implicit_step: null or misaligned argument");
     if (!g->have_par) return fail(g, RT_ERR_BAD_STATE, "rt_implicit_step: rt_set_params has not been called");
-    if (!(dt > 0.0) || !isfinite(dt)) return fail(g, RT_ERR_INVALID_ARG, "rt_implicit_step: dt must be finite and > 0");
+    if (!dt_dev && (!(dt > 0.0) || !isfinite(dt))) return fail(g, RT_ERR_INVALID_ARG, "rt_implicit_step: dt must be finite and > 0");
+    if (with_cfl && (!aligned8(dt_next_dev) || !(cfl > 0.0) || !isfinite(cfl)))
+        return fail(g, RT_ERR_INVALID_ARG, "rt_implicit_step_cfl: cfl must be finite and > 0 and dt_next_device non-null");
     for (int q = 0; q < 4; ++q)
         if (!aligned8(U[q])) return fail(g, RT_ERR_INVALID_ARG, "rt_implicit_step: U[%d] null or misaligned", q);
     const bool feedback = g->par.feedback_momentum && mom != nullptr;
@@ -491,8 +525,15 @@ extern "C" int32_t rt_implicit_step(rt_grid* g, double dt, const double* rho, do
     a.T = T;
     for (int q = 0; q < 3; ++q) a.mom[q] = feedback ? mom[q] : nullptr;
     a.dt = dt;
+    a.dt_dev = dt_dev;
+    a.scr = g->scr;
     a.feedback = feedback;
     a.same_PR = g->same_PR;
+    {
+        const int members[3] = {RT_OPAC_PLANCK, RT_OPAC_ROSSELAND, RT_OPAC_SCATTER};
+        a.os = opac_set(g, members, 3);
+    }
+    a.ichat = 1.0 / g->par.chat;
     a.counters = g->counters;
     ParamsDev P = {g->par.chat, g->par.c, g->par.a_R, g->par.c_v, g->par.E_floor, g->par.solver, g->par.thick_limit,
                    g->par.feedback_momentum};
@@ -500,13 +541,43 @@ extern "C" int32_t rt_implicit_step(rt_grid* g, double dt, const double* rho, do
     dim3 grid((D.n[0] + bx - 1) / bx, D.n[1], D.n[2]);
     {
         ProfScope ps(g, RT_K_IMPLICIT);
-        if (feedback)
-            k_implicit<true><<<grid, bx, 0, g->stream>>>(D, P, g->opac[0], g->opac[1], g->opac[2], a);
+        if (feedback && with_cfl)
+            k_implicit<true, true><<<grid, bx, 0, g->stream>>>(D, P, g->opac[0], g->opac[1], g->opac[2], a);
+        else if (feedback)
+            k_implicit<true, false><<<grid, bx, 0, g->stream>>>(D, P, g->opac[0], g->opac[1], g->opac[2], a);
+        else if (with_cfl)
+            k_implicit<false, true><<<grid, bx, 0, g->stream>>>(D, P, g->opac[0], g->opac[1], g->opac[2], a);
         else
-            k_implicit<false><<<grid, bx, 0, g->stream>>>(D, P, g->opac[0], g->opac[1], g->opac[2], a);
+            k_implicit<false, false><<<grid, bx, 0, g->stream>>>(D, P, g->opac[0], g->opac[1], g->opac[2], a);
     }
     RT_LAUNCH_CHECK(g);
+    if (with_cfl) {
+        {
+            ProfScope ps(g, RT_K_CFL);
+            k_cfl_finalize<<<1, 1, 0, g->stream>>>(g->scr, cfl, dt_next_dev);
+        }
+        RT_LAUNCH_CHECK(g);
+    }
     return RT_OK;
+}
+
+extern "C" int32_t rt_implicit_step(rt_grid* g, double dt, const double* rho, double* T, double* const mom[3], double* const U[4]) {
+    return implicit_impl(g, dt, nullptr, rho, T, mom, U, false, 0.0, nullptr);
+}
+
+extern "C" int32_t rt_implicit_step_cfl(rt_grid* g, double dt, const double* rho, double* T, double* const mom[3],
+                                        double* const U[4], double cfl, double* dt_next_device) {
+    return implicit_impl(g, dt, nullptr, rho, T, mom, U, true, cfl, dt_next_device);
+}
+
+extern "C" int32_t rt_substep(rt_grid* g, double* dt_device, double cfl, const double* rho, double* T, double* const mom[3],
+                              double* const U_in[4], double* const U_out[4]) {
+    if (!g || !aligned8(dt_device)) return fail(g, RT_ERR_INVALID_ARG, "rt_substep: null or misaligned dt_device");
+    if (!(cfl > 0.0) || !isfinite(cfl)) return fail(g, RT_ERR_INVALID_ARG, "rt_substep: cfl must be finite and > 0");
+    if (!aligned8(rho) || !aligned8(T)) return fail(g, RT_ERR_INVALID_ARG, "rt_substep: rho / T null or misaligned");
+    int32_t rc = explicit_impl(g, 0.0, dt_device, rho, T, U_in, U_out);
+    if (rc != RT_OK) return rc;
+    return implicit_impl(g, 0.0, dt_device, rho, T, mom, U_out, true, cfl, dt_device);
 }
 
 extern "C" int32_t rt_cfl_dt_async(rt_grid* g, const double* const U[4], double cfl, double* dt_device) {

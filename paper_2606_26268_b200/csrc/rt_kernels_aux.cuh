@@ -8,6 +8,8 @@
 
 namespace rtm1 {
 
+constexpr int RT_OPAC_SCATTER_IDX = 2;
+
 // ------------------------------------------------------------------------------------------------
 // a0: metric precompute.  The paper gives no metric formulas (L15, L409); DESIGN.md R-G9: exact
 // finite-volume integrals, written as separable 1-D factors.
@@ -155,10 +157,11 @@ __global__ void k_fill_ghosts(GridDev g, Fields4 U, int d) {
 // a9: opacities.  Power law kappa0 (rho/rho0)^a (T/T0)^b clipped (L299) or bilinear table of
 // log10 kappa on a uniform (log10 rho, log10 T) grid (L375; R-G14).
 // ------------------------------------------------------------------------------------------------
-// x^(n2/2) for integer n2: sqrt for the odd part, binary powering for the rest (uniform control flow).
+// x^(n2/2) for integer n2: sqrt for the odd part, binary powering for the rest (warp-uniform control
+// flow); Newton sqrt / reciprocal of rt_math.cuh (x > 0 normal), so ~1-2 ulp against libm pow().
 __device__ __forceinline__ double pow_half_int(double x, int n2) {
     int m = n2 < 0 ? -n2 : n2;
-    double r = (m & 1) ? sqrt(x) : 1.0;
+    double r = (m & 1) ? fsqrt(x) : 1.0;
     int k = m >> 1;
     double base = x;
     while (k) {
@@ -166,35 +169,38 @@ __device__ __forceinline__ double pow_half_int(double x, int n2) {
         base *= base;
         k >>= 1;
     }
-    return n2 < 0 ? 1.0 / r : r;
+    return n2 < 0 ? frcp(r) : r;
 }
 
-__device__ __forceinline__ double opacity_eval(const OpacDev& o, double rho, double T) {
-    if (!o.set) return 0.0;
-    if (o.kind == 0) {
-        const double xr = rho * o.irho0, xt = T * o.iT0;
-        double pr, pt;
-        if (o.n2a != INT_MIN) pr = pow_half_int(xr, o.n2a); else pr = pow(xr, o.a);
-        if (o.n2b != INT_MIN) pt = pow_half_int(xt, o.n2b); else pt = pow(xt, o.b);
-        double k = o.kappa0 * pr * pt;
-        k = dmax(k, o.kmin);
-        k = dmin(k, o.kmax);
-        return k;
-    }
-    double y = log10(T * o.T_unit);
-    y = dmin(dmax(y, o.lT_min), o.lT_max);
+// log10 of the table inputs, shared by every table opacity of a cell when their units agree
+struct LogRT {
+    double lrho, lT;
+};
+
+__device__ __forceinline__ double power_law_eval(const OpacDev& o, double rho, double T) {
+    const double xr = rho * o.irho0, xt = T * o.iT0;
+    double pr, pt;
+    if (o.n2a != INT_MIN) pr = pow_half_int(xr, o.n2a); else pr = pow(xr, o.a);
+    if (o.n2b != INT_MIN) pt = pow_half_int(xt, o.n2b); else pt = pow(xt, o.b);
+    double k = o.kappa0 * pr * pt;
+    k = dmax(k, o.kmin);
+    k = dmin(k, o.kmax);
+    return k;
+}
+
+__device__ __forceinline__ double table_eval(const OpacDev& o, const LogRT& l) {
+    const double y = dmin(dmax(l.lT, o.lT_min), o.lT_max);
     const double v = (y - o.lT_min) * o.sv;
-    int j0 = (int)floor(v);
+    int j0 = (int)v;  // v >= 0: truncation = floor
     j0 = max(0, min(j0, o.n_lT - 2));
     const double tv = v - (double)j0;
     double val;
     if (o.n_lrho == 1) {
         val = (1.0 - tv) * __ldg(o.tab + j0) + tv * __ldg(o.tab + j0 + 1);
     } else {
-        double x = log10(rho * o.rho_unit);
-        x = dmin(dmax(x, o.lrho_min), o.lrho_max);
+        const double x = dmin(dmax(l.lrho, o.lrho_min), o.lrho_max);
         const double u = (x - o.lrho_min) * o.su;
-        int i0 = (int)floor(u);
+        int i0 = (int)u;
         i0 = max(0, min(i0, o.n_lrho - 2));
         const double tu = u - (double)i0;
         const double* p = o.tab + (long long)j0 * o.n_lrho + i0;
@@ -204,6 +210,32 @@ __device__ __forceinline__ double opacity_eval(const OpacDev& o, double rho, dou
     return exp10(val);
 }
 
+__device__ __forceinline__ LogRT log_inputs(const OpacDev& o, double rho, double T) {
+    LogRT l;
+    l.lT = log10(T * o.T_unit);
+    l.lrho = o.n_lrho > 1 ? log10(rho * o.rho_unit) : 0.0;
+    return l;
+}
+
+__device__ __forceinline__ double opacity_eval(const OpacDev& o, double rho, double T) {
+    if (!o.set) return 0.0;
+    if (o.kind == 0) return power_law_eval(o, rho, T);
+    return table_eval(o, log_inputs(o, rho, T));
+}
+
+// Several opacities of one cell.  share = the host found that every TABLE among them has the same
+// rho_unit, T_unit (and n_lrho > 1 or == 1 alike): log10 rho, log10 T are then evaluated once.
+struct OpacSet {
+    int share;  // 1: >= 2 tables in the set and all of them share their log inputs
+    int src;    // RT_OPAC_* index of the table whose units define the shared inputs
+};
+
+__device__ __forceinline__ double opacity_eval_shared(const OpacDev& o, double rho, double T, bool share, const LogRT& l) {
+    if (!o.set) return 0.0;
+    if (o.kind == 0) return power_law_eval(o, rho, T);
+    return share ? table_eval(o, l) : table_eval(o, log_inputs(o, rho, T));
+}
+
 // ------------------------------------------------------------------------------------------------
 // Thick-limit pre-pass (Eq. 25-26; R-G7): per ghosted cell
 //   limd = 4 / (3 tau_cell),  tau_cell = rho chi dx,  chi = kappa_R + sigma (L89),
@@ -211,8 +243,10 @@ __device__ __forceinline__ double opacity_eval(const OpacDev& o, double rho, dou
 // Ghost cells take the value of the periodic image or of the nearest interior cell, so rho and T
 // ghosts are never read.  The sweeps use lim_face = max(limd_a, limd_b) = 4/(3 min(tau_a, tau_b)).
 // ------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(128) k_thick_limit(GridDev g, OpacDev oR, OpacDev oS, const double* __restrict__ rho,
-                                                     const double* __restrict__ T, double* __restrict__ lim) {
+__global__ void __launch_bounds__(128) k_thick_limit(const __grid_constant__ GridDev g, const __grid_constant__ OpacDev oR,
+                                                     const __grid_constant__ OpacDev oS, const __grid_constant__ OpacSet os,
+                                                     const double* __restrict__ rho, const double* __restrict__ T,
+                                                     double* __restrict__ lim) {
     const int ii = blockIdx.x * blockDim.x + threadIdx.x;
     if (ii >= g.nt[0]) return;
     const int jj = blockIdx.y, kk = blockIdx.z;
@@ -226,13 +260,17 @@ __global__ void __launch_bounds__(128) k_thick_limit(GridDev g, OpacDev oR, Opac
     const long long src = (c[0] + g.gh[0]) * g.stride[0] + (c[1] + g.gh[1]) * g.stride[1] + (c[2] + g.gh[2]) * g.stride[2];
     const long long dst = ii * g.stride[0] + jj * g.stride[1] + kk * g.stride[2];
     const double r = rho[src], t = T[src];
-    const double chi = opacity_eval(oR, r, t) + opacity_eval(oS, r, t);
+    LogRT l = {0.0, 0.0};
+    const bool share = os.share != 0;
+    if (share) l = log_inputs(os.src == RT_OPAC_SCATTER_IDX ? oS : oR, r, t);
+    const double chi = opacity_eval_shared(oR, r, t, share, l) + opacity_eval_shared(oS, r, t, share, l);
     double dx = 0.0;
 #pragma unroll
     for (int d = 0; d < 3; ++d)
         if (g.gh[d] > 0) dx = dmax(dx, g.len[d][0][c[0]] * g.len[d][1][c[1]] * g.len[d][2][c[2]]);
     const double tau = r * chi * dx;
-    lim[dst] = 4.0 / (3.0 * tau);
+    // any value >= 1 means "no limit" (|lambda| <= 1, L167): tau -> 0 maps to +inf without a division by zero
+    lim[dst] = tau > 1.0e-100 ? 4.0 * frcp(3.0 * tau) : __builtin_huge_val();
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -293,6 +331,13 @@ __device__ __forceinline__ void block_max_to_global(double v, CflScratch* scr, d
         scr->blocks_done = 0;
         *dt_out = cfl / __longlong_as_double((long long)bits);
     }
+}
+
+// dt = cfl / (running max of the rate), then re-arm the running max (fused-CFL path of k_implicit)
+__global__ void k_cfl_finalize(CflScratch* scr, double cfl, double* dt_out) {
+    const unsigned long long bits = scr->rate_bits;
+    scr->rate_bits = 0ull;
+    *dt_out = cfl / __longlong_as_double((long long)bits);
 }
 
 __global__ void __launch_bounds__(256) k_cfl(GridDev g, double chat, const double* __restrict__ E, const double* __restrict__ F1,

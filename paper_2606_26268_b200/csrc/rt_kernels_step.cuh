@@ -19,8 +19,12 @@ struct SweepArgs {
     const double* uin[4];
     double* uout[4];
     const double* lim;  // thick-limit pre-pass array (ghosted) or nullptr
-    double dtc;         // dt * chat
+    double dtc;         // dt * chat (host-supplied dt)
+    const double* dt_dev;  // device-resident dt (rt_substep) or nullptr; then dt * chat = *dt_dev * chat
+    double chat;
 };
+
+__device__ __forceinline__ double sweep_dtc(const SweepArgs& a) { return a.dt_dev ? __ldg(a.dt_dev) * a.chat : a.dtc; }
 
 constexpr double kInf = __builtin_huge_val();
 
@@ -85,7 +89,8 @@ __global__ void __launch_bounds__(128) k_sweep_x(const __grid_constant__ GridDev
     for (int q = 0; q < 4; ++q) fu[q] = __shfl_down_sync(0xffffffffu, fl[q], 1);
 
     if (lane >= 1 && lane <= kXOut && i < n1) {
-        const double coef = a.dtc * g.cg[0][0][i] * g.cg[0][1][j] * g.cg[0][2][k];
+        const double dtc = sweep_dtc(a);
+        const double coef = dtc * g.cg[0][0][i] * g.cg[0][1][j] * g.cg[0][2][k];
         double out[4];
 #pragma unroll
         for (int q = 0; q < 4; ++q) out[q] = fma(-coef, fu[q] - fl[q], q0[q]);
@@ -93,7 +98,7 @@ __global__ void __launch_bounds__(128) k_sweep_x(const __grid_constant__ GridDev
             const double E2 = q0[0] * q0[0];
             const double F2 = fma(q0[3], q0[3], fma(q0[2], q0[2], q0[1] * q0[1]));
             const Closure c = closure_of(q0[0], E2, F2);
-            const double s = a.dtc * g.invr[i];
+            const double s = dtc * g.invr[i];
             if (g.geometry == 1) {
                 out[1] = fma(s, fma(c.gE * q0[2], q0[2], c.dE), out[1]);
                 out[2] = fma(-s, c.gE * q0[1] * q0[2], out[2]);
@@ -133,7 +138,7 @@ __global__ void __launch_bounds__(128) k_sweep_march(const __grid_constant__ Gri
     const long long S = g.stride[D];
     // index of the cell with sweep coordinate 0
     const long long id0 = (i + g.gh[0]) + (long long)g.gh[D] * S + (long long)(o + g.gh[EO]) * g.stride[EO];
-    const double K = a.dtc * g.cg[D][0][i] * g.cg[D][EO][o];
+    const double K = sweep_dtc(a) * g.cg[D][0][i] * g.cg[D][EO][o];
     const double* __restrict__ cgd = g.cg[D][D];
     const double* __restrict__ wfd = g.wf[D];
 
@@ -210,18 +215,28 @@ struct ImplicitArgs {
     double* T;
     double* mom[3];
     double dt;
+    const double* dt_dev;  // device-resident dt (rt_substep) or nullptr
+    CflScratch* scr;       // CFL: running max of the rate, as the bit pattern of a non-negative double
     int feedback;
     int same_PR;  // kappa_P and kappa_R are the same law: evaluate once
+    OpacSet os;   // shared log10 inputs of the table opacities
+    double ichat; // 1 / chat
     unsigned long long* counters;  // [0] floor activations, [1] clip activations
 };
 
-template <bool FEEDBACK>
+// CFL = true additionally evaluates the step-10 rate (R-G15) of the UPDATED state of each cell and folds it
+// into scr->rate_bits: warp-shuffle max, then one atomicMax per warp that beats the running maximum (a plain
+// load filters the rest, so a few hundred atomics reach L2 instead of one per warp); k_cfl_finalize turns the
+// maximum into dt.  The result equals rt_cfl_dt of the updated state bit for bit (same cell_rate, max is exact).
+template <bool FEEDBACK, bool CFL>
 __global__ void __launch_bounds__(128) k_implicit(const __grid_constant__ GridDev g, const __grid_constant__ ParamsDev par,
                                                   const __grid_constant__ OpacDev oP, const __grid_constant__ OpacDev oR,
                                                   const __grid_constant__ OpacDev oS, const __grid_constant__ ImplicitArgs a) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     const int j = blockIdx.y, k = blockIdx.z;
     bool floored = false, clipped = false;
+    double rate = 0.0;
+    const double dt = a.dt_dev ? __ldg(a.dt_dev) : a.dt;
     if (i < g.n[0]) {
         const long long id = (i + g.gh[0]) + (j + g.gh[1]) * g.stride[1] + (k + g.gh[2]) * g.stride[2];
         double E = a.U[0][id];
@@ -244,11 +259,14 @@ __global__ void __launch_bounds__(128) k_implicit(const __grid_constant__ GridDe
             for (int q = 0; q < 3; ++q) F[q] *= sc;
             clipped = true;
         }
-        const double kP = opacity_eval(oP, rho, T0);
-        const double kR = a.same_PR ? kP : opacity_eval(oR, rho, T0);
-        const double chi = kR + opacity_eval(oS, rho, T0);
-        const double gr = a.dt * par.chat * kP * rho;
-        const double gg = a.dt * par.c * kP * rho;
+        LogRT lg = {0.0, 0.0};
+        const bool share = a.os.share != 0;
+        if (share) lg = log_inputs(a.os.src == 0 ? oP : (a.os.src == 1 ? oR : oS), rho, T0);
+        const double kP = opacity_eval_shared(oP, rho, T0, share, lg);
+        const double kR = a.same_PR ? kP : opacity_eval_shared(oR, rho, T0, share, lg);
+        const double chi = kR + opacity_eval_shared(oS, rho, T0, share, lg);
+        const double gr = dt * par.chat * kP * rho;
+        const double gg = dt * par.c * kP * rho;
         const double Cv = rho * par.c_v;
         const double aT3 = par.a_R * T0 * T0 * T0;
         const double aT4 = aT3 * T0;
@@ -256,15 +274,25 @@ __global__ void __launch_bounds__(128) k_implicit(const __grid_constant__ GridDe
         const double idet = frcp(det);
         const double En = fma(E, fma(4.0 * gg, aT3, Cv), gr * Cv * aT4) * idet;
         const double Tn = fma((1.0 + gr) * Cv, T0, fma(3.0 * gg, aT4, gg * E)) * idet;
-        const double idamp = frcp(fma(a.dt * par.chat * chi, rho, 1.0));
+        const double idamp = frcp(fma(dt * par.chat * chi, rho, 1.0));
         a.U[0][id] = En;
         a.T[id] = Tn;
-        const double ichat = 1.0 / par.chat;
+        const double ichat = a.ichat;
+        double Fn[3];
 #pragma unroll
         for (int q = 0; q < 3; ++q) {
-            const double Fn = F[q] * idamp;
-            if (FEEDBACK) a.mom[q][id] = fma(-(Fn - F[q]), ichat, m[q]);
-            a.U[1 + q][id] = Fn;
+            Fn[q] = F[q] * idamp;
+            if (FEEDBACK) a.mom[q][id] = fma(-(Fn[q] - F[q]), ichat, m[q]);
+            a.U[1 + q][id] = Fn[q];
+        }
+        if (CFL) rate = cell_rate(g, par.chat, En, Fn[0], Fn[1], Fn[2], i, j, k);
+    }
+    if (CFL) {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) rate = dmax(rate, __shfl_xor_sync(0xffffffffu, rate, o));
+        if ((threadIdx.x & 31) == 0) {
+            const unsigned long long bits = (unsigned long long)__double_as_longlong(rate);
+            if (bits > *(volatile unsigned long long*)&a.scr->rate_bits) atomicMax(&a.scr->rate_bits, bits);
         }
     }
     // rare: count floor / clip activations (debug counters, SURVEY.md Sect. 8(d) "Parity")

@@ -60,6 +60,10 @@ _SIGNATURES = {
                                      C.POINTER(C.c_void_p)]),
     "rt_implicit_step": (C.c_int32, [C.c_void_p, C.c_double, C.c_void_p, C.c_void_p, C.POINTER(C.c_void_p),
                                      C.POINTER(C.c_void_p)]),
+    "rt_implicit_step_cfl": (C.c_int32, [C.c_void_p, C.c_double, C.c_void_p, C.c_void_p, C.POINTER(C.c_void_p),
+                                         C.POINTER(C.c_void_p), C.c_double, C.c_void_p]),
+    "rt_substep": (C.c_int32, [C.c_void_p, C.c_void_p, C.c_double, C.c_void_p, C.c_void_p, C.POINTER(C.c_void_p),
+                               C.POINTER(C.c_void_p), C.POINTER(C.c_void_p)]),
     "rt_cfl_dt": (C.c_int32, [C.c_void_p, C.POINTER(C.c_void_p), C.c_double, _dp]),
     "rt_cfl_dt_async": (C.c_int32, [C.c_void_p, C.POINTER(C.c_void_p), C.c_double, C.c_void_p]),
     "rt_get_floor_counts": (C.c_int32, [C.c_void_p, C.POINTER(C.c_int64), C.POINTER(C.c_int64)]),
@@ -256,6 +260,41 @@ class Grid:
         if rc != OK:
             self._raise("rt_implicit_step", rc)
 
+    def implicit_step_cfl(self, dt, rho, T, mom, U, cfl, dt_next_device):
+        _check_field(rho, self.shape, "rho")
+        _check_field(T, self.shape, "T")
+        for q in range(4):
+            _check_field(U[q], self.shape, "U[%d]" % q)
+        if mom is not None:
+            for q in range(3):
+                _check_field(mom[q], self.shape, "mom[%d]" % q)
+        self._check_dt_device(dt_next_device)
+        rc = lib().rt_implicit_step_cfl(self._h, float(dt), rho.data_ptr(), T.data_ptr(),
+                                        _ptr_array(mom) if mom is not None else None, _ptr_array(U), float(cfl),
+                                        dt_next_device.data_ptr())
+        if rc != OK:
+            self._raise("rt_implicit_step_cfl", rc)
+
+    def substep(self, dt_device, cfl, rho, T, mom, U_in, U_out):
+        _check_field(rho, self.shape, "rho")
+        _check_field(T, self.shape, "T")
+        for q in range(4):
+            _check_field(U_in[q], self.shape, "U_in[%d]" % q)
+            _check_field(U_out[q], self.shape, "U_out[%d]" % q)
+        if mom is not None:
+            for q in range(3):
+                _check_field(mom[q], self.shape, "mom[%d]" % q)
+        self._check_dt_device(dt_device)
+        rc = lib().rt_substep(self._h, dt_device.data_ptr(), float(cfl), rho.data_ptr(), T.data_ptr(),
+                              _ptr_array(mom) if mom is not None else None, _ptr_array(U_in), _ptr_array(U_out))
+        if rc != OK:
+            self._raise("rt_substep", rc)
+
+    @staticmethod
+    def _check_dt_device(t):
+        if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float64 and t.numel() >= 1):
+            raise ValueError("dt_device must be a CUDA float64 tensor")
+
     def cfl_dt(self, U, cfl):
         for q in range(4):
             _check_field(U[q], self.shape, "U[%d]" % q)
@@ -342,3 +381,20 @@ def run_substeps(g, w, nsub, dts=None, st=None):
         g.implicit_step(dt, st.rho, st.T, st.mom, st.U2)
         st.U, st.U2 = st.U2, st.U
     return st, used
+
+
+def run_substeps_fused(g, w, nsub, st=None):
+    """nsub sub-steps through rt_substep: the time step never leaves the device (seeded by rt_cfl_dt_async,
+    then produced by the CFL reduction fused behind each implicit half).  Returns (state, dt tensor of the
+    NEXT sub-step, list of the dt used as a device tensor history)."""
+    st = st if st is not None else DeviceState(g, w)
+    dt_dev = torch.zeros(1, dtype=torch.float64, device=g.device)
+    hist = torch.zeros(nsub, dtype=torch.float64, device=g.device)
+    g.cfl_dt_async(st.U, w.cfl, dt_dev)
+    for s in range(nsub):
+        if w.solver_schedule:
+            g.set_params(make_params(**dict(w.params, solver=w.solver_at(s))))
+        hist[s:s + 1].copy_(dt_dev)
+        g.substep(dt_dev, w.cfl, st.rho, st.T, st.mom, st.U, st.U2)
+        st.U, st.U2 = st.U2, st.U
+    return st, dt_dev, hist

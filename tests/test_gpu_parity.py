@@ -269,6 +269,39 @@ def test_uniform_state_is_preserved_on_the_gpu(rt):
         assert torch.all((a - b).abs() <= 2e-16 * 1.7), q
 
 
+# ----------------------------------------------------------------------------- fused sub-step (device-resident dt)
+@pytest.mark.parametrize("geometry,n,table", [(W.CARTESIAN, (70, 33, 9), False), (W.SPHERICAL, (45, 20, 11), True),
+                                              (W.CARTESIAN, (300, 1, 1), False), (W.CYLINDRICAL, (33, 7, 1), False)])
+def test_fused_substep_matches_oracle_and_its_dt_never_leaves_the_device(rt, geometry, n, table):
+    """rt_substep x 5: dt seeded by rt_cfl_dt_async, then produced by the CFL reduction fused behind each
+    implicit half; fields against the oracle stepping with ITS OWN CFL, every dt used against the oracle's."""
+    w = random_workload(geometry, n, W.SOLVER_HLL, 1, seed=41, fmax=0.95, table=table)
+    og = ort.grid_from_workload(w)
+    refU, refT, refm, dts = ort.run_substeps(og, w, 5)
+    g = rt.grid_from_workload(w)
+    st, dt_next, hist = rt.run_substeps_fused(g, w, 5)
+    torch.cuda.synchronize()
+    errs = field_errors(w, to_host(st.U), refU, st.T.cpu().numpy(), refT, to_host(st.mom), refm)
+    assert_below(errs, 5 * TOL1, "fused sub-steps")
+    used = hist.cpu().numpy()
+    assert np.all(np.abs(used - np.array(dts)) <= 1e-12 * np.array(dts)), (used, dts)
+    # the fused reduction equals the stand-alone one on the same state, bit for bit
+    assert g.cfl_dt(st.U, w.cfl) == float(dt_next.item())
+
+
+def test_implicit_step_cfl_equals_implicit_then_cfl(rt):
+    w = random_workload(W.CARTESIAN, (141, 9, 5), W.SOLVER_HLL, 0, seed=43, fmax=1.0, feedback=0)
+    g = rt.grid_from_workload(w)
+    a, b = rt.DeviceState(g, w), rt.DeviceState(g, w)
+    dtn = torch.zeros(1, dtype=torch.float64, device="cuda")
+    g.implicit_step(0.013, a.rho, a.T, None, a.U)
+    g.implicit_step_cfl(0.013, b.rho, b.T, None, b.U, 0.4, dtn)
+    for q in range(4):
+        assert torch.equal(a.U[q], b.U[q])
+    assert torch.equal(a.T, b.T)
+    assert g.cfl_dt(a.U, 0.4) == float(dtn.item())
+
+
 # ----------------------------------------------------------------------------- a11: CFL
 @pytest.mark.parametrize("geometry,n", [(W.CARTESIAN, (141, 37, 35)), (W.SPHERICAL, (67, 33, 18)), (W.CARTESIAN, (300, 1, 1)),
                                         (W.CYLINDRICAL, (1 + 32, 7, 1))])
