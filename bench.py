@@ -38,6 +38,8 @@ def bytes_per_cell(kind, thick, feedback):
         "implicit": 88.0 + (48.0 if feedback else 0.0),        # read E,F,rho,T (+m); write E,F,T (+m)
         "cfl": 32.0 if not FUSED_CFL else 0.0,                 # split API: read E,F; fused: a one-thread finalise kernel
         "ghost_fill": 0.0,                                     # O(surface)
+        # k_substep_fused: read U 4 (+ lim), rho, T (+ m 3); write E, F, T (+ m 3)
+        "fused": 88.0 + (8.0 if thick else 0.0) + (48.0 if feedback else 0.0),
     }[kind]
 
 
@@ -50,6 +52,7 @@ def parse_args():
     ap.add_argument("--impl", default="native", choices=["native", "reference"])
     ap.add_argument("--size", type=int, default=0, help="override the grid side (debug only; marks the line)")
     ap.add_argument("--api", default="fused", choices=["fused", "split"])
+    ap.add_argument("--fused-seg", type=int, default=0, help="rt_set_tuning fused_seg: 0 auto, -1 per-direction kernels, >0 x3 segment")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     return ap.parse_args()
@@ -163,6 +166,7 @@ def run_native(args):
     FUSED_CFL = args.api == "fused"
     w = make_workload(args.workload, args.size)
     g = rt.grid_from_workload(w, device=dev)
+    g.set_tuning(fused_seg=args.fused_seg)
     st = rt.DeviceState(g, w)
     st.dt_dev = torch.zeros(1, dtype=torch.float64, device=dev)
     g.cfl_dt_async(st.U, w.cfl, st.dt_dev)

@@ -133,13 +133,15 @@ int64_t rt_get_launch_count(const rt_grid* g);
  * synchronises, returns the summed milliseconds and launch counts per kernel kind since the last call,
  * and releases the events.  Kinds: */
 enum { RT_K_GHOST = 0, RT_K_THICK = 1, RT_K_SWEEP1 = 2, RT_K_SWEEP2 = 3, RT_K_SWEEP3 = 4, RT_K_IMPLICIT = 5,
-       RT_K_CFL = 6, RT_NKERNEL_KINDS = 8 };
+       RT_K_CFL = 6, RT_K_FUSED = 7 /* k_substep_fused: a2-a11 in one pass (3-D grids) */, RT_NKERNEL_KINDS = 8 };
 int32_t rt_set_profiling(rt_grid* g, int32_t on);
 int32_t rt_get_kernel_times(rt_grid* g, double ms[RT_NKERNEL_KINDS], int64_t launches[RT_NKERNEL_KINDS]);
 
-/* Launch-shape tuning knob, not part of the method: cells marched per thread along the sweep
- * direction in the x2/x3 sweeps (0 = library default). */
-int32_t rt_set_tuning(rt_grid* g, int32_t march_len, int32_t reserved);
+/* Launch-shape tuning knobs, not part of the method.  march_len: cells marched per thread along the sweep
+ * direction in the x2/x3 sweeps (0 = library default).  fused_seg: rt_substep on 3-D grids runs ONE fused kernel
+ * (reconstruction ... implicit coupling + CFL rate in a single pass over U^n, x1-x2 tiles marching along x3);
+ * 0 = on with an automatic x3 segment length, > 0 = that segment length, -1 = off (per-direction kernels). */
+int32_t rt_set_tuning(rt_grid* g, int32_t march_len, int32_t fused_seg);
 
 const char* rt_last_error(const rt_grid* g);
 

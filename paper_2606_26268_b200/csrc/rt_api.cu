@@ -10,7 +10,7 @@
 #include <vector>
 
 #include "../../include/rt.h"
-#include "rt_kernels_step.cuh"
+#include "rt_kernels_fused.cuh"
 
 using namespace rtm1;
 
@@ -32,6 +32,7 @@ struct rt_grid {
     rt_opacity opac_host[3];
     int same_PR;
     int march_len;
+    int fused_seg;  // rt_set_tuning: 0 auto, -1 never use the fused sub-step kernel, > 0 its x3 segment length
     long long launches;
     // optional per-kernel device timing (rt_set_profiling): one event pair per launch
     int profiling;
@@ -110,10 +111,10 @@ extern "C" int32_t rt_get_kernel_times(rt_grid* g, double ms[RT_NKERNEL_KINDS], 
     return RT_OK;
 }
 
-extern "C" int32_t rt_set_tuning(rt_grid* g, int32_t march_len, int32_t reserved) {
-    (void)reserved;
-    if (!g || march_len < 0) return fail(g, RT_ERR_INVALID_ARG, "rt_set_tuning: bad argument");
+extern "C" int32_t rt_set_tuning(rt_grid* g, int32_t march_len, int32_t fused_seg) {
+    if (!g || march_len < 0 || fused_seg < -1) return fail(g, RT_ERR_INVALID_ARG, "rt_set_tuning: bad argument");
     g->march_len = march_len;
+    g->fused_seg = fused_seg;
     return RT_OK;
 }
 
@@ -156,6 +157,7 @@ extern "C" int32_t rt_grid_create(int32_t geometry, const int32_t n[3], int32_t 
     g->have_par = 0;
     g->same_PR = 0;
     g->march_len = 0;
+    g->fused_seg = 0;
     g->launches = 0;
     g->profiling = 0;
     g->err[0] = 0;
@@ -442,6 +444,21 @@ static void launch_sweep(rt_grid* g, int d, bool hll, bool thick, bool curvi, co
     }
 }
 
+static int32_t launch_thick_limit(rt_grid* g, const double* rho, const double* T) {
+    const GridDev& D = g->dev;
+    if (!g->lim) RT_CUDA(g, cudaMalloc(&g->lim, (size_t)D.ntot * sizeof(double)));
+    const int bx = 128;
+    dim3 grid((D.nt[0] + bx - 1) / bx, D.nt[1], D.nt[2]);
+    {
+        ProfScope ps(g, RT_K_THICK);
+        const int members[2] = {RT_OPAC_ROSSELAND, RT_OPAC_SCATTER};
+        k_thick_limit<<<grid, bx, 0, g->stream>>>(D, g->opac[RT_OPAC_ROSSELAND], g->opac[RT_OPAC_SCATTER], opac_set(g, members, 2),
+                                                  rho, T, g->lim);
+    }
+    RT_LAUNCH_CHECK(g);
+    return RT_OK;
+}
+
 // explicit half; the time step is dt (host) or, when dt_dev != nullptr, the device double *dt_dev
 static int32_t explicit_impl(rt_grid* g, double dt, const double* dt_dev, const double* rho, const double* T,
                              double* const U_in[4], double* const U_out[4]) {
@@ -459,16 +476,8 @@ static int32_t explicit_impl(rt_grid* g, double dt, const double* dt_dev, const 
     if (rc != RT_OK) return rc;
 
     if (thick) {
-        if (!g->lim) RT_CUDA(g, cudaMalloc(&g->lim, (size_t)D.ntot * sizeof(double)));
-        const int bx = 128;
-        dim3 grid((D.nt[0] + bx - 1) / bx, D.nt[1], D.nt[2]);
-        {
-            ProfScope ps(g, RT_K_THICK);
-            const int members[2] = {RT_OPAC_ROSSELAND, RT_OPAC_SCATTER};
-            k_thick_limit<<<grid, bx, 0, g->stream>>>(D, g->opac[RT_OPAC_ROSSELAND], g->opac[RT_OPAC_SCATTER], opac_set(g, members, 2),
-                                                      rho, T, g->lim);
-        }
-        RT_LAUNCH_CHECK(g);
+        rc = launch_thick_limit(g, rho, T);
+        if (rc != RT_OK) return rc;
     }
 
     SweepArgs a;
@@ -570,11 +579,144 @@ extern "C" int32_t rt_implicit_step_cfl(rt_grid* g, double dt, const double* rho
     return implicit_impl(g, dt, nullptr, rho, T, mom, U, true, cfl, dt_next_device);
 }
 
+// ------------------------------------------------------------------------------------------------
+// Fused sub-step (3-D grids): ghost fill -> thick-limit pre-pass -> k_substep_fused -> k_cfl_finalize
+template <bool HLL, bool THICK, bool CURVI, bool FEEDBACK>
+static cudaError_t launch_fused_t(rt_grid* g, const ParamsDev& P, const FusedArgs& a, dim3 grid, int seglen) {
+    auto kern = k_substep_fused<HLL, THICK, CURVI, FEEDBACK>;
+    static bool attr_done = false;
+    if (!attr_done) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kFusedSmemBytes);
+        if (e != cudaSuccess) return e;
+        attr_done = true;
+    }
+    kern<<<grid, dim3(32, FNY), kFusedSmemBytes, g->stream>>>(g->dev, P, g->opac[0], g->opac[1], g->opac[2], a, seglen);
+    return cudaSuccess;
+}
+
+static cudaError_t launch_fused(rt_grid* g, bool hll, bool thick, bool curvi, bool feedback, const ParamsDev& P,
+                                const FusedArgs& a, dim3 grid, int seglen) {
+    const int key = (hll ? 8 : 0) | (thick ? 4 : 0) | (curvi ? 2 : 0) | (feedback ? 1 : 0);
+    switch (key) {
+#define RT_FUSED_CASE(K, A, B, C_, D_) case K: return launch_fused_t<A, B, C_, D_>(g, P, a, grid, seglen);
+        RT_FUSED_CASE(0, false, false, false, false)
+        RT_FUSED_CASE(1, false, false, false, true)
+        RT_FUSED_CASE(2, false, false, true, false)
+        RT_FUSED_CASE(3, false, false, true, true)
+        RT_FUSED_CASE(4, false, true, false, false)
+        RT_FUSED_CASE(5, false, true, false, true)
+        RT_FUSED_CASE(6, false, true, true, false)
+        RT_FUSED_CASE(7, false, true, true, true)
+        RT_FUSED_CASE(8, true, false, false, false)
+        RT_FUSED_CASE(9, true, false, false, true)
+        RT_FUSED_CASE(10, true, false, true, false)
+        RT_FUSED_CASE(11, true, false, true, true)
+        RT_FUSED_CASE(12, true, true, false, false)
+        RT_FUSED_CASE(13, true, true, false, true)
+        RT_FUSED_CASE(14, true, true, true, false)
+        default: return launch_fused_t<true, true, true, true>(g, P, a, grid, seglen);
+#undef RT_FUSED_CASE
+    }
+}
+
+// x3 segment length of the fused kernel: the CTA count should fill whole waves of 2 CTAs per SM, with segments
+// long enough that the two half-work planes at the segment ends stay a small share.
+static int fused_segment_length(const rt_grid* g, int tiles) {
+    const int n3 = g->dev.n[2];
+    if (g->fused_seg > 0) return g->fused_seg < n3 ? g->fused_seg : n3;
+    int dev = 0, nsm = 148;
+    if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
+    const double slots = 2.0 * nsm;
+    int best = n3 < 32 ? n3 : 32;
+    double best_score = -1.0;
+    for (int nseg = 1; nseg <= n3; ++nseg) {
+        const int len = (n3 + nseg - 1) / nseg;
+        if (len < 12 && nseg > 1) break;
+        const int ns = (n3 + len - 1) / len;
+        const double ctas = (double)tiles * ns;
+        const double waves = ceil(ctas / slots);
+        const double fill = ctas / (waves * slots);               // tail effect
+        const double work = (double)len / ((double)len + 0.7);    // segment-end overhead
+        const double score = fill * work * (waves >= 2.0 ? 1.0 : 0.9);
+        if (score > best_score) {
+            best_score = score;
+            best = len;
+        }
+    }
+    return best;
+}
+
+static bool fused_eligible(const rt_grid* g) {
+    const GridDev& D = g->dev;
+    return g->fused_seg >= 0 && D.gh[0] > 0 && D.gh[1] > 0 && D.gh[2] > 0;
+}
+
+static int32_t fused_impl(rt_grid* g, double* dt_device, double cfl, const double* rho, double* T, double* const mom[3],
+                          double* const U_in[4], double* const U_out[4]) {
+    if (!U_in || !U_out) return fail(g, RT_ERR_INVALID_ARG, "rt_substep: null argument");
+    if (!g->have_par) return fail(g, RT_ERR_BAD_STATE, "rt_substep: rt_set_params has not been called");
+    for (int q = 0; q < 4; ++q)
+        if (!aligned8(U_in[q]) || !aligned8(U_out[q]) || U_in[q] == U_out[q])
+            return fail(g, RT_ERR_INVALID_ARG, "rt_substep: U_in/U_out[%d] null, misaligned or aliased", q);
+    const bool feedback = g->par.feedback_momentum && mom != nullptr;
+    if (feedback)
+        for (int q = 0; q < 3; ++q)
+            if (!aligned8(mom[q])) return fail(g, RT_ERR_INVALID_ARG, "rt_substep: mom[%d] null or misaligned", q);
+    const GridDev& D = g->dev;
+    const bool thick = g->par.thick_limit != 0;
+
+    int32_t rc = launch_fill_ghosts(g, U_in);
+    if (rc != RT_OK) return rc;
+    if (thick) {
+        rc = launch_thick_limit(g, rho, T);
+        if (rc != RT_OK) return rc;
+    }
+    FusedArgs a;
+    for (int q = 0; q < 4; ++q) {
+        a.src[q] = U_in[q];
+        a.im.U[q] = U_out[q];
+    }
+    a.src[4] = thick ? g->lim : nullptr;
+    a.chat = g->par.chat;
+    a.im.rho = rho;
+    a.im.T = T;
+    for (int q = 0; q < 3; ++q) a.im.mom[q] = feedback ? mom[q] : nullptr;
+    a.im.dt = 0.0;
+    a.im.dt_dev = dt_device;
+    a.im.scr = g->scr;
+    a.im.feedback = feedback;
+    a.im.same_PR = g->same_PR;
+    {
+        const int members[3] = {RT_OPAC_PLANCK, RT_OPAC_ROSSELAND, RT_OPAC_SCATTER};
+        a.im.os = opac_set(g, members, 3);
+    }
+    a.im.ichat = 1.0 / g->par.chat;
+    a.im.counters = g->counters;
+    ParamsDev P = {g->par.chat, g->par.c, g->par.a_R, g->par.c_v, g->par.E_floor, g->par.solver, g->par.thick_limit,
+                   g->par.feedback_momentum};
+    const int tx = (D.n[0] + FTX - 1) / FTX, ty = (D.n[1] + FTY - 1) / FTY;
+    const int seglen = fused_segment_length(g, tx * ty);
+    dim3 grid(tx, ty, (D.n[2] + seglen - 1) / seglen);
+    {
+        ProfScope ps(g, RT_K_FUSED);
+        cudaError_t e = launch_fused(g, g->par.solver == RT_SOLVER_HLL, thick, D.geometry != RT_CARTESIAN, feedback, P, a, grid, seglen);
+        if (e != cudaSuccess) return fail(g, RT_ERR_CUDA, "k_substep_fused attribute: %s", cudaGetErrorString(e));
+    }
+    RT_LAUNCH_CHECK(g);
+    {
+        ProfScope ps(g, RT_K_CFL);
+        k_cfl_finalize<<<1, 1, 0, g->stream>>>(g->scr, cfl, dt_device);
+    }
+    RT_LAUNCH_CHECK(g);
+    return RT_OK;
+}
+
 extern "C" int32_t rt_substep(rt_grid* g, double* dt_device, double cfl, const double* rho, double* T, double* const mom[3],
                               double* const U_in[4], double* const U_out[4]) {
     if (!g || !aligned8(dt_device)) return fail(g, RT_ERR_INVALID_ARG, "rt_substep: null or misaligned dt_device");
     if (!(cfl > 0.0) || !isfinite(cfl)) return fail(g, RT_ERR_INVALID_ARG, "rt_substep: cfl must be finite and > 0");
     if (!aligned8(rho) || !aligned8(T)) return fail(g, RT_ERR_INVALID_ARG, "rt_substep: rho / T null or misaligned");
+    if (fused_eligible(g)) return fused_impl(g, dt_device, cfl, rho, T, mom, U_in, U_out);
     int32_t rc = explicit_impl(g, 0.0, dt_device, rho, T, U_in, U_out);
     if (rc != RT_OK) return rc;
     return implicit_impl(g, 0.0, dt_device, rho, T, mom, U_out, true, cfl, dt_device);

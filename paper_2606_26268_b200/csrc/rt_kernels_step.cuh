@@ -228,6 +228,75 @@ struct ImplicitArgs {
 // into scr->rate_bits: warp-shuffle max, then one atomicMax per warp that beats the running maximum (a plain
 // load filters the rest, so a few hundred atomics reach L2 instead of one per warp); k_cfl_finalize turns the
 // maximum into dt.  The result equals rt_cfl_dt of the updated state bit for bit (same cell_rate, max is exact).
+// One cell of a8-a10 (+ the CFL rate of the updated state when CFL): shared by k_implicit and the fused
+// sub-step kernel.  E, F: the state after the explicit half; writes through the pointers of `a` at index id.
+template <bool FEEDBACK, bool CFL>
+__device__ __forceinline__ double implicit_cell(const GridDev& g, const ParamsDev& par, const OpacDev& oP, const OpacDev& oR,
+                                                const OpacDev& oS, const ImplicitArgs& a, double dt, long long id, int i, int j,
+                                                int k, double E, double F[3], double rho, double T0, const double m[3],
+                                                bool& floored, bool& clipped) {
+    if (E < par.E_floor) {
+        E = par.E_floor;
+        floored = true;
+    }
+    const double F2 = fma(F[2], F[2], fma(F[1], F[1], F[0] * F[0]));
+    if (F2 > E * E) {
+        const double sc = E * rsqrt(F2);
+#pragma unroll
+        for (int q = 0; q < 3; ++q) F[q] *= sc;
+        clipped = true;
+    }
+    LogRT lg = {0.0, 0.0};
+    const bool share = a.os.share != 0;
+    if (share) lg = log_inputs(a.os.src == 0 ? oP : (a.os.src == 1 ? oR : oS), rho, T0);
+    const double kP = opacity_eval_shared(oP, rho, T0, share, lg);
+    const double kR = a.same_PR ? kP : opacity_eval_shared(oR, rho, T0, share, lg);
+    const double chi = kR + opacity_eval_shared(oS, rho, T0, share, lg);
+    const double gr = dt * par.chat * kP * rho;
+    const double gg = dt * par.c * kP * rho;
+    const double Cv = rho * par.c_v;
+    const double aT3 = par.a_R * T0 * T0 * T0;
+    const double aT4 = aT3 * T0;
+    const double det = fma(Cv, 1.0 + gr, 4.0 * gg * aT3);
+    const double idet = frcp(det);
+    const double En = fma(E, fma(4.0 * gg, aT3, Cv), gr * Cv * aT4) * idet;
+    const double Tn = fma((1.0 + gr) * Cv, T0, fma(3.0 * gg, aT4, gg * E)) * idet;
+    const double idamp = frcp(fma(dt * par.chat * chi, rho, 1.0));
+    a.U[0][id] = En;
+    a.T[id] = Tn;
+    const double ichat = a.ichat;
+    double Fn[3];
+#pragma unroll
+    for (int q = 0; q < 3; ++q) {
+        Fn[q] = F[q] * idamp;
+        if (FEEDBACK) a.mom[q][id] = fma(-(Fn[q] - F[q]), ichat, m[q]);
+        a.U[1 + q][id] = Fn[q];
+    }
+    return CFL ? cell_rate(g, par.chat, En, Fn[0], Fn[1], Fn[2], i, j, k) : 0.0;
+}
+
+// fold a warp's CFL rates into the running maximum (see k_implicit) and count floor / clip activations
+template <bool CFL>
+__device__ __forceinline__ void implicit_warp_epilogue(const ImplicitArgs& a, double rate, int nfloor, int nclip) {
+    if (CFL) {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) rate = dmax(rate, __shfl_xor_sync(0xffffffffu, rate, o));
+        if ((threadIdx.x & 31) == 0) {
+            const unsigned long long bits = (unsigned long long)__double_as_longlong(rate);
+            if (bits > *(volatile unsigned long long*)&a.scr->rate_bits) atomicMax(&a.scr->rate_bits, bits);
+        }
+    }
+    // rare: count floor / clip activations (debug counters, SURVEY.md Sect. 8(d) "Parity")
+    if (__any_sync(0xffffffffu, (nfloor | nclip) != 0)) {
+        nfloor = __reduce_add_sync(0xffffffffu, nfloor);
+        nclip = __reduce_add_sync(0xffffffffu, nclip);
+        if ((threadIdx.x & 31) == 0) {
+            if (nfloor) atomicAdd(&a.counters[0], (unsigned long long)nfloor);
+            if (nclip) atomicAdd(&a.counters[1], (unsigned long long)nclip);
+        }
+    }
+}
+
 template <bool FEEDBACK, bool CFL>
 __global__ void __launch_bounds__(128) k_implicit(const __grid_constant__ GridDev g, const __grid_constant__ ParamsDev par,
                                                   const __grid_constant__ OpacDev oP, const __grid_constant__ OpacDev oR,
@@ -239,68 +308,18 @@ __global__ void __launch_bounds__(128) k_implicit(const __grid_constant__ GridDe
     const double dt = a.dt_dev ? __ldg(a.dt_dev) : a.dt;
     if (i < g.n[0]) {
         const long long id = (i + g.gh[0]) + (j + g.gh[1]) * g.stride[1] + (k + g.gh[2]) * g.stride[2];
-        double E = a.U[0][id];
+        const double E = a.U[0][id];
         double F[3] = {a.U[1][id], a.U[2][id], a.U[3][id]};
         const double rho = a.rho[id];
         const double T0 = a.T[id];
-        double m[3];
+        double m[3] = {0.0, 0.0, 0.0};
         if (FEEDBACK) {
 #pragma unroll
             for (int q = 0; q < 3; ++q) m[q] = a.mom[q][id];
         }
-        if (E < par.E_floor) {
-            E = par.E_floor;
-            floored = true;
-        }
-        const double F2 = fma(F[2], F[2], fma(F[1], F[1], F[0] * F[0]));
-        if (F2 > E * E) {
-            const double sc = E * rsqrt(F2);
-#pragma unroll
-            for (int q = 0; q < 3; ++q) F[q] *= sc;
-            clipped = true;
-        }
-        LogRT lg = {0.0, 0.0};
-        const bool share = a.os.share != 0;
-        if (share) lg = log_inputs(a.os.src == 0 ? oP : (a.os.src == 1 ? oR : oS), rho, T0);
-        const double kP = opacity_eval_shared(oP, rho, T0, share, lg);
-        const double kR = a.same_PR ? kP : opacity_eval_shared(oR, rho, T0, share, lg);
-        const double chi = kR + opacity_eval_shared(oS, rho, T0, share, lg);
-        const double gr = dt * par.chat * kP * rho;
-        const double gg = dt * par.c * kP * rho;
-        const double Cv = rho * par.c_v;
-        const double aT3 = par.a_R * T0 * T0 * T0;
-        const double aT4 = aT3 * T0;
-        const double det = fma(Cv, 1.0 + gr, 4.0 * gg * aT3);
-        const double idet = frcp(det);
-        const double En = fma(E, fma(4.0 * gg, aT3, Cv), gr * Cv * aT4) * idet;
-        const double Tn = fma((1.0 + gr) * Cv, T0, fma(3.0 * gg, aT4, gg * E)) * idet;
-        const double idamp = frcp(fma(dt * par.chat * chi, rho, 1.0));
-        a.U[0][id] = En;
-        a.T[id] = Tn;
-        const double ichat = a.ichat;
-        double Fn[3];
-#pragma unroll
-        for (int q = 0; q < 3; ++q) {
-            Fn[q] = F[q] * idamp;
-            if (FEEDBACK) a.mom[q][id] = fma(-(Fn[q] - F[q]), ichat, m[q]);
-            a.U[1 + q][id] = Fn[q];
-        }
-        if (CFL) rate = cell_rate(g, par.chat, En, Fn[0], Fn[1], Fn[2], i, j, k);
+        rate = implicit_cell<FEEDBACK, CFL>(g, par, oP, oR, oS, a, dt, id, i, j, k, E, F, rho, T0, m, floored, clipped);
     }
-    if (CFL) {
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) rate = dmax(rate, __shfl_xor_sync(0xffffffffu, rate, o));
-        if ((threadIdx.x & 31) == 0) {
-            const unsigned long long bits = (unsigned long long)__double_as_longlong(rate);
-            if (bits > *(volatile unsigned long long*)&a.scr->rate_bits) atomicMax(&a.scr->rate_bits, bits);
-        }
-    }
-    // rare: count floor / clip activations (debug counters, SURVEY.md Sect. 8(d) "Parity")
-    const unsigned mf = __ballot_sync(0xffffffffu, floored), mc = __ballot_sync(0xffffffffu, clipped);
-    if ((mf | mc) && (threadIdx.x & 31) == 0) {
-        if (mf) atomicAdd(&a.counters[0], (unsigned long long)__popc(mf));
-        if (mc) atomicAdd(&a.counters[1], (unsigned long long)__popc(mc));
-    }
+    implicit_warp_epilogue<CFL>(a, rate, floored ? 1 : 0, clipped ? 1 : 0);
 }
 
 }  // namespace rtm1

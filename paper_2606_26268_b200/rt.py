@@ -20,7 +20,7 @@ SOLVER_HLL, SOLVER_GLF = 0, 1
 OPAC_PLANCK, OPAC_ROSSELAND, OPAC_SCATTER = 0, 1, 2
 OK, ERR_INVALID_ARG, ERR_BAD_STATE, ERR_CUDA, ERR_NOT_FINITE = 0, 1, 2, 3, 4
 NGHOST = 2
-KERNEL_KINDS = ("ghost_fill", "thick_limit", "sweep_x1", "sweep_x2", "sweep_x3", "implicit", "cfl")
+KERNEL_KINDS = ("ghost_fill", "thick_limit", "sweep_x1", "sweep_x2", "sweep_x3", "implicit", "cfl", "fused")
 NKERNEL_KINDS = 8
 
 _dp = C.POINTER(C.c_double)
@@ -212,8 +212,8 @@ class Grid:
         if rc != OK:
             self._raise("rt_set_opacity", rc)
 
-    def set_tuning(self, march_len=0):
-        rc = lib().rt_set_tuning(self._h, int(march_len), 0)
+    def set_tuning(self, march_len=0, fused_seg=0):
+        rc = lib().rt_set_tuning(self._h, int(march_len), int(fused_seg))
         if rc != OK:
             self._raise("rt_set_tuning", rc)
 

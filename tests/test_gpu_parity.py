@@ -50,15 +50,23 @@ def to_host(ts):
     return [t.cpu().numpy() for t in ts]
 
 
-def run_both(rt, w, nsub, dts=None):
-    """nsub sub-steps on both sides with one dt sequence (the oracle's CFL unless given)."""
+def run_both(rt, w, nsub, dts=None, fused=False, fused_seg=0):
+    """nsub sub-steps on both sides.  fused=False: rt_explicit_step + rt_implicit_step with one dt sequence (the
+    oracle's CFL unless given).  fused=True: rt_substep (ONE fused kernel on 3-D grids, device-resident dt)
+    against the oracle stepping with its own CFL; fused_seg = its x3 segment length (0 = automatic)."""
     og = ort.grid_from_workload(w)
     if dts is None:
         refU, refT, refm, dts = ort.run_substeps(og, w, nsub)
     else:
         refU, refT, refm, _ = ort.run_substeps(og, w, nsub, dts=dts)
     g = rt.grid_from_workload(w)
-    st, _ = rt.run_substeps(g, w, nsub, dts=dts)
+    if fused:
+        g.set_tuning(fused_seg=fused_seg)
+        st, _, hist = rt.run_substeps_fused(g, w, nsub)
+        used = hist.cpu().numpy()
+        assert np.all(np.abs(used - np.array(dts)) <= (1e-12 if nsub <= 5 else 1e-9) * np.array(dts)), (used, dts)
+    else:
+        st, _ = rt.run_substeps(g, w, nsub, dts=dts)
     torch.cuda.synchronize()
     gpuU = to_host(st.U)
     gpuT = st.T.cpu().numpy()
@@ -269,6 +277,62 @@ def test_uniform_state_is_preserved_on_the_gpu(rt):
         assert torch.all((a - b).abs() <= 2e-16 * 1.7), q
 
 
+# ----------------------------------------------------------------------------- the fused 3-D kernel
+# k_substep_fused owns 30 x 6 cells per CTA and marches x3 in segments: (141, 37, 35) leaves ragged tiles in x1
+# and x2; fused_seg = 12 cuts x3 into segments of 12 + 12 + 11, 0 = the library's own choice
+@pytest.mark.parametrize("geometry", [W.CARTESIAN, W.CYLINDRICAL, W.SPHERICAL])
+@pytest.mark.parametrize("solver", [W.SOLVER_HLL, W.SOLVER_GLF])
+@pytest.mark.parametrize("thick", [0, 1])
+def test_fused_kernel_one_substep_random_states(rt, geometry, solver, thick):
+    w = random_workload(geometry, (141, 37, 35), solver, thick, seed=100 + 10 * geometry + 2 * solver + thick)
+    for seg in (0, 12):
+        errs, counts, _ = run_both(rt, w, 1, fused=True, fused_seg=seg)
+        assert_below(errs, TOL1, "fused kernel, one sub-step, seg %d" % seg)
+        assert counts[0] == counts[1]
+
+
+@pytest.mark.parametrize("n", [(2, 2, 2), (31, 7, 3), (30, 6, 40), (61, 13, 2), (3, 50, 5)])
+def test_fused_kernel_small_and_ragged_shapes(rt, n):
+    w = random_workload(W.CARTESIAN, n, W.SOLVER_HLL, 1, seed=23 + sum(n))
+    errs, counts, _ = run_both(rt, w, 1, fused=True)
+    assert_below(errs, TOL1, "fused kernel, shape %s" % (n,))
+    assert counts[0] == counts[1]
+
+
+def test_fused_kernel_tables_boundaries_no_feedback(rt):
+    w = random_workload(W.SPHERICAL, (50, 34, 20), W.SOLVER_HLL, 1, seed=5, bc=(3, 1, 2, 1, 0, 0), table=True)
+    errs, _, _ = run_both(rt, w, 1, fused=True, fused_seg=7)
+    assert_below(errs, TOL1, "fused kernel, table opacities")
+    w = random_workload(W.CARTESIAN, (64, 20, 16), W.SOLVER_GLF, 1, seed=6, bc=(1, 1, 2, 2, 0, 0), feedback=0)
+    errs, _, _ = run_both(rt, w, 1, fused=True)
+    assert_below(errs, TOL1, "fused kernel, no momentum feedback")
+
+
+def test_fused_kernel_streaming_limit(rt):
+    w = streaming_workload(9, exact=True)
+    errs, counts, _ = run_both(rt, w, 1, fused=True, fused_seg=4)
+    assert_below(errs, TOL1, "fused kernel, f = 1 exactly")
+    assert counts[0][0] == counts[1][0]
+
+
+def test_fused_kernel_equals_per_direction_kernels(rt):
+    """same sub-step through the fused kernel and through the per-direction kernels: same formulas, another
+    summation order of the three flux differences -> a few ulp"""
+    w = random_workload(W.SPHERICAL, (67, 33, 18), W.SOLVER_HLL, 1, seed=77, table=True)
+    res = []
+    for seg in (0, -1):
+        g = rt.grid_from_workload(w)
+        g.set_tuning(fused_seg=seg)
+        st, dtn, _ = rt.run_substeps_fused(g, w, 3)
+        res.append((to_host(st.U), st.T.cpu().numpy(), float(dtn.item())))
+    it = w.interior
+    Es = np.abs(res[0][0][0][it]).max()
+    for q in range(4):
+        assert np.abs(res[0][0][q][it] - res[1][0][q][it]).max() <= 1e-13 * Es, q
+    assert np.abs(res[0][1][it] - res[1][1][it]).max() <= 1e-13 * np.abs(res[1][1][it]).max()
+    assert abs(res[0][2] - res[1][2]) <= 1e-13 * res[1][2]
+
+
 # ----------------------------------------------------------------------------- fused sub-step (device-resident dt)
 @pytest.mark.parametrize("geometry,n,table", [(W.CARTESIAN, (70, 33, 9), False), (W.SPHERICAL, (45, 20, 11), True),
                                               (W.CARTESIAN, (300, 1, 1), False), (W.CYLINDRICAL, (33, 7, 1), False)])
@@ -343,37 +407,42 @@ def test_config2_beam_shadow_reduced_and_full_width(rt):
     assert counts[0][1] == counts[1][1]
 
 
-def test_config3_turbulent_box_128_full_length(rt):
+@pytest.mark.parametrize("fused", [False, True])
+def test_config3_turbulent_box_128_full_length(rt, fused):
     w = W.c3()
-    errs1, _, _ = run_both(rt, w, 1)
+    errs1, _, _ = run_both(rt, w, 1, fused=fused)
     assert_below(errs1, TOL1, "C3 1 sub-step")
-    errs, counts, _ = run_both(rt, w, 100)
+    errs, counts, _ = run_both(rt, w, 100, fused=fused)
     assert_below(errs, TOL100, "C3 100 sub-steps")
     assert counts[0] == counts[1]
 
 
-def test_config4_two_opacities_alternating_solvers(rt):
+@pytest.mark.parametrize("fused", [False, True])
+def test_config4_two_opacities_alternating_solvers(rt, fused):
     w = W.c4(nside=96)
-    errs, counts, _ = run_both(rt, w, 100)       # HLL / GLF alternate every sub-step
+    errs, counts, _ = run_both(rt, w, 100, fused=fused)       # HLL / GLF alternate every sub-step
     assert_below(errs, TOL100, "C4 96^3 100 sub-steps")
     assert counts[0] == counts[1]
 
 
-def test_config5_spherical_disc_reduced_full_length(rt):
+@pytest.mark.parametrize("fused", [False, True])
+def test_config5_spherical_disc_reduced_full_length(rt, fused):
     w = W.c5(n=(128, 64, 128))
-    errs1, _, _ = run_both(rt, w, 1)
+    errs1, _, _ = run_both(rt, w, 1, fused=fused)
     assert_below(errs1, TOL1, "C5 128x64x128 1 sub-step")
-    errs, counts, _ = run_both(rt, w, 50)
+    errs, counts, _ = run_both(rt, w, 50, fused=fused)
     assert_below(errs, TOL100, "C5 128x64x128 50 sub-steps")
     assert counts[0] == counts[1]
 
 
 @pytest.mark.parametrize("name", ["C4", "C5"])
-def test_full_size_configs_in_the_bench_launch_configuration(rt, name):
+@pytest.mark.parametrize("fused", [True, False])
+def test_full_size_configs_in_the_bench_launch_configuration(rt, name, fused):
     """BASELINE.json's full sizes (256^3, 256x128x256): two sub-steps (HLL then GLF for C4), every cell
-    compared; the same calls bench.py times."""
+    compared; fused=True is the call bench.py times (rt_substep -> k_substep_fused), fused=False the
+    three-call form of `bench.py --api split`."""
     w = W.BY_NAME[name]()
-    errs1, counts, _ = run_both(rt, w, 2)
+    errs1, counts, _ = run_both(rt, w, 2, fused=fused)
     assert_below(errs1, TOL1 * 2, name + " full size, 2 sub-steps")
     assert counts[0] == counts[1]
 
