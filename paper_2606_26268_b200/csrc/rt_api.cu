@@ -4,6 +4,7 @@
 #include <math.h>
 #include <stdarg.h>
 #include <stdio.h>
+#include <stdlib.h>
 #include <string.h>
 
 #include <new>
@@ -32,6 +33,7 @@ struct rt_grid {
     rt_opacity opac_host[3];
     int same_PR;
     int march_len;
+    int fused_tma_off;  // test hook (env RT_M1_NO_TMA at grid creation): stage the planes by cp.async even where TMA could
     int fused_seg;  // rt_set_tuning: 0 auto, -1 never use the fused sub-step kernel, > 0 its x3 segment length
     long long launches;
     // optional per-kernel device timing (rt_set_profiling): one event pair per launch
@@ -158,6 +160,10 @@ extern "C" int32_t rt_grid_create(int32_t geometry, const int32_t n[3], int32_t 
     g->same_PR = 0;
     g->march_len = 0;
     g->fused_seg = 0;
+    {
+        const char* e = getenv("RT_M1_NO_TMA");
+        g->fused_tma_off = (e && e[0] == '1') ? 1 : 0;
+    }
     g->launches = 0;
     g->profiling = 0;
     g->err[0] = 0;
@@ -581,8 +587,47 @@ extern "C" int32_t rt_implicit_step_cfl(rt_grid* g, double dt, const double* rho
 
 // ------------------------------------------------------------------------------------------------
 // Fused sub-step (3-D grids): ghost fill -> thick-limit pre-pass -> k_substep_fused -> k_cfl_finalize
+// cuTensorMapEncodeTiled through the runtime's driver entry point lookup: no link-time dependency on libcuda
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+static EncodeTiledFn encode_tiled_fn() {
+    static EncodeTiledFn fn = nullptr;
+    static bool tried = false;
+    if (!tried) {
+        tried = true;
+        void* p = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess && q == cudaDriverEntryPointSuccess)
+            fn = (EncodeTiledFn)p;
+        cudaGetLastError();
+    }
+    return fn;
+}
+
+// TMA descriptors of the staged arrays: ghosted (nt1, nt2, nt3) fp64 tensors, box 34 x FPH x 1, zero fill outside.
+// false when the TMA cannot address them (row pitch or base not a multiple of 16 B, or no encoder).
+static bool fused_make_maps(const rt_grid* g, const FusedArgs& a, int narr, FusedMaps* maps) {
+    const GridDev& D = g->dev;
+    if ((D.nt[0] & 1) != 0) return false;
+    EncodeTiledFn enc = encode_tiled_fn();
+    if (!enc) return false;
+    const cuuint64_t gdim[3] = {(cuuint64_t)D.nt[0], (cuuint64_t)D.nt[1], (cuuint64_t)D.nt[2]};
+    const cuuint64_t gstr[2] = {(cuuint64_t)D.nt[0] * 8u, (cuuint64_t)D.nt[0] * (cuuint64_t)D.nt[1] * 8u};
+    const cuuint32_t box[3] = {(cuuint32_t)FPW, (cuuint32_t)FPH, 1u};
+    const cuuint32_t estr[3] = {1u, 1u, 1u};
+    for (int q = 0; q < narr; ++q) {
+        if ((reinterpret_cast<uintptr_t>(a.src[q]) & 15u) != 0) return false;
+        if (enc(&maps->m[q], CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, const_cast<double*>(a.src[q]), gdim, gstr, box, estr,
+                CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+            return false;
+    }
+    return true;
+}
+
 template <bool HLL, bool THICK, bool CURVI, bool FEEDBACK>
-static cudaError_t launch_fused_t(rt_grid* g, const ParamsDev& P, const FusedArgs& a, dim3 grid, int seglen) {
+static cudaError_t launch_fused_t(rt_grid* g, const ParamsDev& P, const FusedArgs& a, const FusedMaps& maps, dim3 grid, int seglen) {
     auto kern = k_substep_fused<HLL, THICK, CURVI, FEEDBACK>;
     static bool attr_done = false;
     if (!attr_done) {
@@ -590,15 +635,15 @@ static cudaError_t launch_fused_t(rt_grid* g, const ParamsDev& P, const FusedArg
         if (e != cudaSuccess) return e;
         attr_done = true;
     }
-    kern<<<grid, dim3(32, FNY), kFusedSmemBytes, g->stream>>>(g->dev, P, g->opac[0], g->opac[1], g->opac[2], a, seglen);
+    kern<<<grid, dim3(32, FNY), kFusedSmemBytes, g->stream>>>(g->dev, P, g->opac[0], g->opac[1], g->opac[2], a, maps, seglen);
     return cudaSuccess;
 }
 
 static cudaError_t launch_fused(rt_grid* g, bool hll, bool thick, bool curvi, bool feedback, const ParamsDev& P,
-                                const FusedArgs& a, dim3 grid, int seglen) {
+                                const FusedArgs& a, const FusedMaps& maps, dim3 grid, int seglen) {
     const int key = (hll ? 8 : 0) | (thick ? 4 : 0) | (curvi ? 2 : 0) | (feedback ? 1 : 0);
     switch (key) {
-#define RT_FUSED_CASE(K, A, B, C_, D_) case K: return launch_fused_t<A, B, C_, D_>(g, P, a, grid, seglen);
+#define RT_FUSED_CASE(K, A, B, C_, D_) case K: return launch_fused_t<A, B, C_, D_>(g, P, a, maps, grid, seglen);
         RT_FUSED_CASE(0, false, false, false, false)
         RT_FUSED_CASE(1, false, false, false, true)
         RT_FUSED_CASE(2, false, false, true, false)
@@ -614,7 +659,7 @@ static cudaError_t launch_fused(rt_grid* g, bool hll, bool thick, bool curvi, bo
         RT_FUSED_CASE(12, true, true, false, false)
         RT_FUSED_CASE(13, true, true, false, true)
         RT_FUSED_CASE(14, true, true, true, false)
-        default: return launch_fused_t<true, true, true, true>(g, P, a, grid, seglen);
+        default: return launch_fused_t<true, true, true, true>(g, P, a, maps, grid, seglen);
 #undef RT_FUSED_CASE
     }
 }
@@ -697,9 +742,12 @@ static int32_t fused_impl(rt_grid* g, double* dt_device, double cfl, const doubl
     const int tx = (D.n[0] + FTX - 1) / FTX, ty = (D.n[1] + FTY - 1) / FTY;
     const int seglen = fused_segment_length(g, tx * ty);
     dim3 grid(tx, ty, (D.n[2] + seglen - 1) / seglen);
+    FusedMaps maps;
+    memset(&maps, 0, sizeof(maps));
+    a.use_tma = (g->fused_tma_off == 0 && fused_make_maps(g, a, thick ? 5 : 4, &maps)) ? 1 : 0;
     {
         ProfScope ps(g, RT_K_FUSED);
-        cudaError_t e = launch_fused(g, g->par.solver == RT_SOLVER_HLL, thick, D.geometry != RT_CARTESIAN, feedback, P, a, grid, seglen);
+        cudaError_t e = launch_fused(g, g->par.solver == RT_SOLVER_HLL, thick, D.geometry != RT_CARTESIAN, feedback, P, a, maps, grid, seglen);
         if (e != cudaSuccess) return fail(g, RT_ERR_CUDA, "k_substep_fused attribute: %s", cudaGetErrorString(e));
     }
     RT_LAUNCH_CHECK(g);

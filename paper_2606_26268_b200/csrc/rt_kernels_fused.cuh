@@ -3,19 +3,28 @@
 //
 // Design.  A CTA owns an x1-x2 tile of 30 x FTY cells and marches
 // along x3 through a segment [ka, kb).  The x1-x2 planes of U^n (and of the thick-limit array) it
-// needs — tile + 2 ghost cells on each side — are staged in shared memory by cp.async into a ring of
-// four planes (c-1, c, c+1 in use, c+2 in flight), so every stencil value is read from HBM/L2 once per
-// CTA and the loads never occupy registers.  Thread (lx, ly) owns cell (i0-1+lx, j0-1+ly): lanes 0 and
-// 31 and rows 0 and FTY+1 are the halo whose face states the tile's outer faces need.  Per plane c:
+// needs — tile + 2 ghost cells on each side — are staged in shared memory by TMA (one
+// cp.async.bulk.tensor.3d box of 34 x (FTY+4) x 1 doubles per field and plane, issued by one thread,
+// completion on an mbarrier) into a ring of four planes (c-1, c, c+1 in use, c+2 in flight): every
+// stencil value is read from HBM/L2 once per CTA, the loads occupy no registers and no issue slots, and
+// boxes hanging over the array edge are zero-filled by the hardware.  Arrays the TMA cannot address
+// (odd x1 extent => row pitch not a multiple of 16 B, or a base pointer not 16-B aligned) take an
+// 8-byte cp.async loop instead.  Thread (lx, ly) owns cell (i0-1+lx, j0-1+ly): lanes 0 and 31 and rows 0
+// and FTY+1 are the halo whose face states the tile's outer faces need.  Per plane c:
 //   Z  : both x3 face states of cell c (Eq. 17-21 + closure + speeds), Riemann flux at face c-1/2 against
 //        the upper-face state of cell c-1 kept in this thread's shared-memory slot;
 //   FIN: cell c-1 is complete: U* = acc - dt/V [A F]_z, then floor/clip, opacities, implicit coupling
 //        (Eq. 29-33, 30, 28), stores, CFL rate of the updated state (a8-a11);
-//   Y  : x2 face states; upper-face states and face fluxes are exchanged through shared memory;
+//   Y  : x2 face states; the upper-face state goes to the row above through shared memory, guarded by a
+//        64-thread named barrier per row pair (producer bar.arrive, consumer bar.sync), and the flux of the
+//        upper face comes back the same way one step later (after the per-plane __syncthreads);
 //   X  : x1 face states; exchanged by warp shuffles; + geometric sources;   acc = U^n - dt/V([AF]_x + [AF]_y).
-// Every closure, wave speed and Riemann flux is evaluated once per face inside the tile; the halo costs
-// 32/30 in x1 and (3 FTY + 1)/(3 FTY) in x2.  Face states, fluxes and U* never touch HBM.
+// One __syncthreads per plane.  Every closure, wave speed and Riemann flux is evaluated once per face inside
+// the tile; the halo costs 32/30 in x1 and (3 FTY + 1)/(3 FTY) in x2.  Face states, fluxes and U* never
+// touch HBM.
 #pragma once
+#include <cuda.h>  // CUtensorMap (type only: the encoder is fetched through cudaGetDriverEntryPoint)
+
 #include "rt_kernels_step.cuh"
 
 namespace rtm1 {
@@ -27,15 +36,27 @@ constexpr int FNT = 32 * FNY;     // threads per CTA
 constexpr int FPW = 34;           // staged plane width  (cells i0-2 .. i0+31)
 constexpr int FPH = FTY + 4;      // staged plane height (cells j0-2 .. j0+FTY+1)
 constexpr int FPHW = FPW * FPH;
+constexpr int FPS = (FPHW + 15) / 16 * 16;  // doubles between staged arrays: every TMA destination 128-B aligned
 constexpr int FNARR = 5;          // E, F1, F2, F3, lim
 constexpr int FNSLOT = 4;
 constexpr int FNST = 10;          // doubles of an exchanged face state: U[4], G[4], lm, lp
-constexpr size_t kFusedSmemBytes = sizeof(double) * (size_t)(FNSLOT * FNARR * FPHW + 2 * FNST * FNT + 4 * FNT);
+constexpr int FNI = 32 * FTY;        // threads of the interior rows 1..FTY       (slot t - 32)
+constexpr int FNP = 32 * (FTY + 1);  // threads of rows 0..FTY (state producers) or 1..FTY+1 (flux producers)
+// staged planes | zhi[FNST][FNI] | yhi[FNST][FNP] | yfl[4][FNP] | fin[2][4][FNI] | mbarriers
+constexpr size_t kFusedSmemBytes =
+    sizeof(double) * (size_t)(FNSLOT * FNARR * FPS + FNST * FNI + FNST * FNP + 4 * FNP + 2 * 4 * FNI) +
+    FNSLOT * sizeof(unsigned long long);
+static_assert(FTY + 1 <= 15, "one named barrier per row pair");
+static_assert(FTY % 2 == 0, "the two halo warps share the implicit half of the FTY rows");
 
 struct FusedArgs {
     const double* src[FNARR];  // U_in[4], lim (or nullptr)
     ImplicitArgs im;           // U = U_out, rho, T, mom, dt / dt_dev, scratch, counters
     double chat;
+    int use_tma;
+};
+struct alignas(64) FusedMaps {
+    CUtensorMap m[FNARR];      // ghosted (nt1, nt2, nt3) fp64 tensors, box 34 x FPH x 1
 };
 
 __device__ __forceinline__ void cp_async8(double* smem_dst, const double* gsrc) {
@@ -45,44 +66,81 @@ __device__ __forceinline__ void cp_async8(double* smem_dst, const double* gsrc) 
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
 
-template <bool HLL>
+__device__ __forceinline__ void mbar_init(unsigned long long* bar, unsigned count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"((unsigned)__cvta_generic_to_shared(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned long long* bar, unsigned bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"((unsigned)__cvta_generic_to_shared(bar)), "r"(bytes)
+                 : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned parity) {
+    const unsigned b = (unsigned)__cvta_generic_to_shared(bar);
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE_%=;\n"
+        "bra WAIT_%=;\n"
+        "DONE_%=:\n"
+        "}\n" ::"r"(b),
+        "r"(parity)
+        : "memory");
+}
+__device__ __forceinline__ void tma_load_3d(double* smem_dst, const CUtensorMap* map, int x, int y, int z, unsigned long long* bar) {
+    asm volatile(
+        "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];" ::"r"(
+            (unsigned)__cvta_generic_to_shared(smem_dst)),
+        "l"(map), "r"(x), "r"(y), "r"(z), "r"((unsigned)__cvta_generic_to_shared(bar))
+        : "memory");
+}
+// 64-thread named barriers: the producer warp arrives, the consumer warp waits
+__device__ __forceinline__ void pair_arrive(int id) { asm volatile("bar.arrive %0, 64;" ::"r"(id) : "memory"); }
+__device__ __forceinline__ void pair_sync(int id) { asm volatile("bar.sync %0, 64;" ::"r"(id) : "memory"); }
+__device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
+
+// a face state in shared memory: component-major, N slots per component (conflict-free)
+template <bool HLL, int N>
 __device__ __forceinline__ void state_store(double* buf, int t, const State& s) {
 #pragma unroll
     for (int q = 0; q < 4; ++q) {
-        buf[q * FNT + t] = s.U[q];
-        buf[(4 + q) * FNT + t] = s.G[q];
+        buf[q * N + t] = s.U[q];
+        buf[(4 + q) * N + t] = s.G[q];
     }
     if (HLL) {
-        buf[8 * FNT + t] = s.lm;
-        buf[9 * FNT + t] = s.lp;
+        buf[8 * N + t] = s.lm;
+        buf[9 * N + t] = s.lp;
     }
 }
-template <bool HLL>
+template <bool HLL, int N>
 __device__ __forceinline__ void state_load(const double* buf, int t, State& s) {
 #pragma unroll
     for (int q = 0; q < 4; ++q) {
-        s.U[q] = buf[q * FNT + t];
-        s.G[q] = buf[(4 + q) * FNT + t];
+        s.U[q] = buf[q * N + t];
+        s.G[q] = buf[(4 + q) * N + t];
     }
     if (HLL) {
-        s.lm = buf[8 * FNT + t];
-        s.lp = buf[9 * FNT + t];
+        s.lm = buf[8 * N + t];
+        s.lp = buf[9 * N + t];
     } else {
         s.lm = 0.0;
         s.lp = 0.0;
     }
 }
 
+
 template <bool HLL, bool THICK, bool CURVI, bool FEEDBACK>
 __global__ void __launch_bounds__(FNT, 2)
     k_substep_fused(const __grid_constant__ GridDev g, const __grid_constant__ ParamsDev par, const __grid_constant__ OpacDev oP,
                     const __grid_constant__ OpacDev oR, const __grid_constant__ OpacDev oS, const __grid_constant__ FusedArgs a,
-                    int seglen) {
-    extern __shared__ double sm[];
+                    const __grid_constant__ FusedMaps maps, int seglen) {
+    extern __shared__ __align__(128) double sm[];
     double* const planes = sm;
-    double* const zhi = planes + FNSLOT * FNARR * FPHW;
-    double* const yhi = zhi + FNST * FNT;
-    double* const yfl = yhi + FNST * FNT;
+    double* const zhi = planes + FNSLOT * FNARR * FPS;  // [FNST][FNI]  own slot: upper x3 face state of the previous plane
+    double* const yhi = zhi + FNST * FNI;               // [FNST][FNP]  upper x2 face states of rows 0..FTY
+    double* const yfl = yhi + FNST * FNP;               // [4][FNP]     fluxes through the lower x2 faces of rows 1..FTY+1
+    double* const fin = yfl + 4 * FNP;                  // [2][4][FNI]  U* of the interior rows, for the implicit half
+    unsigned long long* const mbar = (unsigned long long*)(fin + 2 * 4 * FNI);  // [FNSLOT]
 
     const int lx = threadIdx.x, ly = threadIdx.y;
     const int tid = ly * 32 + lx;
@@ -91,70 +149,98 @@ __global__ void __launch_bounds__(FNT, 2)
     const int kb = min(ka + seglen, g.n[2]);
     const int i = i0 - 1 + lx, j = j0 - 1 + ly;
     const bool row_in = (ly >= 1) && (ly <= FTY);
-    const bool writer = row_in && lx >= 1 && lx <= FTX && i < g.n[0] && j < g.n[1];
     const int ic = min(max(i, 0), g.n[0] - 1), jc = min(max(j, 0), g.n[1] - 1);
     const int o = (ly + 1) * FPW + lx + 1;  // this thread's cell inside a staged plane
-
+    const bool tma = a.use_tma != 0;
     const double dt = a.im.dt_dev ? __ldg(a.im.dt_dev) : a.im.dt;
     const double dtc = dt * a.chat;
-    const double kx = dtc * g.cg[0][0][ic] * g.cg[0][1][jc];
-    const double ky = dtc * g.cg[1][0][ic] * g.cg[1][1][jc];
-    const double kz = dtc * g.cg[2][0][ic] * g.cg[2][1][jc];
-    double wx = 1.0, wy = 1.0;
-    if (CURVI) {
-        wx = g.wf[0][min(max(i, 0), g.n[0])];
-        wy = g.wf[1][min(max(j, 0), g.n[1])];
-    }
-    // element index of cell (i, j, 0) in the ghosted arrays
-    const long long id0 = (ic + g.gh[0]) + (long long)(jc + g.gh[1]) * g.stride[1] + (long long)g.gh[2] * g.stride[2];
 
     constexpr int NA = THICK ? 5 : 4;
-    auto load_plane = [&](int c) {
-        double* dst = planes + ((c + 4) & 3) * (FNARR * FPHW);
-        const long long zoff = (long long)(c + g.gh[2]) * g.stride[2];
-        for (int e = tid; e < NA * FPHW; e += FNT) {
-            const int arr = e / FPHW, r = e - arr * FPHW;
-            const int row = r / FPW, col = r - row * FPW;
-            const int gi = min(i0 + col, g.nt[0] - 1), gj = min(j0 + row, g.nt[1] - 1);
-            cp_async8(dst + e, a.src[arr] + zoff + (long long)gj * g.stride[1] + gi);
+    if (tma) {
+        if (tid == 0) {
+#pragma unroll
+            for (int s = 0; s < FNSLOT; ++s) mbar_init(mbar + s, 1);
+            asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+            asm volatile("fence.proxy.async;" ::: "memory");
         }
-        cp_async_commit();
+        __syncthreads();
+    }
+    // stage plane cc (x3 cell index, -2 .. n3+1) into ring slot (cc + 4) & 3
+    auto load_plane = [&](int cc) {
+        const int slot = (cc + 4) & 3;
+        double* dst = planes + slot * (FNARR * FPS);
+        if (tma) {
+            if (tid == 0) {
+                mbar_expect_tx(mbar + slot, (unsigned)(NA * FPHW * sizeof(double)));
+#pragma unroll
+                for (int arr = 0; arr < NA; ++arr) tma_load_3d(dst + arr * FPS, &maps.m[arr], i0, j0, cc + g.gh[2], mbar + slot);
+            }
+        } else {
+            const long long zoff = (long long)(cc + g.gh[2]) * g.stride[2];
+            for (int e = tid; e < NA * FPHW; e += FNT) {
+                const int arr = e / FPHW, r = e - arr * FPHW;
+                const int row = r / FPW, col = r - row * FPW;
+                const int gi = min(i0 + col, g.nt[0] - 1), gj = min(j0 + row, g.nt[1] - 1);
+                cp_async8(dst + arr * FPS + r, a.src[arr] + zoff + (long long)gj * g.stride[1] + gi);
+            }
+            cp_async_commit();
+        }
+    };
+    // plane p of this segment is the ((p - ka + 2) >> 2)-th use of its slot
+    auto wait_plane = [&](int p) {
+        if (tma) mbar_wait(mbar + ((p + 4) & 3), (unsigned)(((p - ka + 2) >> 2) & 1));
+    };
+    // top of step c: plane c+1 has landed and is visible to all; every warp is done with step c-1
+    auto step_begin = [&](int c) {
+        if (c + 1 <= kb + 1) {
+            if (tma) wait_plane(c + 1); else cp_async_wait_all();
+        }
+        __syncthreads();
+        if (c + 2 <= kb + 1) load_plane(c + 2);
     };
     load_plane(ka - 2);
     load_plane(ka - 1);
     load_plane(ka);
+    wait_plane(ka - 2);
+    wait_plane(ka - 1);
 
-    double acc[4] = {0.0, 0.0, 0.0, 0.0};  // U^n - dt/V ([AF]_x + [AF]_y) + dt S_geo of the previous plane's cell
-    double Fz[4] = {0.0, 0.0, 0.0, 0.0};   // area-weighted flux through the lower x3 face of that cell
-    int nfloor = 0, nclip = 0;  // cells of this thread whose floor / clip fired
-    double rate = 0.0;
-
+    if (row_in) {
+        // ================================================================ interior rows: transport
+        const int ti = tid - 32;  // slot among the interior rows
+        const double kx = dtc * g.cg[0][0][ic] * g.cg[0][1][jc];
+        const double ky = dtc * g.cg[1][0][ic] * g.cg[1][1][jc];
+        const double kz = dtc * g.cg[2][0][ic] * g.cg[2][1][jc];
+        double wx = 1.0, wy = 1.0;
+        if (CURVI) {
+            wx = g.wf[0][min(max(i, 0), g.n[0])];
+            wy = g.wf[1][min(max(j, 0), g.n[1])];
+        }
+        double acc[4] = {0.0, 0.0, 0.0, 0.0};  // U^n - dt/V ([AF]_x + [AF]_y) + dt S_geo of the previous plane's cell,
+                                               // still missing the flux through its upper x2 face (held by the row above)
+        double Fz[4] = {0.0, 0.0, 0.0, 0.0};   // area-weighted flux through the lower x3 face of that cell
 #pragma unroll 1
-    for (int c = ka - 1; c <= kb; ++c) {
-        cp_async_wait_all();
-        __syncthreads();
-        if (c + 2 <= kb + 1) load_plane(c + 2);
-        const double* pc = planes + ((c + 4) & 3) * (FNARR * FPHW);
-
-        if (row_in) {
-            // ---------------------------------------------------------------- Z
-            const double* pm = planes + ((c + 3) & 3) * (FNARR * FPHW);
-            const double* pp = planes + ((c + 5) & 3) * (FNARR * FPHW);
-            double flz[4];
+        for (int c = ka - 1; c <= kb + 1; ++c) {  // step kb+1: the halo warps finish cell kb-1
+            step_begin(c);
+            if (c > kb) break;
+            const double* pc = planes + ((c + 4) & 3) * (FNARR * FPS);
+            // ------------------------------------------------------------ Z
             {
+                const double* pm = planes + ((c + 3) & 3) * (FNARR * FPS);
+                const double* pp = planes + ((c + 5) & 3) * (FNARR * FPS);
                 double q0[4], dm[4], dp[4];
 #pragma unroll
                 for (int q = 0; q < 4; ++q) {
-                    q0[q] = pc[q * FPHW + o];
-                    dm[q] = q0[q] - pm[q * FPHW + o];
-                    dp[q] = pp[q * FPHW + o] - q0[q];
+                    q0[q] = pc[q * FPS + o];
+                    dm[q] = q0[q] - pm[q * FPS + o];
+                    dp[q] = pp[q * FPS + o] - q0[q];
                 }
                 State lo, hi;
-                cell_faces<2, HLL>(q0, dm, dp, c >= ka, c < kb, lo, hi);
+                cell_faces<2, HLL>(q0, dm, dp, true, true, lo, hi);  // both always: one basic block, two independent chains
+                double flz[4] = {0.0, 0.0, 0.0, 0.0};
                 if (c >= ka) {
                     State L;
-                    state_load<HLL>(zhi, tid, L);
-                    const double limd = THICK ? dmax(pm[4 * FPHW + o], pc[4 * FPHW + o]) : kInf;
+                    state_load<HLL, FNI>(zhi, ti, L);
+                    const double limd = THICK ? dmax(pm[4 * FPS + o], pc[4 * FPS + o]) : kInf;
                     riemann<HLL>(L, lo, limd, flz);
                     if (CURVI) {
                         const double w = g.wf[2][c];
@@ -162,122 +248,212 @@ __global__ void __launch_bounds__(FNT, 2)
                         for (int q = 0; q < 4; ++q) flz[q] *= w;
                     }
                 }
-                if (c < kb) state_store<HLL>(zhi, tid, hi);
-            }
-            // ---------------------------------------------------------------- FIN (cell c-1)
-            if (c > ka) {
-                const double coef = kz * g.cg[2][2][c - 1];
-                double E = fma(-coef, flz[0] - Fz[0], acc[0]);
-                double F[3];
+                state_store<HLL, FNI>(zhi, ti, hi);
+                if (c > ka) {
+                    // cell c-1 is complete: U* goes to the halo warps, which run the implicit half one step from now
+                    const double coef = kz * g.cg[2][2][c - 1];
+                    const double cyp = ky * g.cg[1][2][c - 1];
+                    double* fb = fin + (c & 1) * (4 * FNI);
 #pragma unroll
-                for (int q = 0; q < 3; ++q) F[q] = fma(-coef, flz[1 + q] - Fz[1 + q], acc[1 + q]);
-                if (writer) {
-                    const long long id = id0 + (long long)(c - 1) * g.stride[2];
-                    const double rho = a.im.rho[id];
-                    const double T0 = a.im.T[id];
-                    double m[3] = {0.0, 0.0, 0.0};
-                    if (FEEDBACK) {
-#pragma unroll
-                        for (int q = 0; q < 3; ++q) m[q] = a.im.mom[q][id];
-                    }
-                    bool floored = false, clipped = false;
-                    const double r = implicit_cell<FEEDBACK, true>(g, par, oP, oR, oS, a.im, dt, id, i, j, c - 1, E, F, rho, T0, m,
-                                                                   floored, clipped);
-                    rate = dmax(rate, r);
-                    nfloor += floored ? 1 : 0;
-                    nclip += clipped ? 1 : 0;
+                    for (int q = 0; q < 4; ++q)
+                        fb[q * FNI + ti] = fma(-coef, flz[q] - Fz[q], fma(-cyp, yfl[q * FNP + tid], acc[q]));
                 }
-            }
-            if (c >= ka) {
 #pragma unroll
                 for (int q = 0; q < 4; ++q) Fz[q] = flz[q];
             }
-        }
-
-        if (c >= ka && c < kb) {  // block-uniform
-            // ---------------------------------------------------------------- Y
-            double fly[4], qy[4];
-            {
-                double dm[4], dp[4];
+            if (c >= ka && c < kb) {
+                double qc[4];
 #pragma unroll
-                for (int q = 0; q < 4; ++q) {
-                    qy[q] = pc[q * FPHW + o];
-                    dm[q] = qy[q] - pc[q * FPHW + o - FPW];
-                    dp[q] = pc[q * FPHW + o + FPW] - qy[q];
+                for (int q = 0; q < 4; ++q) qc[q] = pc[q * FPS + o];
+                // -------------------------------------------------------- Y: face states; the upper one to the row above
+                State ylo;
+                {
+                    double dm[4], dp[4];
+#pragma unroll
+                    for (int q = 0; q < 4; ++q) {
+                        dm[q] = qc[q] - pc[q * FPS + o - FPW];
+                        dp[q] = pc[q * FPS + o + FPW] - qc[q];
+                    }
+                    State hi;
+                    cell_faces<1, HLL>(qc, dm, dp, true, true, ylo, hi);
+                    state_store<HLL, FNP>(yhi, tid, hi);
+                    pair_arrive(1 + ly);
                 }
-                State lo, hi;
-                cell_faces<1, HLL>(qy, dm, dp, ly >= 1, ly <= FTY, lo, hi);
-                if (ly <= FTY) state_store<HLL>(yhi, tid, hi);
-                __syncthreads();
-                if (ly >= 1) {
+                // -------------------------------------------------------- X
+                {
+                    double dm[4], dp[4];
+#pragma unroll
+                    for (int q = 0; q < 4; ++q) {
+                        dm[q] = qc[q] - pc[q * FPS + o - 1];
+                        dp[q] = pc[q * FPS + o + 1] - qc[q];
+                    }
+                    State lo, hi;
+                    cell_faces<0, HLL>(qc, dm, dp, true, true, lo, hi);
                     State L;
-                    state_load<HLL>(yhi, tid - 32, L);
-                    const double limd = THICK ? dmax(pc[4 * FPHW + o - FPW], pc[4 * FPHW + o]) : kInf;
-                    riemann<HLL>(L, lo, limd, fly);
+#pragma unroll
+                    for (int q = 0; q < 4; ++q) {
+                        L.U[q] = __shfl_up_sync(0xffffffffu, hi.U[q], 1);
+                        L.G[q] = __shfl_up_sync(0xffffffffu, hi.G[q], 1);
+                    }
+                    if (HLL) {
+                        L.lm = __shfl_up_sync(0xffffffffu, hi.lm, 1);
+                        L.lp = __shfl_up_sync(0xffffffffu, hi.lp, 1);
+                    }
+                    double fl[4];
+                    const double limd = THICK ? dmax(pc[4 * FPS + o - 1], pc[4 * FPS + o]) : kInf;
+                    riemann<HLL>(L, lo, limd, fl);
+                    if (CURVI) {
+#pragma unroll
+                        for (int q = 0; q < 4; ++q) fl[q] *= wx;
+                    }
+                    const double cx = kx * g.cg[0][2][c];
+#pragma unroll
+                    for (int q = 0; q < 4; ++q) {
+                        const double fu = __shfl_down_sync(0xffffffffu, fl[q], 1);
+                        acc[q] = fma(-cx, fu - fl[q], qc[q]);
+                    }
+                    if (CURVI) {
+                        const double E2 = qc[0] * qc[0];
+                        const double F2 = fma(qc[3], qc[3], fma(qc[2], qc[2], qc[1] * qc[1]));
+                        const Closure cl = closure_of(qc[0], E2, F2);
+                        const double s = dtc * g.invr[ic];
+                        if (g.geometry == 1) {
+                            acc[1] = fma(s, fma(cl.gE * qc[2], qc[2], cl.dE), acc[1]);
+                            acc[2] = fma(-s, cl.gE * qc[1] * qc[2], acc[2]);
+                        } else {
+                            const double ct = g.cot[jc];
+                            const double Ptt = fma(cl.gE * qc[2], qc[2], cl.dE);
+                            const double Ppp = fma(cl.gE * qc[3], qc[3], cl.dE);
+                            const double Prt = cl.gE * qc[1] * qc[2];
+                            const double Prp = cl.gE * qc[1] * qc[3];
+                            const double Ptp = cl.gE * qc[2] * qc[3];
+                            acc[1] = fma(s, Ptt + Ppp, acc[1]);
+                            acc[2] = fma(s, fma(ct, Ppp, -Prt), acc[2]);
+                            acc[3] = fma(-s, fma(ct, Ptp, Prp), acc[3]);
+                        }
+                    }
+                }
+                // -------------------------------------------------------- Y: flux through the lower x2 face
+                {
+                    pair_sync(ly);  // the row below has stored its upper-face state
+                    State L;
+                    state_load<HLL, FNP>(yhi, tid - 32, L);
+                    const double limd = THICK ? dmax(pc[4 * FPS + o - FPW], pc[4 * FPS + o]) : kInf;
+                    double fly[4];
+                    riemann<HLL>(L, ylo, limd, fly);
+                    const double cy = ky * g.cg[1][2][c];
 #pragma unroll
                     for (int q = 0; q < 4; ++q) {
                         if (CURVI) fly[q] *= wy;
-                        yfl[q * FNT + tid] = fly[q];
+                        // read by the row below at the start of the next step.  Single buffer: that row read the previous
+                        // value BEFORE its pair_arrive of this step, and this store comes AFTER the pair_sync on it.
+                        yfl[q * FNP + tid - 32] = fly[q];
+                        acc[q] = fma(cy, fly[q], acc[q]);
                     }
                 }
-                __syncthreads();
             }
-            if (row_in) {
-                const double cy = ky * g.cg[1][2][c];
+        }
+        return;
+    }
+
+    // ==================================================================== halo rows
+    // Row 0 supplies the upper x2 face state below the tile, row FTY+1 the flux through the face above it; both
+    // also run the implicit half (a8-a11) of the interior rows, FTY/2 rows each, one step behind the transport.
+    const int h = (ly == 0) ? 0 : 1;
+    int nfloor = 0, nclip = 0;  // cells of this thread whose floor / clip fired
+    double rate = 0.0;
+    const bool xin = lx >= 1 && lx <= FTX && i < g.n[0];
+    // implicit half of plane kk from fin[buf]
+    auto finish_plane = [&](int kk, int buf) {
+        const double* fb = fin + buf * (4 * FNI);
+        constexpr int NR = FTY / 2;
+        // all loads of the NR cells first: the stores of one cell may alias the loads of the next as far as the
+        // compiler knows, and the halo warps must not serialise NR DRAM round trips per plane
+        long long id[NR];
+        bool ok[NR];
+        double rho[NR], T0[NR], m[NR][3], E[NR], F[NR][3];
 #pragma unroll
-                for (int q = 0; q < 4; ++q) acc[q] = fma(-cy, yfl[q * FNT + tid + 32] - fly[q], qy[q]);
-                // ------------------------------------------------------------ X
-                double dm[4], dp[4];
+        for (int k3 = 0; k3 < NR; ++k3) {
+            const int r = h * NR + k3;
+            const int jj = j0 + r;
+            ok[k3] = xin && jj < g.n[1];
+            id[k3] = (ic + g.gh[0]) + (long long)(min(jj, g.n[1] - 1) + g.gh[1]) * g.stride[1] + (long long)(kk + g.gh[2]) * g.stride[2];
+            const int slot = r * 32 + lx;
+            rho[k3] = __ldg(a.im.rho + id[k3]);
+            T0[k3] = a.im.T[id[k3]];
 #pragma unroll
-                for (int q = 0; q < 4; ++q) {
-                    dm[q] = qy[q] - pc[q * FPHW + o - 1];
-                    dp[q] = pc[q * FPHW + o + 1] - qy[q];
-                }
-                State lo, hi;
-                cell_faces<0, HLL>(qy, dm, dp, true, true, lo, hi);
-                State L;
+            for (int q = 0; q < 3; ++q) m[k3][q] = FEEDBACK ? a.im.mom[q][id[k3]] : 0.0;
+            E[k3] = fb[slot];
 #pragma unroll
-                for (int q = 0; q < 4; ++q) {
-                    L.U[q] = __shfl_up_sync(0xffffffffu, hi.U[q], 1);
-                    L.G[q] = __shfl_up_sync(0xffffffffu, hi.G[q], 1);
-                }
-                if (HLL) {
-                    L.lm = __shfl_up_sync(0xffffffffu, hi.lm, 1);
-                    L.lp = __shfl_up_sync(0xffffffffu, hi.lp, 1);
-                }
-                double fl[4];
-                const double limd = THICK ? dmax(pc[4 * FPHW + o - 1], pc[4 * FPHW + o]) : kInf;
-                riemann<HLL>(L, lo, limd, fl);
-                if (CURVI) {
+            for (int q = 0; q < 3; ++q) F[k3][q] = fb[(1 + q) * FNI + slot];
+        }
 #pragma unroll
-                    for (int q = 0; q < 4; ++q) fl[q] *= wx;
-                }
-                const double cx = kx * g.cg[0][2][c];
+        for (int k3 = 0; k3 < NR; ++k3) {
+            if (ok[k3]) {
+                bool floored = false, clipped = false;
+                const double rr = implicit_cell<FEEDBACK, true>(g, par, oP, oR, oS, a.im, dt, id[k3], i, j0 + h * NR + k3, kk, E[k3],
+                                                                F[k3], rho[k3], T0[k3], m[k3], floored, clipped);
+                rate = dmax(rate, rr);
+                nfloor += floored ? 1 : 0;
+                nclip += clipped ? 1 : 0;
+            }
+        }
+    };
+    auto prefetch_plane = [&](int kk) {
 #pragma unroll
-                for (int q = 0; q < 4; ++q) {
-                    const double fu = __shfl_down_sync(0xffffffffu, fl[q], 1);
-                    acc[q] = fma(-cx, fu - fl[q], acc[q]);
+        for (int k3 = 0; k3 < FTY / 2; ++k3) {
+            const int jj = j0 + h * (FTY / 2) + k3;
+            if (xin && jj < g.n[1]) {
+                const long long id = (i + g.gh[0]) + (long long)(jj + g.gh[1]) * g.stride[1] + (long long)(kk + g.gh[2]) * g.stride[2];
+                prefetch_l2(a.im.rho + id);
+                prefetch_l2(a.im.T + id);
+                if (FEEDBACK) {
+#pragma unroll
+                    for (int q = 0; q < 3; ++q) prefetch_l2(a.im.mom[q] + id);
                 }
-                if (CURVI) {
-                    const double E2 = qy[0] * qy[0];
-                    const double F2 = fma(qy[3], qy[3], fma(qy[2], qy[2], qy[1] * qy[1]));
-                    const Closure cl = closure_of(qy[0], E2, F2);
-                    const double s = dtc * g.invr[ic];
-                    if (g.geometry == 1) {
-                        acc[1] = fma(s, fma(cl.gE * qy[2], qy[2], cl.dE), acc[1]);
-                        acc[2] = fma(-s, cl.gE * qy[1] * qy[2], acc[2]);
-                    } else {
-                        const double ct = g.cot[jc];
-                        const double Ptt = fma(cl.gE * qy[2], qy[2], cl.dE);
-                        const double Ppp = fma(cl.gE * qy[3], qy[3], cl.dE);
-                        const double Prt = cl.gE * qy[1] * qy[2];
-                        const double Prp = cl.gE * qy[1] * qy[3];
-                        const double Ptp = cl.gE * qy[2] * qy[3];
-                        acc[1] = fma(s, Ptt + Ppp, acc[1]);
-                        acc[2] = fma(s, fma(ct, Ppp, -Prt), acc[2]);
-                        acc[3] = fma(-s, fma(ct, Ptp, Prp), acc[3]);
-                    }
-                }
+            }
+        }
+    };
+    const double ky = dtc * g.cg[1][0][ic] * g.cg[1][1][jc];
+    (void)ky;
+    double wy = 1.0;
+    if (CURVI) wy = g.wf[1][min(max(j, 0), g.n[1])];
+
+#pragma unroll 1
+    for (int c = ka - 1; c <= kb + 1; ++c) {
+        step_begin(c);
+        const double* pc = planes + ((c + 4) & 3) * (FNARR * FPS);
+        const bool active = (c >= ka && c < kb);
+        double qc[4], dm[4], dp[4];
+        if (active) {
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                qc[q] = pc[q * FPS + o];
+                dm[q] = qc[q] - pc[q * FPS + o - FPW];
+                dp[q] = pc[q * FPS + o + FPW] - qc[q];
+            }
+        }
+        if (h == 0 && active) {  // the state the row above waits for comes first
+            State lo, hi;
+            cell_faces<1, HLL>(qc, dm, dp, false, true, lo, hi);
+            state_store<HLL, FNP>(yhi, tid, hi);
+            pair_arrive(1);
+        }
+        if (c - 1 >= ka && c - 1 < kb) prefetch_plane(c - 1);      // inputs of the implicit half of the next step
+        if (c - 2 >= ka) finish_plane(c - 2, (c - 1) & 1);          // U* written by the interior rows one step ago
+        if (h == 1 && active) {
+            State lo, hi;
+            cell_faces<1, HLL>(qc, dm, dp, true, false, lo, hi);
+            pair_sync(FTY + 1);
+            State L;
+            state_load<HLL, FNP>(yhi, tid - 32, L);
+            const double limd = THICK ? dmax(pc[4 * FPS + o - FPW], pc[4 * FPS + o]) : kInf;
+            double fly[4];
+            riemann<HLL>(L, lo, limd, fly);
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                if (CURVI) fly[q] *= wy;
+                yfl[q * FNP + tid - 32] = fly[q];
             }
         }
     }
