@@ -326,6 +326,7 @@ extern "C" int32_t rt_set_opacity(rt_grid* g, int32_t which, const rt_opacity* o
         d.kmax = o->kmax;
         d.n2a = half_int_exponent(o->a);
         d.n2b = half_int_exponent(o->b);
+        d.fast = (d.n2a != INT_MIN && d.n2b != INT_MIN && abs(d.n2a) <= 15 && abs(d.n2b) <= 15) ? 1 : 0;
     } else if (o->kind == 1) {
         if (!o->log10_kappa || o->n_lT < 2 || o->n_lrho < 1)
             return fail(g, RT_ERR_INVALID_ARG, "rt_set_opacity: table needs n_lT >= 2, n_lrho >= 2 (or == 1) and data");
@@ -693,7 +694,7 @@ static int fused_segment_length(const rt_grid* g, int tiles) {
 
 static bool fused_eligible(const rt_grid* g) {
     const GridDev& D = g->dev;
-    return g->fused_seg >= 0 && D.gh[0] > 0 && D.gh[1] > 0 && D.gh[2] > 0;
+    return g->fused_seg >= 0 && D.gh[0] > 0 && D.gh[1] > 0 && D.gh[2] > 0 && D.ntot < (1LL << 31);  // 32-bit element offsets inside the kernel
 }
 
 static int32_t fused_impl(rt_grid* g, double* dt_device, double cfl, const double* rho, double* T, double* const mom[3],

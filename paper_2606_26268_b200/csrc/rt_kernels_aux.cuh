@@ -177,7 +177,33 @@ struct LogRT {
     double lrho, lT;
 };
 
+// x^(m2/2) for 0 <= m2 <= 15, m2 warp-uniform: three squarings, selects, one optional square root; no loop
+__device__ __forceinline__ double pow_half_small(double x, int m2) {
+    const int p = m2 >> 1;
+    const double x2 = x * x, x4 = x2 * x2;
+    double r = (p & 1) ? x : 1.0;
+    r = (p & 2) ? r * x2 : r;
+    r = (p & 4) ? r * x4 : r;
+    if (m2 & 1) r *= fsqrt(x);
+    return r;
+}
+
+// kappa0 (rho/rho0)^a (T/T0)^b with half-integer a, b (|2a|, |2b| <= 15): positive powers multiply, negative powers
+// share ONE reciprocal.  ~1-2 ulp against libm pow().
+__device__ __forceinline__ double power_law_fast(const OpacDev& o, double rho, double T) {
+    const double xr = rho * o.irho0, xt = T * o.iT0;
+    const int na = o.n2a, nb = o.n2b;
+    const double pr = pow_half_small(xr, na < 0 ? -na : na);
+    const double pt = pow_half_small(xt, nb < 0 ? -nb : nb);
+    double num = o.kappa0, den = 1.0;
+    if (na < 0) den = pr; else num *= pr;
+    if (nb < 0) den *= pt; else num *= pt;
+    if ((na | nb) < 0) num *= frcp(den);
+    return dmin(dmax(num, o.kmin), o.kmax);
+}
+
 __device__ __forceinline__ double power_law_eval(const OpacDev& o, double rho, double T) {
+    if (o.fast) return power_law_fast(o, rho, T);
     const double xr = rho * o.irho0, xt = T * o.iT0;
     double pr, pt;
     if (o.n2a != INT_MIN) pr = pow_half_int(xr, o.n2a); else pr = pow(xr, o.a);
@@ -285,8 +311,8 @@ struct CflScratch {
     unsigned int pad;
 };
 
-__device__ __forceinline__ double cell_rate(const GridDev& g, double chat, double E, double F1, double F2, double F3, int i,
-                                            int j, int k) {
+// il[d] = 1/dl_d of the cell (0 for an inactive direction: it then adds nothing)
+__device__ __forceinline__ double cell_rate_il(double chat, double E, double F1, double F2, double F3, const double il[3]) {
     const double E2 = E * E;
     const double Fq = fma(F3, F3, fma(F2, F2, F1 * F1));
     const Closure c = closure_of(E, E2, Fq);
@@ -294,14 +320,24 @@ __device__ __forceinline__ double cell_rate(const GridDev& g, double chat, doubl
     double sum = 0.0;
 #pragma unroll
     for (int d = 0; d < 3; ++d) {
-        if (g.gh[d] == 0) continue;
         const double b = c.gE * F[d];
         const double z2 = (2.0 * c.dE) * fma(-b, F[d], c.sE);
         const double z = fsqrt(dmax(z2, kTiny));
-        const double il = g.ilen[d][0][i] * g.ilen[d][1][j] * g.ilen[d][2][k];
-        sum = fma((fabs(F[d]) + z) * c.rsE, il, sum);
+        sum = fma((fabs(F[d]) + z) * c.rsE, il[d], sum);
     }
     return sum * chat;
+}
+
+__device__ __forceinline__ void cell_inv_lengths(const GridDev& g, int i, int j, int k, double il[3]) {
+#pragma unroll
+    for (int d = 0; d < 3; ++d) il[d] = g.gh[d] == 0 ? 0.0 : g.ilen[d][0][i] * g.ilen[d][1][j] * g.ilen[d][2][k];
+}
+
+__device__ __forceinline__ double cell_rate(const GridDev& g, double chat, double E, double F1, double F2, double F3, int i,
+                                            int j, int k) {
+    double il[3];
+    cell_inv_lengths(g, i, j, k, il);
+    return cell_rate_il(chat, E, F1, F2, F3, il);
 }
 
 __device__ __forceinline__ void block_max_to_global(double v, CflScratch* scr, double cfl, double* dt_out, unsigned nblocks) {

@@ -30,8 +30,9 @@
 namespace rtm1 {
 
 constexpr int FTX = 30;           // output cells per CTA along x1 (32 lanes, 1 halo lane each side)
-constexpr int FTY = 6;            // output cells per CTA along x2
-constexpr int FNY = FTY + 2;      // thread rows
+constexpr int FTY = 8;            // output cells per CTA along x2 = thread rows (no halo rows: rows 0 and FTY-1
+                                  // build the face states of the cells below / above the tile themselves)
+constexpr int FNY = FTY;          // thread rows
 constexpr int FNT = 32 * FNY;     // threads per CTA
 constexpr int FPW = 34;           // staged plane width  (cells i0-2 .. i0+31)
 constexpr int FPH = FTY + 4;      // staged plane height (cells j0-2 .. j0+FTY+1)
@@ -40,14 +41,10 @@ constexpr int FPS = (FPHW + 15) / 16 * 16;  // doubles between staged arrays: ev
 constexpr int FNARR = 5;          // E, F1, F2, F3, lim
 constexpr int FNSLOT = 4;
 constexpr int FNST = 10;          // doubles of an exchanged face state: U[4], G[4], lm, lp
-constexpr int FNI = 32 * FTY;        // threads of the interior rows 1..FTY       (slot t - 32)
-constexpr int FNP = 32 * (FTY + 1);  // threads of rows 0..FTY (state producers) or 1..FTY+1 (flux producers)
-// staged planes | zhi[FNST][FNI] | yhi[FNST][FNP] | yfl[4][FNP] | fin[2][4][FNI] | mbarriers
+// staged planes | zhi[FNST][FNT] | yex[FNST][FNT] | mbarriers
 constexpr size_t kFusedSmemBytes =
-    sizeof(double) * (size_t)(FNSLOT * FNARR * FPS + FNST * FNI + FNST * FNP + 4 * FNP + 2 * 4 * FNI) +
-    FNSLOT * sizeof(unsigned long long);
-static_assert(FTY + 1 <= 15, "one named barrier per row pair");
-static_assert(FTY % 2 == 0, "the two halo warps share the implicit half of the FTY rows");
+    sizeof(double) * (size_t)(FNSLOT * FNARR * FPS + 2 * FNST * FNT) + FNSLOT * sizeof(unsigned long long);
+static_assert(FTY <= 15, "one named barrier per row pair");
 
 struct FusedArgs {
     const double* src[FNARR];  // U_in[4], lim (or nullptr)
@@ -129,6 +126,7 @@ __device__ __forceinline__ void state_load(const double* buf, int t, State& s) {
 }
 
 
+
 template <bool HLL, bool THICK, bool CURVI, bool FEEDBACK>
 __global__ void __launch_bounds__(FNT, 2)
     k_substep_fused(const __grid_constant__ GridDev g, const __grid_constant__ ParamsDev par, const __grid_constant__ OpacDev oP,
@@ -136,21 +134,21 @@ __global__ void __launch_bounds__(FNT, 2)
                     const __grid_constant__ FusedMaps maps, int seglen) {
     extern __shared__ __align__(128) double sm[];
     double* const planes = sm;
-    double* const zhi = planes + FNSLOT * FNARR * FPS;  // [FNST][FNI]  own slot: upper x3 face state of the previous plane
-    double* const yhi = zhi + FNST * FNI;               // [FNST][FNP]  upper x2 face states of rows 0..FTY
-    double* const yfl = yhi + FNST * FNP;               // [4][FNP]     fluxes through the lower x2 faces of rows 1..FTY+1
-    double* const fin = yfl + 4 * FNP;                  // [2][4][FNI]  U* of the interior rows, for the implicit half
-    unsigned long long* const mbar = (unsigned long long*)(fin + 2 * 4 * FNI);  // [FNSLOT]
+    double* const zhi = planes + FNSLOT * FNARR * FPS;  // [FNST][FNT] own slot: upper x3 face state of the previous plane
+    double* const yex = zhi + FNST * FNT;               // [FNST][FNT] x2 exchange, one slot per thread: its upper x2 face
+                                                        // state on the way up, then (components 0-3) the flux through
+                                                        // that face on the way back down
+    unsigned long long* const mbar = (unsigned long long*)(yex + FNST * FNT);  // [FNSLOT]
 
     const int lx = threadIdx.x, ly = threadIdx.y;
     const int tid = ly * 32 + lx;
     const int i0 = blockIdx.x * FTX, j0 = blockIdx.y * FTY;
     const int ka = blockIdx.z * seglen;
     const int kb = min(ka + seglen, g.n[2]);
-    const int i = i0 - 1 + lx, j = j0 - 1 + ly;
-    const bool row_in = (ly >= 1) && (ly <= FTY);
-    const int ic = min(max(i, 0), g.n[0] - 1), jc = min(max(j, 0), g.n[1] - 1);
-    const int o = (ly + 1) * FPW + lx + 1;  // this thread's cell inside a staged plane
+    const int i = i0 - 1 + lx, j = j0 + ly;
+    const bool writer = lx >= 1 && lx <= FTX && i < g.n[0] && j < g.n[1];
+    const int ic = min(max(i, 0), g.n[0] - 1), jc = min(j, g.n[1] - 1);
+    const int o = (ly + 2) * FPW + lx + 1;  // this thread's cell inside a staged plane
     const bool tma = a.use_tma != 0;
     const double dt = a.im.dt_dev ? __ldg(a.im.dt_dev) : a.im.dt;
     const double dtc = dt * a.chat;
@@ -190,270 +188,223 @@ __global__ void __launch_bounds__(FNT, 2)
     auto wait_plane = [&](int p) {
         if (tma) mbar_wait(mbar + ((p + 4) & 3), (unsigned)(((p - ka + 2) >> 2) & 1));
     };
-    // top of step c: plane c+1 has landed and is visible to all; every warp is done with step c-1
-    auto step_begin = [&](int c) {
-        if (c + 1 <= kb + 1) {
-            if (tma) wait_plane(c + 1); else cp_async_wait_all();
-        }
-        __syncthreads();
-        if (c + 2 <= kb + 1) load_plane(c + 2);
-    };
     load_plane(ka - 2);
     load_plane(ka - 1);
     load_plane(ka);
     wait_plane(ka - 2);
     wait_plane(ka - 1);
 
-    if (row_in) {
-        // ================================================================ interior rows: transport
-        const int ti = tid - 32;  // slot among the interior rows
-        const double kx = dtc * g.cg[0][0][ic] * g.cg[0][1][jc];
-        const double ky = dtc * g.cg[1][0][ic] * g.cg[1][1][jc];
-        const double kz = dtc * g.cg[2][0][ic] * g.cg[2][1][jc];
-        double wx = 1.0, wy = 1.0;
-        if (CURVI) {
-            wx = g.wf[0][min(max(i, 0), g.n[0])];
-            wy = g.wf[1][min(max(j, 0), g.n[1])];
-        }
-        double acc[4] = {0.0, 0.0, 0.0, 0.0};  // U^n - dt/V ([AF]_x + [AF]_y) + dt S_geo of the previous plane's cell,
-                                               // still missing the flux through its upper x2 face (held by the row above)
-        double Fz[4] = {0.0, 0.0, 0.0, 0.0};   // area-weighted flux through the lower x3 face of that cell
-#pragma unroll 1
-        for (int c = ka - 1; c <= kb + 1; ++c) {  // step kb+1: the halo warps finish cell kb-1
-            step_begin(c);
-            if (c > kb) break;
-            const double* pc = planes + ((c + 4) & 3) * (FNARR * FPS);
-            // ------------------------------------------------------------ Z
-            {
-                const double* pm = planes + ((c + 3) & 3) * (FNARR * FPS);
-                const double* pp = planes + ((c + 5) & 3) * (FNARR * FPS);
-                double q0[4], dm[4], dp[4];
-#pragma unroll
-                for (int q = 0; q < 4; ++q) {
-                    q0[q] = pc[q * FPS + o];
-                    dm[q] = q0[q] - pm[q * FPS + o];
-                    dp[q] = pp[q * FPS + o] - q0[q];
-                }
-                State lo, hi;
-                cell_faces<2, HLL>(q0, dm, dp, true, true, lo, hi);  // both always: one basic block, two independent chains
-                double flz[4] = {0.0, 0.0, 0.0, 0.0};
-                if (c >= ka) {
-                    State L;
-                    state_load<HLL, FNI>(zhi, ti, L);
-                    const double limd = THICK ? dmax(pm[4 * FPS + o], pc[4 * FPS + o]) : kInf;
-                    riemann<HLL>(L, lo, limd, flz);
-                    if (CURVI) {
-                        const double w = g.wf[2][c];
-#pragma unroll
-                        for (int q = 0; q < 4; ++q) flz[q] *= w;
-                    }
-                }
-                state_store<HLL, FNI>(zhi, ti, hi);
-                if (c > ka) {
-                    // cell c-1 is complete: U* goes to the halo warps, which run the implicit half one step from now
-                    const double coef = kz * g.cg[2][2][c - 1];
-                    const double cyp = ky * g.cg[1][2][c - 1];
-                    double* fb = fin + (c & 1) * (4 * FNI);
-#pragma unroll
-                    for (int q = 0; q < 4; ++q)
-                        fb[q * FNI + ti] = fma(-coef, flz[q] - Fz[q], fma(-cyp, yfl[q * FNP + tid], acc[q]));
-                }
-#pragma unroll
-                for (int q = 0; q < 4; ++q) Fz[q] = flz[q];
-            }
-            if (c >= ka && c < kb) {
-                double qc[4];
-#pragma unroll
-                for (int q = 0; q < 4; ++q) qc[q] = pc[q * FPS + o];
-                // -------------------------------------------------------- Y: face states; the upper one to the row above
-                State ylo;
-                {
-                    double dm[4], dp[4];
-#pragma unroll
-                    for (int q = 0; q < 4; ++q) {
-                        dm[q] = qc[q] - pc[q * FPS + o - FPW];
-                        dp[q] = pc[q * FPS + o + FPW] - qc[q];
-                    }
-                    State hi;
-                    cell_faces<1, HLL>(qc, dm, dp, true, true, ylo, hi);
-                    state_store<HLL, FNP>(yhi, tid, hi);
-                    pair_arrive(1 + ly);
-                }
-                // -------------------------------------------------------- X
-                {
-                    double dm[4], dp[4];
-#pragma unroll
-                    for (int q = 0; q < 4; ++q) {
-                        dm[q] = qc[q] - pc[q * FPS + o - 1];
-                        dp[q] = pc[q * FPS + o + 1] - qc[q];
-                    }
-                    State lo, hi;
-                    cell_faces<0, HLL>(qc, dm, dp, true, true, lo, hi);
-                    State L;
-#pragma unroll
-                    for (int q = 0; q < 4; ++q) {
-                        L.U[q] = __shfl_up_sync(0xffffffffu, hi.U[q], 1);
-                        L.G[q] = __shfl_up_sync(0xffffffffu, hi.G[q], 1);
-                    }
-                    if (HLL) {
-                        L.lm = __shfl_up_sync(0xffffffffu, hi.lm, 1);
-                        L.lp = __shfl_up_sync(0xffffffffu, hi.lp, 1);
-                    }
-                    double fl[4];
-                    const double limd = THICK ? dmax(pc[4 * FPS + o - 1], pc[4 * FPS + o]) : kInf;
-                    riemann<HLL>(L, lo, limd, fl);
-                    if (CURVI) {
-#pragma unroll
-                        for (int q = 0; q < 4; ++q) fl[q] *= wx;
-                    }
-                    const double cx = kx * g.cg[0][2][c];
-#pragma unroll
-                    for (int q = 0; q < 4; ++q) {
-                        const double fu = __shfl_down_sync(0xffffffffu, fl[q], 1);
-                        acc[q] = fma(-cx, fu - fl[q], qc[q]);
-                    }
-                    if (CURVI) {
-                        const double E2 = qc[0] * qc[0];
-                        const double F2 = fma(qc[3], qc[3], fma(qc[2], qc[2], qc[1] * qc[1]));
-                        const Closure cl = closure_of(qc[0], E2, F2);
-                        const double s = dtc * g.invr[ic];
-                        if (g.geometry == 1) {
-                            acc[1] = fma(s, fma(cl.gE * qc[2], qc[2], cl.dE), acc[1]);
-                            acc[2] = fma(-s, cl.gE * qc[1] * qc[2], acc[2]);
-                        } else {
-                            const double ct = g.cot[jc];
-                            const double Ptt = fma(cl.gE * qc[2], qc[2], cl.dE);
-                            const double Ppp = fma(cl.gE * qc[3], qc[3], cl.dE);
-                            const double Prt = cl.gE * qc[1] * qc[2];
-                            const double Prp = cl.gE * qc[1] * qc[3];
-                            const double Ptp = cl.gE * qc[2] * qc[3];
-                            acc[1] = fma(s, Ptt + Ppp, acc[1]);
-                            acc[2] = fma(s, fma(ct, Ppp, -Prt), acc[2]);
-                            acc[3] = fma(-s, fma(ct, Ptp, Prp), acc[3]);
-                        }
-                    }
-                }
-                // -------------------------------------------------------- Y: flux through the lower x2 face
-                {
-                    pair_sync(ly);  // the row below has stored its upper-face state
-                    State L;
-                    state_load<HLL, FNP>(yhi, tid - 32, L);
-                    const double limd = THICK ? dmax(pc[4 * FPS + o - FPW], pc[4 * FPS + o]) : kInf;
-                    double fly[4];
-                    riemann<HLL>(L, ylo, limd, fly);
-                    const double cy = ky * g.cg[1][2][c];
-#pragma unroll
-                    for (int q = 0; q < 4; ++q) {
-                        if (CURVI) fly[q] *= wy;
-                        // read by the row below at the start of the next step.  Single buffer: that row read the previous
-                        // value BEFORE its pair_arrive of this step, and this store comes AFTER the pair_sync on it.
-                        yfl[q * FNP + tid - 32] = fly[q];
-                        acc[q] = fma(cy, fly[q], acc[q]);
-                    }
-                }
-            }
-        }
-        return;
-    }
-
-    // ==================================================================== halo rows
-    // Row 0 supplies the upper x2 face state below the tile, row FTY+1 the flux through the face above it; both
-    // also run the implicit half (a8-a11) of the interior rows, FTY/2 rows each, one step behind the transport.
-    const int h = (ly == 0) ? 0 : 1;
-    int nfloor = 0, nclip = 0;  // cells of this thread whose floor / clip fired
-    double rate = 0.0;
-    const bool xin = lx >= 1 && lx <= FTX && i < g.n[0];
-    // implicit half of plane kk from fin[buf]
-    auto finish_plane = [&](int kk, int buf) {
-        const double* fb = fin + buf * (4 * FNI);
-        constexpr int NR = FTY / 2;
-        // all loads of the NR cells first: the stores of one cell may alias the loads of the next as far as the
-        // compiler knows, and the halo warps must not serialise NR DRAM round trips per plane
-        long long id[NR];
-        bool ok[NR];
-        double rho[NR], T0[NR], m[NR][3], E[NR], F[NR][3];
-#pragma unroll
-        for (int k3 = 0; k3 < NR; ++k3) {
-            const int r = h * NR + k3;
-            const int jj = j0 + r;
-            ok[k3] = xin && jj < g.n[1];
-            id[k3] = (ic + g.gh[0]) + (long long)(min(jj, g.n[1] - 1) + g.gh[1]) * g.stride[1] + (long long)(kk + g.gh[2]) * g.stride[2];
-            const int slot = r * 32 + lx;
-            rho[k3] = __ldg(a.im.rho + id[k3]);
-            T0[k3] = a.im.T[id[k3]];
-#pragma unroll
-            for (int q = 0; q < 3; ++q) m[k3][q] = FEEDBACK ? a.im.mom[q][id[k3]] : 0.0;
-            E[k3] = fb[slot];
-#pragma unroll
-            for (int q = 0; q < 3; ++q) F[k3][q] = fb[(1 + q) * FNI + slot];
-        }
-#pragma unroll
-        for (int k3 = 0; k3 < NR; ++k3) {
-            if (ok[k3]) {
-                bool floored = false, clipped = false;
-                const double rr = implicit_cell<FEEDBACK, true>(g, par, oP, oR, oS, a.im, dt, id[k3], i, j0 + h * NR + k3, kk, E[k3],
-                                                                F[k3], rho[k3], T0[k3], m[k3], floored, clipped);
-                rate = dmax(rate, rr);
-                nfloor += floored ? 1 : 0;
-                nclip += clipped ? 1 : 0;
-            }
-        }
-    };
-    auto prefetch_plane = [&](int kk) {
-#pragma unroll
-        for (int k3 = 0; k3 < FTY / 2; ++k3) {
-            const int jj = j0 + h * (FTY / 2) + k3;
-            if (xin && jj < g.n[1]) {
-                const long long id = (i + g.gh[0]) + (long long)(jj + g.gh[1]) * g.stride[1] + (long long)(kk + g.gh[2]) * g.stride[2];
-                prefetch_l2(a.im.rho + id);
-                prefetch_l2(a.im.T + id);
-                if (FEEDBACK) {
-#pragma unroll
-                    for (int q = 0; q < 3; ++q) prefetch_l2(a.im.mom[q] + id);
-                }
-            }
-        }
-    };
+    const double kx = dtc * g.cg[0][0][ic] * g.cg[0][1][jc];
     const double ky = dtc * g.cg[1][0][ic] * g.cg[1][1][jc];
-    (void)ky;
-    double wy = 1.0;
-    if (CURVI) wy = g.wf[1][min(max(j, 0), g.n[1])];
+    const double kz = dtc * g.cg[2][0][ic] * g.cg[2][1][jc];
+    double wx = 1.0, wylo = 1.0, wyhi = 1.0;  // face-area weights of this cell's lower x1 face, lower / upper x2 faces
+    if (CURVI) {
+        wx = g.wf[0][min(max(i, 0), g.n[0])];
+        wylo = g.wf[1][min(j, g.n[1])];
+        wyhi = g.wf[1][min(j + 1, g.n[1])];
+    }
+    const int id0 = (ic + g.gh[0]) + (jc + g.gh[1]) * (int)g.stride[1] + g.gh[2] * (int)g.stride[2];  // cell (i, j, 0)
+    const int zstride = (int)g.stride[2];
+    double ilxy[3];  // x1-x2 part of 1/dl_d (CFL)
+#pragma unroll
+    for (int d = 0; d < 3; ++d) ilxy[d] = g.ilen[d][0][ic] * g.ilen[d][1][jc];
+
+    double acc[4] = {0.0, 0.0, 0.0, 0.0};  // U^n - dt/V ([AF]_x + [AF]_y) + dt S_geo of the previous plane's cell,
+                                           // still missing the flux through its upper x2 face (held by the row above)
+    double Fz[4] = {0.0, 0.0, 0.0, 0.0};   // area-weighted flux through the lower x3 face of that cell
+    int nfloor = 0, nclip = 0;             // cells of this thread whose floor / clip fired
+    double rate = 0.0;
 
 #pragma unroll 1
-    for (int c = ka - 1; c <= kb + 1; ++c) {
-        step_begin(c);
+    for (int c = ka - 1; c <= kb; ++c) {
+        if (tma) wait_plane(c + 1); else cp_async_wait_all();
+        __syncthreads();  // plane c+1 visible to all; every warp is done with step c-1
+        if (c + 2 <= kb + 1) load_plane(c + 2);
         const double* pc = planes + ((c + 4) & 3) * (FNARR * FPS);
-        const bool active = (c >= ka && c < kb);
-        double qc[4], dm[4], dp[4];
-        if (active) {
+        if (writer && c < kb) {  // inputs of the implicit half of cell c, needed one step from now
+            const int idn = id0 + c * zstride;
+            prefetch_l2(a.im.rho + idn);
+            prefetch_l2(a.im.T + idn);
+            if (FEEDBACK) {
+#pragma unroll
+                for (int q = 0; q < 3; ++q) prefetch_l2(a.im.mom[q] + idn);
+            }
+        }
+        // ---------------------------------------------------------------- Z
+        {
+            const double* pm = planes + ((c + 3) & 3) * (FNARR * FPS);
+            const double* pp = planes + ((c + 5) & 3) * (FNARR * FPS);
+            double q0[4], dm[4], dp[4];
 #pragma unroll
             for (int q = 0; q < 4; ++q) {
-                qc[q] = pc[q * FPS + o];
+                q0[q] = pc[q * FPS + o];
+                dm[q] = q0[q] - pm[q * FPS + o];
+                dp[q] = pp[q * FPS + o] - q0[q];
+            }
+            State lo, hi;
+            cell_faces<2, HLL>(q0, dm, dp, true, true, lo, hi);  // both always: one basic block, two independent chains
+            double flz[4] = {0.0, 0.0, 0.0, 0.0};
+            if (c >= ka) {
+                State L;
+                state_load<HLL, FNT>(zhi, tid, L);
+                const double limd = THICK ? dmax(pm[4 * FPS + o], pc[4 * FPS + o]) : kInf;
+                riemann<HLL>(L, lo, limd, flz);
+                if (CURVI) {
+                    const double w = g.wf[2][c];
+#pragma unroll
+                    for (int q = 0; q < 4; ++q) flz[q] *= w;
+                }
+            }
+            state_store<HLL, FNT>(zhi, tid, hi);
+            // ------------------------------------------------------------ FIN (cell c-1): a8-a11
+            if (c > ka) {
+                const double coef = kz * g.cg[2][2][c - 1];
+                const double cyp = ky * g.cg[1][2][c - 1];
+                double U4[4];
+#pragma unroll
+                for (int q = 0; q < 4; ++q) U4[q] = fma(-coef, flz[q] - Fz[q], fma(-cyp, yex[q * FNT + tid], acc[q]));
+                if (writer) {
+                    const int id = id0 + (c - 1) * zstride;
+                    const double rho = __ldg(a.im.rho + id);
+                    const double T0 = a.im.T[id];
+                    double m[3] = {0.0, 0.0, 0.0};
+                    if (FEEDBACK) {
+#pragma unroll
+                        for (int q = 0; q < 3; ++q) m[q] = a.im.mom[q][id];
+                    }
+                    double F[3] = {U4[1], U4[2], U4[3]};
+                    const double il[3] = {ilxy[0] * g.ilen[0][2][c - 1], ilxy[1] * g.ilen[1][2][c - 1], ilxy[2] * g.ilen[2][2][c - 1]};
+                    bool floored = false, clipped = false;
+                    const double r = implicit_cell<FEEDBACK, true>(g, par, oP, oR, oS, a.im, dt, (long long)id, il, U4[0], F, rho, T0, m,
+                                                                   floored, clipped);
+                    rate = dmax(rate, r);
+                    nfloor += floored ? 1 : 0;
+                    nclip += clipped ? 1 : 0;
+                }
+            }
+#pragma unroll
+            for (int q = 0; q < 4; ++q) Fz[q] = flz[q];
+        }
+        if (c < ka || c >= kb) continue;  // block-uniform
+
+        double qc[4];
+#pragma unroll
+        for (int q = 0; q < 4; ++q) qc[q] = pc[q * FPS + o];
+        // ---------------------------------------------------------------- Y: face states; the upper one to the row above
+        State ylo;
+        {
+            double dm[4], dp[4];
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
                 dm[q] = qc[q] - pc[q * FPS + o - FPW];
                 dp[q] = pc[q * FPS + o + FPW] - qc[q];
             }
+            State hi;
+            cell_faces<1, HLL>(qc, dm, dp, true, true, ylo, hi);
+            if (ly < FTY - 1) {
+                state_store<HLL, FNT>(yex, tid, hi);
+                pair_arrive(1 + ly);
+            } else {
+                // top row: the lower-face state of the cell above the tile, and the flux through the face between them
+                double qa[4], dma[4], dpa[4];
+#pragma unroll
+                for (int q = 0; q < 4; ++q) {
+                    qa[q] = pc[q * FPS + o + FPW];
+                    dma[q] = qa[q] - qc[q];
+                    dpa[q] = pc[q * FPS + o + 2 * FPW] - qa[q];
+                }
+                State loa, hia;
+                cell_faces<1, HLL>(qa, dma, dpa, true, false, loa, hia);
+                const double limd = THICK ? dmax(pc[4 * FPS + o], pc[4 * FPS + o + FPW]) : kInf;
+                double fup[4];
+                riemann<HLL>(hi, loa, limd, fup);
+#pragma unroll
+                for (int q = 0; q < 4; ++q) yex[q * FNT + tid] = CURVI ? fup[q] * wyhi : fup[q];
+            }
         }
-        if (h == 0 && active) {  // the state the row above waits for comes first
-            State lo, hi;
-            cell_faces<1, HLL>(qc, dm, dp, false, true, lo, hi);
-            state_store<HLL, FNP>(yhi, tid, hi);
-            pair_arrive(1);
-        }
-        if (c - 1 >= ka && c - 1 < kb) prefetch_plane(c - 1);      // inputs of the implicit half of the next step
-        if (c - 2 >= ka) finish_plane(c - 2, (c - 1) & 1);          // U* written by the interior rows one step ago
-        if (h == 1 && active) {
-            State lo, hi;
-            cell_faces<1, HLL>(qc, dm, dp, true, false, lo, hi);
-            pair_sync(FTY + 1);
-            State L;
-            state_load<HLL, FNP>(yhi, tid - 32, L);
-            const double limd = THICK ? dmax(pc[4 * FPS + o - FPW], pc[4 * FPS + o]) : kInf;
-            double fly[4];
-            riemann<HLL>(L, lo, limd, fly);
+        // ---------------------------------------------------------------- X
+        {
+            double dm[4], dp[4];
 #pragma unroll
             for (int q = 0; q < 4; ++q) {
-                if (CURVI) fly[q] *= wy;
-                yfl[q * FNP + tid - 32] = fly[q];
+                dm[q] = qc[q] - pc[q * FPS + o - 1];
+                dp[q] = pc[q * FPS + o + 1] - qc[q];
+            }
+            State lo, hi;
+            cell_faces<0, HLL>(qc, dm, dp, true, true, lo, hi);
+            State L;
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                L.U[q] = __shfl_up_sync(0xffffffffu, hi.U[q], 1);
+                L.G[q] = __shfl_up_sync(0xffffffffu, hi.G[q], 1);
+            }
+            if (HLL) {
+                L.lm = __shfl_up_sync(0xffffffffu, hi.lm, 1);
+                L.lp = __shfl_up_sync(0xffffffffu, hi.lp, 1);
+            }
+            double fl[4];
+            const double limd = THICK ? dmax(pc[4 * FPS + o - 1], pc[4 * FPS + o]) : kInf;
+            riemann<HLL>(L, lo, limd, fl);
+            if (CURVI) {
+#pragma unroll
+                for (int q = 0; q < 4; ++q) fl[q] *= wx;
+            }
+            const double cx = kx * g.cg[0][2][c];
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                const double fu = __shfl_down_sync(0xffffffffu, fl[q], 1);
+                acc[q] = fma(-cx, fu - fl[q], qc[q]);
+            }
+            if (CURVI) {
+                const double E2 = qc[0] * qc[0];
+                const double F2 = fma(qc[3], qc[3], fma(qc[2], qc[2], qc[1] * qc[1]));
+                const Closure cl = closure_of(qc[0], E2, F2);
+                const double s = dtc * g.invr[ic];
+                if (g.geometry == 1) {
+                    acc[1] = fma(s, fma(cl.gE * qc[2], qc[2], cl.dE), acc[1]);
+                    acc[2] = fma(-s, cl.gE * qc[1] * qc[2], acc[2]);
+                } else {
+                    const double ct = g.cot[jc];
+                    const double Ptt = fma(cl.gE * qc[2], qc[2], cl.dE);
+                    const double Ppp = fma(cl.gE * qc[3], qc[3], cl.dE);
+                    const double Prt = cl.gE * qc[1] * qc[2];
+                    const double Prp = cl.gE * qc[1] * qc[3];
+                    const double Ptp = cl.gE * qc[2] * qc[3];
+                    acc[1] = fma(s, Ptt + Ppp, acc[1]);
+                    acc[2] = fma(s, fma(ct, Ppp, -Prt), acc[2]);
+                    acc[3] = fma(-s, fma(ct, Ptp, Prp), acc[3]);
+                }
+            }
+        }
+        // ---------------------------------------------------------------- Y: flux through the lower x2 face
+        {
+            State L;
+            if (ly > 0) {
+                pair_sync(ly);  // the row below has stored its upper-face state
+                state_load<HLL, FNT>(yex, tid - 32, L);
+            } else {
+                // bottom row: the upper-face state of the cell below the tile
+                double qb[4], dmb[4], dpb[4];
+#pragma unroll
+                for (int q = 0; q < 4; ++q) {
+                    qb[q] = pc[q * FPS + o - FPW];
+                    dmb[q] = qb[q] - pc[q * FPS + o - 2 * FPW];
+                    dpb[q] = qc[q] - qb[q];
+                }
+                State lob;
+                cell_faces<1, HLL>(qb, dmb, dpb, false, true, lob, L);
+            }
+            const double limd = THICK ? dmax(pc[4 * FPS + o - FPW], pc[4 * FPS + o]) : kInf;
+            double fly[4];
+            riemann<HLL>(L, ylo, limd, fly);
+            const double cy = ky * g.cg[1][2][c];
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                if (CURVI) fly[q] *= wylo;
+                // back down to the row below, which reads it at the start of the next step, into the slot its state came
+                // from: that row wrote the slot BEFORE its pair_arrive, this store comes AFTER the pair_sync on it
+                if (ly > 0) yex[q * FNT + tid - 32] = fly[q];
+                acc[q] = fma(cy, fly[q], acc[q]);
             }
         }
     }

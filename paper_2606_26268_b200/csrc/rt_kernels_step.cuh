@@ -232,9 +232,9 @@ struct ImplicitArgs {
 // sub-step kernel.  E, F: the state after the explicit half; writes through the pointers of `a` at index id.
 template <bool FEEDBACK, bool CFL>
 __device__ __forceinline__ double implicit_cell(const GridDev& g, const ParamsDev& par, const OpacDev& oP, const OpacDev& oR,
-                                                const OpacDev& oS, const ImplicitArgs& a, double dt, long long id, int i, int j,
-                                                int k, double E, double F[3], double rho, double T0, const double m[3],
-                                                bool& floored, bool& clipped) {
+                                                const OpacDev& oS, const ImplicitArgs& a, double dt, long long id,
+                                                const double il[3] /* 1/dl_d of the cell (CFL only) */, double E, double F[3],
+                                                double rho, double T0, const double m[3], bool& floored, bool& clipped) {
     if (E < par.E_floor) {
         E = par.E_floor;
         floored = true;
@@ -272,7 +272,7 @@ __device__ __forceinline__ double implicit_cell(const GridDev& g, const ParamsDe
         if (FEEDBACK) a.mom[q][id] = fma(-(Fn[q] - F[q]), ichat, m[q]);
         a.U[1 + q][id] = Fn[q];
     }
-    return CFL ? cell_rate(g, par.chat, En, Fn[0], Fn[1], Fn[2], i, j, k) : 0.0;
+    return CFL ? cell_rate_il(par.chat, En, Fn[0], Fn[1], Fn[2], il) : 0.0;
 }
 
 // fold a warp's CFL rates into the running maximum (see k_implicit) and count floor / clip activations
@@ -317,7 +317,9 @@ __global__ void __launch_bounds__(128) k_implicit(const __grid_constant__ GridDe
 #pragma unroll
             for (int q = 0; q < 3; ++q) m[q] = a.mom[q][id];
         }
-        rate = implicit_cell<FEEDBACK, CFL>(g, par, oP, oR, oS, a, dt, id, i, j, k, E, F, rho, T0, m, floored, clipped);
+        double il[3] = {0.0, 0.0, 0.0};
+        if (CFL) cell_inv_lengths(g, i, j, k, il);
+        rate = implicit_cell<FEEDBACK, CFL>(g, par, oP, oR, oS, a, dt, id, il, E, F, rho, T0, m, floored, clipped);
     }
     implicit_warp_epilogue<CFL>(a, rate, floored ? 1 : 0, clipped ? 1 : 0);
 }

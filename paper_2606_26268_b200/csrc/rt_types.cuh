@@ -32,6 +32,7 @@ struct OpacDev {
     int set;   // 0: never set -> kappa = 0
     int kind;  // 0 power law, 1 table
     int n2a, n2b;  // 2a, 2b when both are integers with |.| <= 64 (half-integer fast path), else INT_MIN
+    int fast;      // both exponents are half-integers with |2a|, |2b| <= 15: straight-line evaluation (power_law_fast)
     double kappa0, irho0, iT0, a, b, kmin, kmax;
     int n_lrho, n_lT;
     double lrho_min, lrho_max, lT_min, lT_max;
