@@ -177,29 +177,40 @@ struct LogRT {
     double lrho, lT;
 };
 
-// x^(m2/2) for 0 <= m2 <= 15, m2 warp-uniform: three squarings, selects, one optional square root; no loop
+// x^(m2/2) for 0 <= m2 <= 15, m2 warp-uniform: one uniform branch into a straight-line product, one optional
+// square root; no loop, no selects
 __device__ __forceinline__ double pow_half_small(double x, int m2) {
-    const int p = m2 >> 1;
-    const double x2 = x * x, x4 = x2 * x2;
-    double r = (p & 1) ? x : 1.0;
-    r = (p & 2) ? r * x2 : r;
-    r = (p & 4) ? r * x4 : r;
+    const double x2 = x * x;
+    double r;
+    switch (m2 >> 1) {
+        case 0: r = 1.0; break;
+        case 1: r = x; break;
+        case 2: r = x2; break;
+        case 3: r = x2 * x; break;
+        case 4: r = x2 * x2; break;
+        case 5: r = x2 * x2 * x; break;
+        case 6: r = x2 * x2 * x2; break;
+        default: r = x2 * x2 * x2 * x; break;
+    }
     if (m2 & 1) r *= fsqrt(x);
     return r;
 }
 
 // kappa0 (rho/rho0)^a (T/T0)^b with half-integer a, b (|2a|, |2b| <= 15): positive powers multiply, negative powers
-// share ONE reciprocal.  ~1-2 ulp against libm pow().
-__device__ __forceinline__ double power_law_fast(const OpacDev& o, double rho, double T) {
-    const double xr = rho * o.irho0, xt = T * o.iT0;
-    const int na = o.n2a, nb = o.n2b;
-    const double pr = pow_half_small(xr, na < 0 ? -na : na);
-    const double pt = pow_half_small(xt, nb < 0 ? -nb : nb);
-    double num = o.kappa0, den = 1.0;
+// share ONE reciprocal.  ~1-2 ulp against libm pow().  The scalars are passed in so that a caller looping over
+// cells keeps them in registers.
+__device__ __forceinline__ double power_law_fast_v(double kappa0, double irho0, double iT0, int na, int nb, double kmin,
+                                                   double kmax, double rho, double T) {
+    const double pr = pow_half_small(rho * irho0, na < 0 ? -na : na);
+    const double pt = pow_half_small(T * iT0, nb < 0 ? -nb : nb);
+    double num = kappa0, den = 1.0;
     if (na < 0) den = pr; else num *= pr;
     if (nb < 0) den *= pt; else num *= pt;
     if ((na | nb) < 0) num *= frcp(den);
-    return dmin(dmax(num, o.kmin), o.kmax);
+    return dmin(dmax(num, kmin), kmax);
+}
+__device__ __forceinline__ double power_law_fast(const OpacDev& o, double rho, double T) {
+    return power_law_fast_v(o.kappa0, o.irho0, o.iT0, o.n2a, o.n2b, o.kmin, o.kmax, rho, T);
 }
 
 __device__ __forceinline__ double power_law_eval(const OpacDev& o, double rho, double T) {
@@ -269,34 +280,59 @@ __device__ __forceinline__ double opacity_eval_shared(const OpacDev& o, double r
 // Ghost cells take the value of the periodic image or of the nearest interior cell, so rho and T
 // ghosts are never read.  The sweeps use lim_face = max(limd_a, limd_b) = 4/(3 min(tau_a, tau_b)).
 // ------------------------------------------------------------------------------------------------
+constexpr int kThickRows = 4;  // x2 rows per block: ~200 k one-cell blocks cost more to schedule than to run
+// LEAN: chi is ONE half-integer power law (kappa_R fast, no scattering): its scalars live in registers
+template <bool LEAN>
 __global__ void __launch_bounds__(128) k_thick_limit(const __grid_constant__ GridDev g, const __grid_constant__ OpacDev oR,
                                                      const __grid_constant__ OpacDev oS, const __grid_constant__ OpacSet os,
                                                      const double* __restrict__ rho, const double* __restrict__ T,
                                                      double* __restrict__ lim) {
-    const int ii = blockIdx.x * blockDim.x + threadIdx.x;
-    if (ii >= g.nt[0]) return;
-    const int jj = blockIdx.y, kk = blockIdx.z;
-    int c[3] = {ii - g.gh[0], jj - g.gh[1], kk - g.gh[2]};
-#pragma unroll
-    for (int e = 0; e < 3; ++e) {
-        const int n = g.n[e];
-        if (c[e] < 0) c[e] = (g.bc[2 * e] == 0) ? c[e] + n : 0;
-        else if (c[e] >= n) c[e] = (g.bc[2 * e] == 0) ? c[e] - n : n - 1;
-    }
-    const long long src = (c[0] + g.gh[0]) * g.stride[0] + (c[1] + g.gh[1]) * g.stride[1] + (c[2] + g.gh[2]) * g.stride[2];
-    const long long dst = ii * g.stride[0] + jj * g.stride[1] + kk * g.stride[2];
-    const double r = rho[src], t = T[src];
-    LogRT l = {0.0, 0.0};
+    const int kk = blockIdx.y;
+    int c2 = kk - g.gh[2];
+    if (c2 < 0) c2 = (g.bc[4] == 0) ? c2 + g.n[2] : 0;
+    else if (c2 >= g.n[2]) c2 = (g.bc[4] == 0) ? c2 - g.n[2] : g.n[2] - 1;
     const bool share = os.share != 0;
-    if (share) l = log_inputs(os.src == RT_OPAC_SCATTER_IDX ? oS : oR, r, t);
-    const double chi = opacity_eval_shared(oR, r, t, share, l) + opacity_eval_shared(oS, r, t, share, l);
-    double dx = 0.0;
+    const double k0 = oR.kappa0, ir0 = oR.irho0, it0 = oR.iT0, kmin = oR.kmin, kmax = oR.kmax;
+    const int na = oR.n2a, nb = oR.n2b;
+    const double* __restrict__ len0[3] = {g.len[0][0], g.len[1][0], g.len[2][0]};
+    const int gh0 = g.gh[0], n0 = g.n[0], nt0 = g.nt[0];
+    const bool per0 = g.bc[0] == 0;
+    for (int jr = 0; jr < kThickRows; ++jr) {
+        const int jj = blockIdx.x * kThickRows + jr;
+        if (jj >= g.nt[1]) break;
+        int c1 = jj - g.gh[1];
+        if (c1 < 0) c1 = (g.bc[2] == 0) ? c1 + g.n[1] : 0;
+        else if (c1 >= g.n[1]) c1 = (g.bc[2] == 0) ? c1 - g.n[1] : g.n[1] - 1;
+        // rows are block-uniform: 64-bit row bases once, 32-bit offsets along x1
+        const long long srow = (c1 + g.gh[1]) * g.stride[1] + (c2 + g.gh[2]) * g.stride[2];
+        const double* __restrict__ rrow = rho + srow;
+        const double* __restrict__ trow = T + srow;
+        double* __restrict__ lrow = lim + jj * g.stride[1] + kk * g.stride[2];
+        double l12[3];  // the x2 and x3 factors of the three cell lengths (0 for an inactive direction)
 #pragma unroll
-    for (int d = 0; d < 3; ++d)
-        if (g.gh[d] > 0) dx = dmax(dx, g.len[d][0][c[0]] * g.len[d][1][c[1]] * g.len[d][2][c[2]]);
-    const double tau = r * chi * dx;
-    // any value >= 1 means "no limit" (|lambda| <= 1, L167): tau -> 0 maps to +inf without a division by zero
-    lim[dst] = tau > 1.0e-100 ? 4.0 * frcp(3.0 * tau) : __builtin_huge_val();
+        for (int d = 0; d < 3; ++d) l12[d] = g.gh[d] > 0 ? 1.0 : 0.0;
+        for (int ii = threadIdx.x; ii < nt0; ii += blockDim.x) {
+            int c0 = ii - gh0;
+            if (c0 < 0) c0 = per0 ? c0 + n0 : 0;
+            else if (c0 >= n0) c0 = per0 ? c0 - n0 : n0 - 1;
+            const double r = __ldg(rrow + c0 + gh0), t = __ldg(trow + c0 + gh0);
+            double chi;
+            if (LEAN) {
+                chi = power_law_fast_v(k0, ir0, it0, na, nb, kmin, kmax, r, t);
+            } else {
+                LogRT l = {0.0, 0.0};
+                if (share) l = log_inputs(os.src == RT_OPAC_SCATTER_IDX ? oS : oR, r, t);
+                chi = opacity_eval_shared(oR, r, t, share, l) + opacity_eval_shared(oS, r, t, share, l);
+            }
+            double dx = 0.0;
+#pragma unroll
+            for (int d = 0; d < 3; ++d)
+                dx = dmax(dx, l12[d] * (__ldg(len0[d] + c0) * __ldg(g.len[d][1] + c1) * __ldg(g.len[d][2] + c2)));
+            const double tau = r * chi * dx;
+            // any value >= 1 means "no limit" (|lambda| <= 1, L167): tau -> 0 maps to +inf without a division by zero
+            lrow[ii] = tau > 1.0e-100 ? 4.0 * frcp(3.0 * tau) : __builtin_huge_val();
+        }
+    }
 }
 
 // ------------------------------------------------------------------------------------------------

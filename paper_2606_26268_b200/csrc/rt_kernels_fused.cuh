@@ -290,38 +290,6 @@ __global__ void __launch_bounds__(FNT, 2)
         double qc[4];
 #pragma unroll
         for (int q = 0; q < 4; ++q) qc[q] = pc[q * FPS + o];
-        // ---------------------------------------------------------------- Y: face states; the upper one to the row above
-        State ylo;
-        {
-            double dm[4], dp[4];
-#pragma unroll
-            for (int q = 0; q < 4; ++q) {
-                dm[q] = qc[q] - pc[q * FPS + o - FPW];
-                dp[q] = pc[q * FPS + o + FPW] - qc[q];
-            }
-            State hi;
-            cell_faces<1, HLL>(qc, dm, dp, true, true, ylo, hi);
-            if (ly < FTY - 1) {
-                state_store<HLL, FNT>(yex, tid, hi);
-                pair_arrive(1 + ly);
-            } else {
-                // top row: the lower-face state of the cell above the tile, and the flux through the face between them
-                double qa[4], dma[4], dpa[4];
-#pragma unroll
-                for (int q = 0; q < 4; ++q) {
-                    qa[q] = pc[q * FPS + o + FPW];
-                    dma[q] = qa[q] - qc[q];
-                    dpa[q] = pc[q * FPS + o + 2 * FPW] - qa[q];
-                }
-                State loa, hia;
-                cell_faces<1, HLL>(qa, dma, dpa, true, false, loa, hia);
-                const double limd = THICK ? dmax(pc[4 * FPS + o], pc[4 * FPS + o + FPW]) : kInf;
-                double fup[4];
-                riemann<HLL>(hi, loa, limd, fup);
-#pragma unroll
-                for (int q = 0; q < 4; ++q) yex[q * FNT + tid] = CURVI ? fup[q] * wyhi : fup[q];
-            }
-        }
         // ---------------------------------------------------------------- X
         {
             double dm[4], dp[4];
@@ -374,6 +342,38 @@ __global__ void __launch_bounds__(FNT, 2)
                     acc[2] = fma(s, fma(ct, Ppp, -Prt), acc[2]);
                     acc[3] = fma(-s, fma(ct, Ptp, Prp), acc[3]);
                 }
+            }
+        }
+        // ---------------------------------------------------------------- Y: face states; the upper one to the row above
+        State ylo;
+        {
+            double dm[4], dp[4];
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                dm[q] = qc[q] - pc[q * FPS + o - FPW];
+                dp[q] = pc[q * FPS + o + FPW] - qc[q];
+            }
+            State hi;
+            cell_faces<1, HLL>(qc, dm, dp, true, true, ylo, hi);
+            if (ly < FTY - 1) {
+                state_store<HLL, FNT>(yex, tid, hi);
+                pair_arrive(1 + ly);
+            } else {
+                // top row: the lower-face state of the cell above the tile, and the flux through the face between them
+                double qa[4], dma[4], dpa[4];
+#pragma unroll
+                for (int q = 0; q < 4; ++q) {
+                    qa[q] = pc[q * FPS + o + FPW];
+                    dma[q] = qa[q] - qc[q];
+                    dpa[q] = pc[q * FPS + o + 2 * FPW] - qa[q];
+                }
+                State loa, hia;
+                cell_faces<1, HLL>(qa, dma, dpa, true, false, loa, hia);
+                const double limd = THICK ? dmax(pc[4 * FPS + o], pc[4 * FPS + o + FPW]) : kInf;
+                double fup[4];
+                riemann<HLL>(hi, loa, limd, fup);
+#pragma unroll
+                for (int q = 0; q < 4; ++q) yex[q * FNT + tid] = CURVI ? fup[q] * wyhi : fup[q];
             }
         }
         // ---------------------------------------------------------------- Y: flux through the lower x2 face
