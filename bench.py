@@ -3,9 +3,11 @@
     python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C4|C5|C3|CP] [--impl native|reference]
 
 A "step" is one pass of the whole hot path over the resident fields, one rt_substep call: ghost fill ->
-thick-limit pre-pass -> fused sweeps x1/x2/x3 -> floor + opacities + implicit coupling with the CFL reduction
-of the updated state fused behind it (the time step stays on the device).  `--api split` times the three-call
-form rt_cfl_dt (8-byte result to the host) -> rt_explicit_step -> rt_implicit_step instead.  Default workload: C4,
+thick-limit pre-pass -> k_substep_fused (ONE kernel: reconstruction, f-fix, closure, wave speeds, Riemann fluxes of
+the three directions, flux divergence + geometric sources, floor, opacities, implicit coupling, CFL rate of the
+updated state) -> one-thread dt finalise; the time step stays on the device.  `--fused-seg -1` runs the same call
+on the per-direction kernels (x1/x2/x3 sweeps + implicit), `--api split` times the three-call form rt_cfl_dt
+(8-byte result to the host) -> rt_explicit_step -> rt_implicit_step.  Default workload: C4,
 the 256^3 Cartesian config the north_star target is quoted on (C5 = the spherical one).
 Prints ONE JSON line (see DESIGN.md "Measurement" for every key).  `--impl reference` times the CPU
 oracle instead (the only other place oracle/ may be executed besides the cpu_baseline leg).
@@ -27,6 +29,15 @@ METRIC = "radiation cell-updates/sec (fp64, 1 B200)"
 UNIT = "cell-updates/s"
 
 FUSED_CFL = True
+
+# fp64-pipe roof (DESIGN.md Sect. 5): 148 SMs x 64 fp64 lanes/clk x 1.965 GHz (B200_PROFILING.md unit counts and clock)
+FP64_PEAK_TINST = 148 * 64 * 1.965e9 / 1e12
+# Algorithmic fp64-pipe instructions (DFMA/DMUL/DADD/DSETP) per cell-update of k_substep_fused: ncu's executed count of
+# the committed capture (profiles/r1_ncu_full_fused.md) x the useful-lane fraction of the launch (30 of 32 lanes along
+# x1 and the ragged last tile, edge-row extras, segment ends) -- derivation in DESIGN.md Sect. 5.
+FUSED_FP64_PER_CELL = {"C4": 0.5 * (800.0 + 680.0),   # HLL / GLF alternate
+                       "C5": 935.0}                    # HLL, spherical, table opacities
+
 
 # Algorithmic bytes per interior cell and launch: 8 B x (fields read + written)
 def bytes_per_cell(kind, thick, feedback):
@@ -72,7 +83,8 @@ def workload_config(w, args):
     n = w.n
     cfg = {"workload": "%s: %s %dx%dx%d, %s" % (w.name, ("cartesian", "cylindrical", "spherical")[w.geometry], n[0], n[1], n[2],
                                                 w.notes),
-           "cells": w.ncells, "substep": "rt_substep (device-resident dt)" if args.api == "fused" else
+           "cells": w.ncells, "substep": ("rt_substep (k_substep_fused, device-resident dt)" if args.fused_seg >= 0 else
+                                       "rt_substep (per-direction kernels, device-resident dt)") if args.api == "fused" else
            "rt_cfl_dt + rt_explicit_step + rt_implicit_step",
            "solver": "HLL/GLF alternating" if w.solver_schedule else ("HLL" if w.params["solver"] == 0 else "GLF"),
            "thick_limit": int(w.params["thick_limit"]), "feedback_momentum": int(w.params["feedback_momentum"]),
@@ -231,6 +243,18 @@ def run_native(args):
                 "substep_alg_bytes_per_cell": sum(bytes_per_cell(k, thick, feedback) * kernels[k]["launches_per_step"]
                                                   for k in kernels),
                 "substep_GBps": None, "kernel_ms_sum_per_step": round(tot_ms / K, 4)}
+    if dom == "fused" and w.name in FUSED_FP64_PER_CELL and not args.size:
+        # the fused kernel is bound by the fp64 pipe, not by HBM (DESIGN.md Sect. 5): report it against that roof and
+        # keep its HBM figure beside it
+        inst = FUSED_FP64_PER_CELL[w.name] * w.ncells
+        ach = inst / (kernels[dom]["avg_ms"] * 1e-3) / 1e12
+        roofline.update({"bound": "alu", "achieved": round(ach, 3), "peak": round(FP64_PEAK_TINST, 3),
+                         "unit": "Tinst/s (fp64 pipe: DFMA/DMUL/DADD/DSETP thread instructions)",
+                         "frac": round(ach / FP64_PEAK_TINST, 4),
+                         "peak_source": "148 SMs x 64 fp64 lanes/clk x 1.965 GHz (B200_PROFILING.md unit counts and clock)",
+                         "alg_fp64_inst_per_cell": FUSED_FP64_PER_CELL[w.name],
+                         "hbm": {"achieved": achieved, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                                 "frac": round(achieved / peaks["hbm_gbs"], 4), "peak_source": peaks["source"]}})
     roofline["substep_GBps"] = round(roofline["substep_alg_bytes_per_cell"] * value / world / 1e9, 1)
     roofline["substep_frac"] = round(roofline["substep_GBps"] / peaks["hbm_gbs"], 4)
 
@@ -265,14 +289,17 @@ def load_peaks():
 
 
 def load_traffic(kernel, workload):
-    """DRAM bytes per launch of `kernel` from the committed ncu --set full capture (profiles/ncu_traffic.json,
-    written by hand from the capture named inside it), or None"""
+    """DRAM bytes per launch of `kernel` from the committed ncu --set full capture (profiles/ncu_traffic.csv,
+    written by hand from the capture named in profiles/ncu_traffic.md), or None"""
     try:
-        with open(os.path.join(ROOT, "profiles", "ncu_traffic.json")) as fh:
-            d = json.load(fh)
-        return d.get(workload, {}).get(kernel)
+        with open(os.path.join(ROOT, "profiles", "ncu_traffic.csv")) as fh:
+            for line in fh.read().splitlines()[1:]:
+                wl, k, b = line.split(",")
+                if wl == workload and k == kernel:
+                    return float(b)
     except Exception:
-        return None
+        pass
+    return None
 
 
 def run_e2e(rt, g, w, st, K, world, dev, barrier):

@@ -1,27 +1,31 @@
 // rt_kernels_fused.cuh — ONE kernel for the whole sub-step on 3-D grids (SURVEY.md Sect. 8(f) NEXT-1):
 // steps 3-8 and the rate of step 10 in a single pass over U^n.
 //
-// Design.  A CTA owns an x1-x2 tile of 30 x FTY cells and marches
-// along x3 through a segment [ka, kb).  The x1-x2 planes of U^n (and of the thick-limit array) it
-// needs — tile + 2 ghost cells on each side — are staged in shared memory by TMA (one
+// Design (DESIGN.md Sect. 5 "Fused sub-step kernel").  A CTA of 32 x FTY threads owns an x1-x2 tile of
+// 30 x FTY cells and marches along x3 through a segment [ka, kb).  The x1-x2 planes of U^n (and of the
+// thick-limit array) it needs — tile + 2 ghost cells on each side — are staged in shared memory by TMA (one
 // cp.async.bulk.tensor.3d box of 34 x (FTY+4) x 1 doubles per field and plane, issued by one thread,
 // completion on an mbarrier) into a ring of four planes (c-1, c, c+1 in use, c+2 in flight): every
 // stencil value is read from HBM/L2 once per CTA, the loads occupy no registers and no issue slots, and
 // boxes hanging over the array edge are zero-filled by the hardware.  Arrays the TMA cannot address
 // (odd x1 extent => row pitch not a multiple of 16 B, or a base pointer not 16-B aligned) take an
-// 8-byte cp.async loop instead.  Thread (lx, ly) owns cell (i0-1+lx, j0-1+ly): lanes 0 and 31 and rows 0
-// and FTY+1 are the halo whose face states the tile's outer faces need.  Per plane c:
+// 8-byte cp.async loop instead.  Thread (lx, ly) owns cell (i0-1+lx, j0+ly): lanes 0 and 31 are the x1 halo
+// whose face states the tile's outer x1 faces need.  Per plane c, every thread:
 //   Z  : both x3 face states of cell c (Eq. 17-21 + closure + speeds), Riemann flux at face c-1/2 against
 //        the upper-face state of cell c-1 kept in this thread's shared-memory slot;
 //   FIN: cell c-1 is complete: U* = acc - dt/V [A F]_z, then floor/clip, opacities, implicit coupling
-//        (Eq. 29-33, 30, 28), stores, CFL rate of the updated state (a8-a11);
-//   Y  : x2 face states; the upper-face state goes to the row above through shared memory, guarded by a
-//        64-thread named barrier per row pair (producer bar.arrive, consumer bar.sync), and the flux of the
-//        upper face comes back the same way one step later (after the per-plane __syncthreads);
-//   X  : x1 face states; exchanged by warp shuffles; + geometric sources;   acc = U^n - dt/V([AF]_x + [AF]_y).
-// One __syncthreads per plane.  Every closure, wave speed and Riemann flux is evaluated once per face inside
-// the tile; the halo costs 32/30 in x1 and (3 FTY + 1)/(3 FTY) in x2.  Face states, fluxes and U* never
-// touch HBM.
+//        (Eq. 29-33, 30, 28), stores, CFL rate of the updated state (a8-a11); its rho, T, m were
+//        prefetched into L2 one plane earlier;
+//   X  : x1 face states; exchanged by warp shuffles; + geometric sources;
+//   Y  : x2 face states; the upper-face state goes to the row above through the thread's shared-memory slot,
+//        guarded by a 64-thread named barrier per row pair (producer bar.arrive, consumer bar.sync); the row
+//        above computes the flux through that face and writes it back INTO THE SAME SLOT, where the owner picks
+//        it up one plane later (after the per-plane __syncthreads).  The bottom row builds the upper-face state
+//        of the cell below the tile itself, the top row the lower-face state of the cell above and that flux.
+//   acc = U^n - dt/V([AF]_x + [AF]_y) + dt S_geo.
+// One __syncthreads per plane, no idle warps.  Every closure, wave speed and Riemann flux is evaluated once per
+// face inside the tile; the halo costs 32/30 in x1 and one extra face state + flux per edge row in x2.  Face
+// states, fluxes and U* never touch HBM.
 #pragma once
 #include <cuda.h>  // CUtensorMap (type only: the encoder is fetched through cudaGetDriverEntryPoint)
 

@@ -278,8 +278,9 @@ def test_uniform_state_is_preserved_on_the_gpu(rt):
 
 
 # ----------------------------------------------------------------------------- the fused 3-D kernel
-# k_substep_fused owns 30 x 6 cells per CTA and marches x3 in segments: (141, 37, 35) leaves ragged tiles in x1
-# and x2; fused_seg = 12 cuts x3 into segments of 12 + 12 + 11, 0 = the library's own choice
+# k_substep_fused owns 30 x 8 cells per CTA and marches x3 in segments: (141, 37, 35) leaves ragged tiles in x1
+# and x2 and has an odd x1 pitch (planes staged by cp.async); the even-pitch shapes below go through TMA.
+# fused_seg = 12 cuts x3 into segments of 12 + 12 + 11, 0 = the library's own choice
 @pytest.mark.parametrize("geometry", [W.CARTESIAN, W.CYLINDRICAL, W.SPHERICAL])
 @pytest.mark.parametrize("solver", [W.SOLVER_HLL, W.SOLVER_GLF])
 @pytest.mark.parametrize("thick", [0, 1])
@@ -291,7 +292,7 @@ def test_fused_kernel_one_substep_random_states(rt, geometry, solver, thick):
         assert counts[0] == counts[1]
 
 
-@pytest.mark.parametrize("n", [(2, 2, 2), (31, 7, 3), (30, 6, 40), (61, 13, 2), (3, 50, 5)])
+@pytest.mark.parametrize("n", [(2, 2, 2), (31, 7, 3), (30, 8, 40), (61, 13, 2), (3, 50, 5), (64, 17, 33), (92, 24, 9)])
 def test_fused_kernel_small_and_ragged_shapes(rt, n):
     w = random_workload(W.CARTESIAN, n, W.SOLVER_HLL, 1, seed=23 + sum(n))
     errs, counts, _ = run_both(rt, w, 1, fused=True)
