@@ -44,6 +44,9 @@ constexpr int FPHW = FPW * FPH;
 constexpr int FPS = (FPHW + 15) / 16 * 16;  // doubles between staged arrays: every TMA destination 128-B aligned
 constexpr int FNARR = 5;          // E, F1, F2, F3, lim
 constexpr int FNSLOT = 4;
+#ifndef FUSED_MINB
+#define FUSED_MINB 2
+#endif
 constexpr int FNST = 10;          // doubles of an exchanged face state: U[4], G[4], lm, lp
 // staged planes | zhi[FNST][FNT] | yex[FNST][FNT] | mbarriers
 constexpr size_t kFusedSmemBytes =
@@ -132,7 +135,7 @@ __device__ __forceinline__ void state_load(const double* buf, int t, State& s) {
 
 
 template <bool HLL, bool THICK, bool CURVI, bool FEEDBACK>
-__global__ void __launch_bounds__(FNT, 2)
+__global__ void __launch_bounds__(FNT, FUSED_MINB)
     k_substep_fused(const __grid_constant__ GridDev g, const __grid_constant__ ParamsDev par, const __grid_constant__ OpacDev oP,
                     const __grid_constant__ OpacDev oR, const __grid_constant__ OpacDev oS, const __grid_constant__ FusedArgs a,
                     const __grid_constant__ FusedMaps maps, int seglen) {
@@ -234,6 +237,13 @@ __global__ void __launch_bounds__(FNT, 2)
                 for (int q = 0; q < 3; ++q) prefetch_l2(a.im.mom[q] + idn);
             }
         }
+        // gas state of cell c-1 for FIN: issued here so that the x3 phase hides what is left of its latency
+        double rho_f = 1.0, T_f = 1.0;
+        if (writer && c > ka) {
+            const int id = id0 + (c - 1) * zstride;
+            rho_f = __ldg(a.im.rho + id);
+            T_f = a.im.T[id];
+        }
         // ---------------------------------------------------------------- Z
         {
             const double* pm = planes + ((c + 3) & 3) * (FNARR * FPS);
@@ -269,8 +279,7 @@ __global__ void __launch_bounds__(FNT, 2)
                 for (int q = 0; q < 4; ++q) U4[q] = fma(-coef, flz[q] - Fz[q], fma(-cyp, yex[q * FNT + tid], acc[q]));
                 if (writer) {
                     const int id = id0 + (c - 1) * zstride;
-                    const double rho = __ldg(a.im.rho + id);
-                    const double T0 = a.im.T[id];
+                    const double rho = rho_f, T0 = T_f;
                     double m[3] = {0.0, 0.0, 0.0};
                     if (FEEDBACK) {
 #pragma unroll
@@ -279,8 +288,15 @@ __global__ void __launch_bounds__(FNT, 2)
                     double F[3] = {U4[1], U4[2], U4[3]};
                     const double il[3] = {ilxy[0] * g.ilen[0][2][c - 1], ilxy[1] * g.ilen[1][2][c - 1], ilxy[2] * g.ilen[2][2][c - 1]};
                     bool floored = false, clipped = false;
-                    const double r = implicit_cell<FEEDBACK, true>(g, par, oP, oR, oS, a.im, dt, (long long)id, il, U4[0], F, rho, T0, m,
-                                                                   floored, clipped);
+                    // rho chi of the cell from the thick-limit array of this sub-step: lim = 4/(3 rho chi dx), dx = the
+                    // cell's largest extent = 1/min_d(1/dl_d); lim = +inf stands for rho chi dx <= 1e-100
+                    double rhochi = 0.0;
+                    if (THICK) {
+                        const double lim = pm[4 * FPS + o];
+                        rhochi = lim > 1.0e300 ? 0.0 : (4.0 / 3.0) * dmin(il[0], dmin(il[1], il[2])) * frcp(lim);
+                    }
+                    const double r = implicit_cell<FEEDBACK, true, THICK>(g, par, oP, oR, oS, a.im, dt, (long long)id, il, U4[0], F, rho,
+                                                                          T0, m, floored, clipped, rhochi);
                     rate = dmax(rate, r);
                     nfloor += floored ? 1 : 0;
                     nclip += clipped ? 1 : 0;

@@ -230,11 +230,14 @@ struct ImplicitArgs {
 // maximum into dt.  The result equals rt_cfl_dt of the updated state bit for bit (same cell_rate, max is exact).
 // One cell of a8-a10 (+ the CFL rate of the updated state when CFL): shared by k_implicit and the fused
 // sub-step kernel.  E, F: the state after the explicit half; writes through the pointers of `a` at index id.
-template <bool FEEDBACK, bool CFL>
+// CHIGIVEN: rho chi of the cell is passed in (the fused kernel recovers it from the thick-limit array of the SAME
+// sub-step, lim = 4/(3 rho chi dx): kappa_R and sigma are then not evaluated a second time).
+template <bool FEEDBACK, bool CFL, bool CHIGIVEN = false>
 __device__ __forceinline__ double implicit_cell(const GridDev& g, const ParamsDev& par, const OpacDev& oP, const OpacDev& oR,
                                                 const OpacDev& oS, const ImplicitArgs& a, double dt, long long id,
                                                 const double il[3] /* 1/dl_d of the cell (CFL only) */, double E, double F[3],
-                                                double rho, double T0, const double m[3], bool& floored, bool& clipped) {
+                                                double rho, double T0, const double m[3], bool& floored, bool& clipped,
+                                                double rhochi_given = 0.0) {
     if (E < par.E_floor) {
         E = par.E_floor;
         floored = true;
@@ -246,12 +249,18 @@ __device__ __forceinline__ double implicit_cell(const GridDev& g, const ParamsDe
         for (int q = 0; q < 3; ++q) F[q] *= sc;
         clipped = true;
     }
-    LogRT lg = {0.0, 0.0};
-    const bool share = a.os.share != 0;
-    if (share) lg = log_inputs(a.os.src == 0 ? oP : (a.os.src == 1 ? oR : oS), rho, T0);
-    const double kP = opacity_eval_shared(oP, rho, T0, share, lg);
-    const double kR = a.same_PR ? kP : opacity_eval_shared(oR, rho, T0, share, lg);
-    const double chi = kR + opacity_eval_shared(oS, rho, T0, share, lg);
+    double kP, rhochi;
+    if (CHIGIVEN) {
+        kP = opacity_eval(oP, rho, T0);
+        rhochi = rhochi_given;
+    } else {
+        LogRT lg = {0.0, 0.0};
+        const bool share = a.os.share != 0;
+        if (share) lg = log_inputs(a.os.src == 0 ? oP : (a.os.src == 1 ? oR : oS), rho, T0);
+        kP = opacity_eval_shared(oP, rho, T0, share, lg);
+        const double kR = a.same_PR ? kP : opacity_eval_shared(oR, rho, T0, share, lg);
+        rhochi = (kR + opacity_eval_shared(oS, rho, T0, share, lg)) * rho;
+    }
     const double gr = dt * par.chat * kP * rho;
     const double gg = dt * par.c * kP * rho;
     const double Cv = rho * par.c_v;
@@ -261,7 +270,7 @@ __device__ __forceinline__ double implicit_cell(const GridDev& g, const ParamsDe
     const double idet = frcp(det);
     const double En = fma(E, fma(4.0 * gg, aT3, Cv), gr * Cv * aT4) * idet;
     const double Tn = fma((1.0 + gr) * Cv, T0, fma(3.0 * gg, aT4, gg * E)) * idet;
-    const double idamp = frcp(fma(dt * par.chat * chi, rho, 1.0));
+    const double idamp = frcp(fma(dt * par.chat, rhochi, 1.0));
     a.U[0][id] = En;
     a.T[id] = Tn;
     const double ichat = a.ichat;
