@@ -111,7 +111,9 @@ int32_t rt_implicit_step_cfl(rt_grid* g, double dt, const double* rho, double* T
  *   dt = *dt_device  ->  rt_explicit_step(dt, U_in -> U_out)  ->  rt_implicit_step_cfl(dt, U_out)  ->  *dt_device = next dt.
  * dt_device: DEVICE double, read by the kernels of this sub-step and overwritten at its end (seed it with
  * rt_cfl_dt_async).  No host synchronisation anywhere: a sequence of sub-steps can be enqueued back to back or
- * captured in a CUDA graph.  rho and T are required.  Same argument errors as the two halves. */
+ * captured in a CUDA graph.  rho and T are required.  Same argument errors as the two halves.  On 3-D grids the
+ * whole sub-step is one fused kernel (rt_set_tuning) and step 1 fills the face-normal ghosts of U_in only: edge and
+ * corner ghosts, which no stencil of the scheme reads, are left as they were. */
 int32_t rt_substep(rt_grid* g, double* dt_device, double cfl, const double* rho, double* T,
                    double* const mom[3], double* const U_in[4], double* const U_out[4]);
 

@@ -403,6 +403,29 @@ static int32_t launch_fill_ghosts(rt_grid* g, double* const U[4]) {
     return RT_OK;
 }
 
+// face-normal ghosts of all active axes in one launch (the sub-step kernels read nothing else)
+static int32_t launch_fill_faces(rt_grid* g, double* const U[4]) {
+    const GridDev& D = g->dev;
+    Fields4 F;
+    for (int q = 0; q < 4; ++q) F.q[q] = U[q];
+    long long tot = 0;
+    for (int d = 0; d < 3; ++d) {
+        if (D.gh[d] == 0 || (D.bc[2 * d] == RT_BC_FIXED && D.bc[2 * d + 1] == RT_BC_FIXED)) continue;
+        long long c = 4;
+        for (int e = 0; e < 3; ++e)
+            if (e != d) c *= D.n[e];
+        tot += c;
+    }
+    if (tot == 0) return RT_OK;
+    const int nb = (int)((tot + 255) / 256 > 8192 ? 8192 : (tot + 255) / 256);
+    {
+        ProfScope ps(g, RT_K_GHOST);
+        k_fill_faces<<<nb, 256, 0, g->stream>>>(D, F);
+    }
+    RT_LAUNCH_CHECK(g);
+    return RT_OK;
+}
+
 extern "C" int32_t rt_fill_ghosts(rt_grid* g, double* const U[4]) {
     if (!g || !U) return fail(g, RT_ERR_INVALID_ARG, "rt_fill_ghosts: null argument");
     for (int q = 0; q < 4; ++q)
@@ -718,7 +741,7 @@ static int32_t fused_impl(rt_grid* g, double* dt_device, double cfl, const doubl
     const GridDev& D = g->dev;
     const bool thick = g->par.thick_limit != 0;
 
-    int32_t rc = launch_fill_ghosts(g, U_in);
+    int32_t rc = launch_fill_faces(g, U_in);
     if (rc != RT_OK) return rc;
     if (thick) {
         rc = launch_thick_limit(g, rho, T);

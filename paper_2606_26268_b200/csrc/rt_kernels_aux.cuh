@@ -153,6 +153,53 @@ __global__ void k_fill_ghosts(GridDev g, Fields4 U, int d) {
     }
 }
 
+// a1 for the sub-step kernels, ONE launch: the face-normal ghosts of every active axis (other axes over their
+// interior range only).  The scheme never reads edge / corner ghosts — each direction's stencil leaves the
+// interior along its own axis only — so rt_substep does not need the axis-by-axis ordering of k_fill_ghosts.
+__global__ void k_fill_faces(GridDev g, Fields4 U) {
+    long long cnt[3], tot = 0;
+    for (int d = 0; d < 3; ++d) {
+        const int ea = (d == 0) ? 1 : 0, eb = (d == 2) ? 1 : 2;
+        const bool skip = g.gh[d] == 0 || (g.bc[2 * d] == 3 && g.bc[2 * d + 1] == 3);
+        cnt[d] = skip ? 0 : 4LL * g.n[ea] * g.n[eb];
+        tot += cnt[d];
+    }
+    for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < tot; t += (long long)gridDim.x * blockDim.x) {
+        long long r = t;
+        int d = 0;
+        while (r >= cnt[d]) {
+            r -= cnt[d];
+            ++d;
+        }
+        const int ea = (d == 0) ? 1 : 0, eb = (d == 2) ? 1 : 2;
+        const long long na = g.n[ea], nb = g.n[eb];
+        const int a = (int)(r % na);
+        const int b = (int)((r / na) % nb);
+        const int ls = (int)(r / (na * nb));  // 0..3
+        const int gl = ls & 1, side = ls >> 1;
+        const int kind = g.bc[2 * d + side];
+        if (kind == 3) continue;
+        const int nd = g.n[d];
+        const int dst = side == 0 ? -1 - gl : nd + gl;
+        int src;
+        if (kind == 0) src = side == 0 ? nd - 1 - gl : gl;
+        else if (kind == 1) src = side == 0 ? 0 : nd - 1;
+        else src = side == 0 ? gl : nd - 1 - gl;
+        int c[3];
+        c[ea] = a;
+        c[eb] = b;
+        c[d] = 0;
+        const long long base = (c[0] + g.gh[0]) * g.stride[0] + (c[1] + g.gh[1]) * g.stride[1] + (c[2] + g.gh[2]) * g.stride[2];
+        const long long id = base + dst * g.stride[d], is = base + src * g.stride[d];
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            double v = U.q[q][is];
+            if (kind == 2 && q == 1 + d) v = -v;
+            U.q[q][id] = v;
+        }
+    }
+}
+
 // ------------------------------------------------------------------------------------------------
 // a9: opacities.  Power law kappa0 (rho/rho0)^a (T/T0)^b clipped (L299) or bilinear table of
 // log10 kappa on a uniform (log10 rho, log10 T) grid (L375; R-G14).
@@ -310,7 +357,7 @@ __global__ void __launch_bounds__(128) k_thick_limit(const __grid_constant__ Gri
         double* __restrict__ lrow = lim + jj * g.stride[1] + kk * g.stride[2];
         double l12[3];  // the x2 and x3 factors of the three cell lengths (0 for an inactive direction)
 #pragma unroll
-        for (int d = 0; d < 3; ++d) l12[d] = g.gh[d] > 0 ? 1.0 : 0.0;
+        for (int d = 0; d < 3; ++d) l12[d] = g.gh[d] > 0 ? __ldg(g.len[d][1] + c1) * __ldg(g.len[d][2] + c2) : 0.0;
         for (int ii = threadIdx.x; ii < nt0; ii += blockDim.x) {
             int c0 = ii - gh0;
             if (c0 < 0) c0 = per0 ? c0 + n0 : 0;
@@ -327,7 +374,7 @@ __global__ void __launch_bounds__(128) k_thick_limit(const __grid_constant__ Gri
             double dx = 0.0;
 #pragma unroll
             for (int d = 0; d < 3; ++d)
-                dx = dmax(dx, l12[d] * (__ldg(len0[d] + c0) * __ldg(g.len[d][1] + c1) * __ldg(g.len[d][2] + c2)));
+                dx = dmax(dx, __ldg(len0[d] + c0) * l12[d]);
             const double tau = r * chi * dx;
             // any value >= 1 means "no limit" (|lambda| <= 1, L167): tau -> 0 maps to +inf without a division by zero
             lrow[ii] = tau > 1.0e-100 ? 4.0 * frcp(3.0 * tau) : __builtin_huge_val();
