@@ -29,6 +29,7 @@ METRIC = "radiation cell-updates/sec (fp64, 1 B200)"
 UNIT = "cell-updates/s"
 
 FUSED_CFL = True
+FUSED_KERNEL = True   # rt_substep runs k_substep_fused (3-D grids, --fused-seg >= 0, --api fused)
 
 # fp64-pipe roof (DESIGN.md Sect. 5): 148 SMs x 64 fp64 lanes/clk x 1.965 GHz (B200_PROFILING.md unit counts and clock)
 FP64_PEAK_TINST = 148 * 64 * 1.965e9 / 1e12
@@ -42,7 +43,7 @@ FUSED_FP64_PER_CELL = {"C4": 0.5 * (800.0 + 680.0),   # HLL / GLF alternate
 # Algorithmic bytes per interior cell and launch: 8 B x (fields read + written)
 def bytes_per_cell(kind, thick, feedback):
     return {
-        "thick_limit": 24.0,                                   # read rho, T; write lim
+        "thick_limit": 24.0 if not FUSED_KERNEL else 32.0,     # read rho, T; write lim (+ rho kappa_P for the fused kernel)
         "sweep_x1": 64.0 + (8.0 if thick else 0.0),            # read U 4 (+ lim); write U_out 4
         "sweep_x2": 96.0 + (8.0 if thick else 0.0),            # read U 4 (+ lim) + U_out 4; write U_out 4
         "sweep_x3": 96.0 + (8.0 if thick else 0.0),
@@ -50,7 +51,7 @@ def bytes_per_cell(kind, thick, feedback):
         "cfl": 32.0 if not FUSED_CFL else 0.0,                 # split API: read E,F; fused: a one-thread finalise kernel
         "ghost_fill": 0.0,                                     # O(surface)
         # k_substep_fused: read U 4 (+ lim), rho, T (+ m 3); write E, F, T (+ m 3)
-        "fused": 88.0 + (8.0 if thick else 0.0) + (48.0 if feedback else 0.0),
+        "fused": 88.0 + (16.0 if thick else 0.0) + (48.0 if feedback else 0.0),   # thick: + lim + rho kappa_P
     }[kind]
 
 
@@ -174,8 +175,9 @@ def run_native(args):
     if world > 1:
         dist.init_process_group("nccl", device_id=dev)
 
-    global FUSED_CFL
+    global FUSED_CFL, FUSED_KERNEL
     FUSED_CFL = args.api == "fused"
+    FUSED_KERNEL = FUSED_CFL and args.fused_seg >= 0
     w = make_workload(args.workload, args.size)
     g = rt.grid_from_workload(w, device=dev)
     g.set_tuning(fused_seg=args.fused_seg)

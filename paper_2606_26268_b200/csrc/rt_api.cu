@@ -20,6 +20,7 @@ struct rt_grid {
     cudaStream_t stream;
     double* metric_buf;
     double* lim;  // thick-limit pre-pass array, ntot doubles (lazily allocated)
+    double* kpr;  // rho kappa_P per cell, written by the pre-pass of the fused sub-step (lazily allocated)
     CflScratch* scr;
     double* dt_dev;
     double* dt_pinned;
@@ -151,6 +152,7 @@ extern "C" int32_t rt_grid_create(int32_t geometry, const int32_t n[3], int32_t 
     g->stream = reinterpret_cast<cudaStream_t>(cuda_stream);
     g->metric_buf = nullptr;
     g->lim = nullptr;
+    g->kpr = nullptr;
     g->scr = nullptr;
     g->dt_dev = nullptr;
     g->dt_pinned = nullptr;
@@ -247,6 +249,7 @@ extern "C" int32_t rt_grid_destroy(rt_grid* g) {
     }
     cudaFree(g->metric_buf);
     cudaFree(g->lim);
+    cudaFree(g->kpr);
     cudaFree(g->scr);
     cudaFree(g->dt_dev);
     cudaFree(g->counters);
@@ -474,22 +477,26 @@ static void launch_sweep(rt_grid* g, int d, bool hll, bool thick, bool curvi, co
     }
 }
 
-static int32_t launch_thick_limit(rt_grid* g, const double* rho, const double* T) {
+// with_kp: also write rho kappa_P per cell into g->kpr (fused sub-step: the implicit half then evaluates no opacity)
+static int32_t launch_thick_limit(rt_grid* g, const double* rho, const double* T, bool with_kp = false) {
     const GridDev& D = g->dev;
     if (!g->lim) RT_CUDA(g, cudaMalloc(&g->lim, (size_t)D.ntot * sizeof(double)));
+    if (with_kp && !g->kpr) RT_CUDA(g, cudaMalloc(&g->kpr, (size_t)D.ntot * sizeof(double)));
     const int bx = 128;
     dim3 grid((D.nt[1] + kThickRows - 1) / kThickRows, D.nt[2]);
     {
         ProfScope ps(g, RT_K_THICK);
-        const int members[2] = {RT_OPAC_ROSSELAND, RT_OPAC_SCATTER};
-        const bool lean = g->opac[RT_OPAC_ROSSELAND].set && g->opac[RT_OPAC_ROSSELAND].kind == 0 && g->opac[RT_OPAC_ROSSELAND].fast &&
-                          !g->opac[RT_OPAC_SCATTER].set;
+        const OpacDev &oP = g->opac[RT_OPAC_PLANCK], &oR = g->opac[RT_OPAC_ROSSELAND], &oS = g->opac[RT_OPAC_SCATTER];
+        const int m2[2] = {RT_OPAC_ROSSELAND, RT_OPAC_SCATTER};
+        const int m3[3] = {RT_OPAC_PLANCK, RT_OPAC_ROSSELAND, RT_OPAC_SCATTER};
+        const OpacSet os = with_kp ? opac_set(g, m3, 3) : opac_set(g, m2, 2);
+        bool lean = oR.set && oR.kind == 0 && oR.fast && !oS.set;
+        if (with_kp) lean = lean && (g->same_PR || (oP.set && oP.kind == 0 && oP.fast));
+        double* kpr = with_kp ? g->kpr : nullptr;
         if (lean)
-            k_thick_limit<true><<<grid, bx, 0, g->stream>>>(D, g->opac[RT_OPAC_ROSSELAND], g->opac[RT_OPAC_SCATTER],
-                                                            opac_set(g, members, 2), rho, T, g->lim);
+            k_thick_limit<true><<<grid, bx, 0, g->stream>>>(D, oR, oS, os, rho, T, g->lim, oP, g->same_PR, kpr);
         else
-            k_thick_limit<false><<<grid, bx, 0, g->stream>>>(D, g->opac[RT_OPAC_ROSSELAND], g->opac[RT_OPAC_SCATTER],
-                                                             opac_set(g, members, 2), rho, T, g->lim);
+            k_thick_limit<false><<<grid, bx, 0, g->stream>>>(D, oR, oS, os, rho, T, g->lim, oP, g->same_PR, kpr);
     }
     RT_LAUNCH_CHECK(g);
     return RT_OK;
@@ -744,7 +751,7 @@ static int32_t fused_impl(rt_grid* g, double* dt_device, double cfl, const doubl
     int32_t rc = launch_fill_faces(g, U_in);
     if (rc != RT_OK) return rc;
     if (thick) {
-        rc = launch_thick_limit(g, rho, T);
+        rc = launch_thick_limit(g, rho, T, true);
         if (rc != RT_OK) return rc;
     }
     FusedArgs a;
@@ -753,6 +760,7 @@ static int32_t fused_impl(rt_grid* g, double* dt_device, double cfl, const doubl
         a.im.U[q] = U_out[q];
     }
     a.src[4] = thick ? g->lim : nullptr;
+    a.kpr = thick ? g->kpr : nullptr;
     a.chat = g->par.chat;
     a.im.rho = rho;
     a.im.T = T;

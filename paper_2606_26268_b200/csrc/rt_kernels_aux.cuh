@@ -224,21 +224,13 @@ struct LogRT {
     double lrho, lT;
 };
 
-// x^(m2/2) for 0 <= m2 <= 15, m2 warp-uniform: one uniform branch into a straight-line product, one optional
-// square root; no loop, no selects
+// x^(m2/2) for 0 <= m2 <= 15, m2 uniform over the launch: binary powering with uniform predicates (no jump table,
+// no loop), one optional square root
 __device__ __forceinline__ double pow_half_small(double x, int m2) {
     const double x2 = x * x;
-    double r;
-    switch (m2 >> 1) {
-        case 0: r = 1.0; break;
-        case 1: r = x; break;
-        case 2: r = x2; break;
-        case 3: r = x2 * x; break;
-        case 4: r = x2 * x2; break;
-        case 5: r = x2 * x2 * x; break;
-        case 6: r = x2 * x2 * x2; break;
-        default: r = x2 * x2 * x2 * x; break;
-    }
+    double r = (m2 & 2) ? x : 1.0;
+    if (m2 & 4) r *= x2;
+    if (m2 & 8) r *= x2 * x2;
     if (m2 & 1) r *= fsqrt(x);
     return r;
 }
@@ -329,11 +321,15 @@ __device__ __forceinline__ double opacity_eval_shared(const OpacDev& o, double r
 // ------------------------------------------------------------------------------------------------
 constexpr int kThickRows = 4;  // x2 rows per block: ~200 k one-cell blocks cost more to schedule than to run
 // LEAN: chi is ONE half-integer power law (kappa_R fast, no scattering): its scalars live in registers
+// kpr != nullptr (fused sub-step): the pre-pass also hands rho kappa_P of every cell to the implicit half, so that
+// the fused kernel carries no opacity evaluation at all; oP / same_PR describe kappa_P (same_PR: kappa_P is the
+// same law as kappa_R and costs nothing extra).
 template <bool LEAN>
 __global__ void __launch_bounds__(128) k_thick_limit(const __grid_constant__ GridDev g, const __grid_constant__ OpacDev oR,
                                                      const __grid_constant__ OpacDev oS, const __grid_constant__ OpacSet os,
                                                      const double* __restrict__ rho, const double* __restrict__ T,
-                                                     double* __restrict__ lim) {
+                                                     double* __restrict__ lim, const __grid_constant__ OpacDev oP,
+                                                     int same_PR, double* __restrict__ kpr) {
     const int kk = blockIdx.y;
     int c2 = kk - g.gh[2];
     if (c2 < 0) c2 = (g.bc[4] == 0) ? c2 + g.n[2] : 0;
@@ -363,14 +359,18 @@ __global__ void __launch_bounds__(128) k_thick_limit(const __grid_constant__ Gri
             if (c0 < 0) c0 = per0 ? c0 + n0 : 0;
             else if (c0 >= n0) c0 = per0 ? c0 - n0 : n0 - 1;
             const double r = __ldg(rrow + c0 + gh0), t = __ldg(trow + c0 + gh0);
-            double chi;
+            double chi, kP = 0.0;
             if (LEAN) {
                 chi = power_law_fast_v(k0, ir0, it0, na, nb, kmin, kmax, r, t);
+                if (kpr) kP = same_PR ? chi : power_law_fast(oP, r, t);
             } else {
                 LogRT l = {0.0, 0.0};
-                if (share) l = log_inputs(os.src == RT_OPAC_SCATTER_IDX ? oS : oR, r, t);
-                chi = opacity_eval_shared(oR, r, t, share, l) + opacity_eval_shared(oS, r, t, share, l);
+                if (share) l = log_inputs(os.src == RT_OPAC_SCATTER_IDX ? oS : (os.src == 1 ? oR : oP), r, t);
+                const double kR = opacity_eval_shared(oR, r, t, share, l);
+                chi = kR + opacity_eval_shared(oS, r, t, share, l);
+                if (kpr) kP = same_PR ? kR : opacity_eval_shared(oP, r, t, share, l);
             }
+            if (kpr) kpr[jj * g.stride[1] + kk * g.stride[2] + ii] = kP * r;
             double dx = 0.0;
 #pragma unroll
             for (int d = 0; d < 3; ++d)

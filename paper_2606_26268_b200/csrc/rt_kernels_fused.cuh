@@ -55,6 +55,7 @@ static_assert(FTY <= 15, "one named barrier per row pair");
 
 struct FusedArgs {
     const double* src[FNARR];  // U_in[4], lim (or nullptr)
+    const double* kpr;         // rho kappa_P per cell from the pre-pass (with lim), or nullptr
     ImplicitArgs im;           // U = U_out, rho, T, mom, dt / dt_dev, scratch, counters
     double chat;
     int use_tma;
@@ -232,18 +233,21 @@ __global__ void __launch_bounds__(FNT, FUSED_MINB)
             const int idn = id0 + c * zstride;
             prefetch_l2(a.im.rho + idn);
             prefetch_l2(a.im.T + idn);
+            if (THICK) prefetch_l2(a.kpr + idn);
             if (FEEDBACK) {
 #pragma unroll
                 for (int q = 0; q < 3; ++q) prefetch_l2(a.im.mom[q] + idn);
             }
         }
         // gas state of cell c-1 for FIN: issued here so that the x3 phase hides what is left of its latency
-        double rho_f = 1.0, T_f = 1.0;
+        double rho_f = 1.0, T_f = 1.0, kpr_f = 0.0;
         if (writer && c > ka) {
             const int id = id0 + (c - 1) * zstride;
             rho_f = __ldg(a.im.rho + id);
             T_f = a.im.T[id];
+            if (THICK) kpr_f = __ldg(a.kpr + id);
         }
+        double invEc;
         // ---------------------------------------------------------------- Z
         {
             const double* pm = planes + ((c + 3) & 3) * (FNARR * FPS);
@@ -256,7 +260,8 @@ __global__ void __launch_bounds__(FNT, FUSED_MINB)
                 dp[q] = pp[q * FPS + o] - q0[q];
             }
             State lo, hi;
-            cell_faces<2, HLL>(q0, dm, dp, true, true, lo, hi);  // both always: one basic block, two independent chains
+            invEc = frcp(q0[0]);  // shared by the three directions of this cell
+            cell_faces<2, HLL, true>(q0, dm, dp, true, true, lo, hi, invEc);  // both always: one basic block, two independent chains
             double flz[4] = {0.0, 0.0, 0.0, 0.0};
             if (c >= ka) {
                 State L;
@@ -296,7 +301,7 @@ __global__ void __launch_bounds__(FNT, FUSED_MINB)
                         rhochi = lim > 1.0e300 ? 0.0 : (4.0 / 3.0) * dmin(il[0], dmin(il[1], il[2])) * frcp(lim);
                     }
                     const double r = implicit_cell<FEEDBACK, true, THICK>(g, par, oP, oR, oS, a.im, dt, (long long)id, il, U4[0], F, rho,
-                                                                          T0, m, floored, clipped, rhochi);
+                                                                          T0, m, floored, clipped, rhochi, kpr_f);
                     rate = dmax(rate, r);
                     nfloor += floored ? 1 : 0;
                     nclip += clipped ? 1 : 0;
@@ -319,7 +324,7 @@ __global__ void __launch_bounds__(FNT, FUSED_MINB)
                 dp[q] = pc[q * FPS + o + 1] - qc[q];
             }
             State lo, hi;
-            cell_faces<0, HLL>(qc, dm, dp, true, true, lo, hi);
+            cell_faces<0, HLL, true>(qc, dm, dp, true, true, lo, hi, invEc);
             State L;
 #pragma unroll
             for (int q = 0; q < 4; ++q) {
@@ -374,7 +379,7 @@ __global__ void __launch_bounds__(FNT, FUSED_MINB)
                 dp[q] = pc[q * FPS + o + FPW] - qc[q];
             }
             State hi;
-            cell_faces<1, HLL>(qc, dm, dp, true, true, ylo, hi);
+            cell_faces<1, HLL, true>(qc, dm, dp, true, true, ylo, hi, invEc);
             if (ly < FTY - 1) {
                 state_store<HLL, FNT>(yex, tid, hi);
                 pair_arrive(1 + ly);

@@ -230,14 +230,15 @@ struct ImplicitArgs {
 // maximum into dt.  The result equals rt_cfl_dt of the updated state bit for bit (same cell_rate, max is exact).
 // One cell of a8-a10 (+ the CFL rate of the updated state when CFL): shared by k_implicit and the fused
 // sub-step kernel.  E, F: the state after the explicit half; writes through the pointers of `a` at index id.
-// CHIGIVEN: rho chi of the cell is passed in (the fused kernel recovers it from the thick-limit array of the SAME
-// sub-step, lim = 4/(3 rho chi dx): kappa_R and sigma are then not evaluated a second time).
+// CHIGIVEN: rho chi and rho kappa_P of the cell are passed in (the fused kernel recovers the first from the
+// thick-limit array of the SAME sub-step, lim = 4/(3 rho chi dx), and gets the second from the same pre-pass): no
+// opacity is evaluated here.
 template <bool FEEDBACK, bool CFL, bool CHIGIVEN = false>
 __device__ __forceinline__ double implicit_cell(const GridDev& g, const ParamsDev& par, const OpacDev& oP, const OpacDev& oR,
                                                 const OpacDev& oS, const ImplicitArgs& a, double dt, long long id,
                                                 const double il[3] /* 1/dl_d of the cell (CFL only) */, double E, double F[3],
                                                 double rho, double T0, const double m[3], bool& floored, bool& clipped,
-                                                double rhochi_given = 0.0) {
+                                                double rhochi_given = 0.0, double rhokp_given = 0.0) {
     if (E < par.E_floor) {
         E = par.E_floor;
         floored = true;
@@ -249,20 +250,21 @@ __device__ __forceinline__ double implicit_cell(const GridDev& g, const ParamsDe
         for (int q = 0; q < 3; ++q) F[q] *= sc;
         clipped = true;
     }
-    double kP, rhochi;
+    double rhokp, rhochi;
     if (CHIGIVEN) {
-        kP = opacity_eval(oP, rho, T0);
+        rhokp = rhokp_given;
         rhochi = rhochi_given;
     } else {
         LogRT lg = {0.0, 0.0};
         const bool share = a.os.share != 0;
         if (share) lg = log_inputs(a.os.src == 0 ? oP : (a.os.src == 1 ? oR : oS), rho, T0);
-        kP = opacity_eval_shared(oP, rho, T0, share, lg);
+        const double kP = opacity_eval_shared(oP, rho, T0, share, lg);
         const double kR = a.same_PR ? kP : opacity_eval_shared(oR, rho, T0, share, lg);
+        rhokp = kP * rho;
         rhochi = (kR + opacity_eval_shared(oS, rho, T0, share, lg)) * rho;
     }
-    const double gr = dt * par.chat * kP * rho;
-    const double gg = dt * par.c * kP * rho;
+    const double gr = dt * par.chat * rhokp;
+    const double gg = dt * par.c * rhokp;
     const double Cv = rho * par.c_v;
     const double aT3 = par.a_R * T0 * T0 * T0;
     const double aT4 = aT3 * T0;

@@ -177,16 +177,17 @@ __device__ __forceinline__ void riemann(const State& L, const State& R, double l
 // Both face states of one cell along D from the cell value q0 and the two one-sided differences.
 // lo = state at the cell's lower face (RIGHT state of face c-1/2), hi = state at its upper face
 // (LEFT state of face c+1/2).  WANT_LO / WANT_HI are warp-uniform run-time flags.
-template <int D, bool HLL>
+// KNOWN: the caller passes 1/E_c (the three directions of one cell share it).
+template <int D, bool HLL, bool KNOWN = false>
 __device__ __forceinline__ void cell_faces(const double q0[4], const double dm[4], const double dp[4], bool want_lo,
-                                           bool want_hi, State& lo, State& hi) {
+                                           bool want_hi, State& lo, State& hi, double invEc_known = 0.0) {
     double h[4];
 #pragma unroll
     for (int q = 0; q < 4; ++q) h[q] = half_slope(dm[q], dp[q]);
     const double Ec = q0[0];
     const double Ec2 = Ec * Ec;
     const double F2c = fma(q0[3], q0[3], fma(q0[2], q0[2], q0[1] * q0[1]));
-    const double invEc = frcp(Ec);
+    const double invEc = KNOWN ? invEc_known : frcp(Ec);
     if (want_lo) {
 #pragma unroll
         for (int q = 0; q < 4; ++q) lo.U[q] = q0[q] - h[q];
