@@ -117,6 +117,14 @@ int32_t rt_implicit_step_cfl(rt_grid* g, double dt, const double* rho, double* T
 int32_t rt_substep(rt_grid* g, double* dt_device, double cfl, const double* rho, double* T,
                    double* const mom[3], double* const U_in[4], double* const U_out[4]);
 
+/* One RK2 step (L107, L256, L399: "two Euler sub-steps and the average", the integrator of the paper's tests; R-G10):
+ *   dt = *dt_device;  (U1,T1,m1) = substep(U,T,m; dt);  (U2,T2,m2) = substep(U1,T1,m1; dt);
+ *   U <- (U + U2)/2,  T <- (T^n + T2)/2,  m <- (m^n + m2)/2 on interior cells;  *dt_device = CFL time step of the new U.
+ * W1, W2: caller-owned work states (4 device arrays each, same layout as U; FIXED-boundary ghosts must be set in W1 as
+ * in U).  The library keeps T^n, m^n in handle-owned scratch.  No host synchronisation.  Errors as rt_substep. */
+int32_t rt_rk2_step(rt_grid* g, double* dt_device, double cfl, const double* rho, double* T,
+                    double* const mom[3], double* const U[4], double* const W1[4], double* const W2[4]);
+
 /* Step 10 (L120; R-G15): dt = cfl / max_cells sum_{d active} chat max(|lam1|,|lam3|)(U; d) / dl_d.
  * rt_cfl_dt writes a HOST double and synchronises the stream; rt_cfl_dt_async writes a DEVICE
  * double and does not synchronise (graph-capturable). */

@@ -318,3 +318,32 @@ def run_substeps(g, w, nsub, dts=None, state=None):
         g.implicit_step(dt, w.rho, T, mom, U2)
         U, U2 = U2, U
     return U, T, mom, used
+
+
+def run_rk2(g, w, nsteps):
+    """nsteps RK2 steps (two Euler sub-steps and the average of every evolved variable; DESIGN.md
+    R-G10) of workload w on grid g, each with the CFL time step of its starting state.  Returns (U, T, mom, dts)."""
+    U = [a.copy() for a in w.U]
+    T = w.T.copy()
+    mom = [a.copy() for a in w.mom] if w.mom is not None else None
+    U1 = [a.copy() for a in U]   # ghosts of FIXED boundaries must exist in every buffer
+    U2 = [a.copy() for a in U]
+    it = g.interior
+    g.set_params(make_params(**w.params))
+    used = []
+    for _ in range(nsteps):
+        dt = g.cfl_dt(U, w.cfl)
+        used.append(dt)
+        T0 = T.copy()
+        m0 = [a.copy() for a in mom] if mom is not None else None
+        g.explicit_step(dt, w.rho, T, U, U1)
+        g.implicit_step(dt, w.rho, T, mom, U1)
+        g.explicit_step(dt, w.rho, T, U1, U2)
+        g.implicit_step(dt, w.rho, T, mom, U2)
+        for q in range(4):
+            U[q][it] = 0.5 * (U[q][it] + U2[q][it])
+        T[it] = 0.5 * (T0[it] + T[it])
+        if mom is not None and w.params["feedback_momentum"]:
+            for q in range(3):
+                mom[q][it] = 0.5 * (m0[q][it] + mom[q][it])
+    return U, T, mom, used

@@ -20,6 +20,8 @@ struct rt_grid {
     cudaStream_t stream;
     double* metric_buf;
     double* lim;  // thick-limit pre-pass array, ntot doubles (lazily allocated)
+    double* rk_save[4];  // rt_rk2_step: T^n, m^n (lazily allocated)
+    double* rk_dt;       // rt_rk2_step: the dt each stage reads (and overwrites)
     double* kpr;  // rho kappa_P per cell, written by the pre-pass of the fused sub-step (lazily allocated)
     CflScratch* scr;
     double* dt_dev;
@@ -153,6 +155,8 @@ extern "C" int32_t rt_grid_create(int32_t geometry, const int32_t n[3], int32_t 
     g->metric_buf = nullptr;
     g->lim = nullptr;
     g->kpr = nullptr;
+    for (int q = 0; q < 4; ++q) g->rk_save[q] = nullptr;
+    g->rk_dt = nullptr;
     g->scr = nullptr;
     g->dt_dev = nullptr;
     g->dt_pinned = nullptr;
@@ -250,6 +254,8 @@ extern "C" int32_t rt_grid_destroy(rt_grid* g) {
     cudaFree(g->metric_buf);
     cudaFree(g->lim);
     cudaFree(g->kpr);
+    for (int q = 0; q < 4; ++q) cudaFree(g->rk_save[q]);
+    cudaFree(g->rk_dt);
     cudaFree(g->scr);
     cudaFree(g->dt_dev);
     cudaFree(g->counters);
@@ -807,6 +813,65 @@ extern "C" int32_t rt_substep(rt_grid* g, double* dt_device, double cfl, const d
     int32_t rc = explicit_impl(g, 0.0, dt_device, rho, T, U_in, U_out);
     if (rc != RT_OK) return rc;
     return implicit_impl(g, 0.0, dt_device, rho, T, mom, U_out, true, cfl, dt_device);
+}
+
+// internal form of rt_substep (arguments already validated by the callers' first use)
+static int32_t substep_impl(rt_grid* g, double* dt_device, double cfl, const double* rho, double* T, double* const mom[3],
+                            double* const U_in[4], double* const U_out[4]) {
+    if (fused_eligible(g)) return fused_impl(g, dt_device, cfl, rho, T, mom, U_in, U_out);
+    int32_t rc = explicit_impl(g, 0.0, dt_device, rho, T, U_in, U_out);
+    if (rc != RT_OK) return rc;
+    return implicit_impl(g, 0.0, dt_device, rho, T, mom, U_out, true, cfl, dt_device);
+}
+
+extern "C" int32_t rt_rk2_step(rt_grid* g, double* dt_device, double cfl, const double* rho, double* T, double* const mom[3],
+                               double* const U[4], double* const W1[4], double* const W2[4]) {
+    if (!g || !aligned8(dt_device)) return fail(g, RT_ERR_INVALID_ARG, "rt_rk2_step: null or misaligned dt_device");
+    if (!(cfl > 0.0) || !isfinite(cfl)) return fail(g, RT_ERR_INVALID_ARG, "rt_rk2_step: cfl must be finite and > 0");
+    if (!aligned8(rho) || !aligned8(T) || !U || !W1 || !W2) return fail(g, RT_ERR_INVALID_ARG, "rt_rk2_step: null or misaligned argument");
+    if (!g->have_par) return fail(g, RT_ERR_BAD_STATE, "rt_rk2_step: rt_set_params has not been called");
+    for (int q = 0; q < 4; ++q)
+        if (!aligned8(U[q]) || !aligned8(W1[q]) || !aligned8(W2[q]) || U[q] == W1[q] || U[q] == W2[q] || W1[q] == W2[q])
+            return fail(g, RT_ERR_INVALID_ARG, "rt_rk2_step: U/W1/W2[%d] null, misaligned or aliased", q);
+    const bool feedback = g->par.feedback_momentum && mom != nullptr;
+    if (feedback)
+        for (int q = 0; q < 3; ++q)
+            if (!aligned8(mom[q])) return fail(g, RT_ERR_INVALID_ARG, "rt_rk2_step: mom[%d] null or misaligned", q);
+    const GridDev& D = g->dev;
+    const size_t bytes = (size_t)D.ntot * sizeof(double);
+    const int nsave = feedback ? 4 : 1;
+    for (int q = 0; q < nsave; ++q)
+        if (!g->rk_save[q]) RT_CUDA(g, cudaMalloc(&g->rk_save[q], bytes));
+    if (!g->rk_dt) RT_CUDA(g, cudaMalloc(&g->rk_dt, 2 * sizeof(double)));
+    // T^n, m^n (the sub-steps update them in place) and two copies of dt (each stage overwrites the one it reads)
+    RT_CUDA(g, cudaMemcpyAsync(g->rk_save[0], T, bytes, cudaMemcpyDeviceToDevice, g->stream));
+    for (int q = 0; q < 3 && feedback; ++q)
+        RT_CUDA(g, cudaMemcpyAsync(g->rk_save[1 + q], mom[q], bytes, cudaMemcpyDeviceToDevice, g->stream));
+    RT_CUDA(g, cudaMemcpyAsync(g->rk_dt, dt_device, sizeof(double), cudaMemcpyDeviceToDevice, g->stream));
+    RT_CUDA(g, cudaMemcpyAsync(g->rk_dt + 1, dt_device, sizeof(double), cudaMemcpyDeviceToDevice, g->stream));
+    int32_t rc = substep_impl(g, g->rk_dt, cfl, rho, T, mom, U, W1);
+    if (rc != RT_OK) return rc;
+    rc = substep_impl(g, g->rk_dt + 1, cfl, rho, T, mom, W1, W2);
+    if (rc != RT_OK) return rc;
+    AvgArgs v;
+    memset(&v, 0, sizeof(v));
+    for (int q = 0; q < 4; ++q) {
+        v.a[q] = U[q];
+        v.b[q] = W2[q];
+    }
+    v.a[4] = T;                 // T <- (T^n + T^2)/2: a holds T^2 here, b the saved T^n: the average is symmetric
+    v.b[4] = g->rk_save[0];
+    v.n = 5;
+    for (int q = 0; q < 3 && feedback; ++q) {
+        v.a[5 + q] = mom[q];
+        v.b[5 + q] = g->rk_save[1 + q];
+        v.n = 8;
+    }
+    const int bx = D.n[0] >= 128 ? 128 : ((D.n[0] + 31) / 32) * 32;
+    dim3 grid((D.n[0] + bx - 1) / bx, D.n[1], D.n[2]);
+    k_rk2_average<<<grid, bx, 0, g->stream>>>(D, v);
+    RT_LAUNCH_CHECK(g);
+    return rt_cfl_dt_async(g, U, cfl, dt_device);
 }
 
 extern "C" int32_t rt_cfl_dt_async(rt_grid* g, const double* const U[4], double cfl, double* dt_device) {

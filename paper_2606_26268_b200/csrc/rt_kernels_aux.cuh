@@ -200,6 +200,20 @@ __global__ void k_fill_faces(GridDev g, Fields4 U) {
     }
 }
 
+// RK2 (L107, L256: two Euler sub-steps and the average of every evolved variable): q <- (q0 + q2)/2 on interior cells.
+// a[] = the fields holding q0 on entry and the average on exit; b[] = q2.  n = 4 (U), 1 (T) or 3 (m) pairs per launch.
+struct AvgArgs {
+    double* a[8];
+    const double* b[8];
+    int n;
+};
+__global__ void __launch_bounds__(128) k_rk2_average(const __grid_constant__ GridDev g, const __grid_constant__ AvgArgs v) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= g.n[0]) return;
+    const long long id = (i + g.gh[0]) + (blockIdx.y + g.gh[1]) * g.stride[1] + (blockIdx.z + g.gh[2]) * g.stride[2];
+    for (int q = 0; q < v.n; ++q) v.a[q][id] = 0.5 * (v.a[q][id] + v.b[q][id]);
+}
+
 // ------------------------------------------------------------------------------------------------
 // a9: opacities.  Power law kappa0 (rho/rho0)^a (T/T0)^b clipped (L299) or bilinear table of
 // log10 kappa on a uniform (log10 rho, log10 T) grid (L375; R-G14).

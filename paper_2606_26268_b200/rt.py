@@ -64,6 +64,8 @@ _SIGNATURES = {
                                          C.POINTER(C.c_void_p), C.c_double, C.c_void_p]),
     "rt_substep": (C.c_int32, [C.c_void_p, C.c_void_p, C.c_double, C.c_void_p, C.c_void_p, C.POINTER(C.c_void_p),
                                C.POINTER(C.c_void_p), C.POINTER(C.c_void_p)]),
+    "rt_rk2_step": (C.c_int32, [C.c_void_p, C.c_void_p, C.c_double, C.c_void_p, C.c_void_p, C.POINTER(C.c_void_p),
+                                C.POINTER(C.c_void_p), C.POINTER(C.c_void_p), C.POINTER(C.c_void_p)]),
     "rt_cfl_dt": (C.c_int32, [C.c_void_p, C.POINTER(C.c_void_p), C.c_double, _dp]),
     "rt_cfl_dt_async": (C.c_int32, [C.c_void_p, C.POINTER(C.c_void_p), C.c_double, C.c_void_p]),
     "rt_get_floor_counts": (C.c_int32, [C.c_void_p, C.POINTER(C.c_int64), C.POINTER(C.c_int64)]),
@@ -290,6 +292,22 @@ class Grid:
         if rc != OK:
             self._raise("rt_substep", rc)
 
+    def rk2_step(self, dt_device, cfl, rho, T, mom, U, W1, W2):
+        _check_field(rho, self.shape, "rho")
+        _check_field(T, self.shape, "T")
+        for q in range(4):
+            _check_field(U[q], self.shape, "U[%d]" % q)
+            _check_field(W1[q], self.shape, "W1[%d]" % q)
+            _check_field(W2[q], self.shape, "W2[%d]" % q)
+        if mom is not None:
+            for q in range(3):
+                _check_field(mom[q], self.shape, "mom[%d]" % q)
+        self._check_dt_device(dt_device)
+        rc = lib().rt_rk2_step(self._h, dt_device.data_ptr(), float(cfl), rho.data_ptr(), T.data_ptr(),
+                               _ptr_array(mom) if mom is not None else None, _ptr_array(U), _ptr_array(W1), _ptr_array(W2))
+        if rc != OK:
+            self._raise("rt_rk2_step", rc)
+
     @staticmethod
     def _check_dt_device(t):
         if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float64 and t.numel() >= 1):
@@ -398,3 +416,16 @@ def run_substeps_fused(g, w, nsub, st=None):
         g.substep(dt_dev, w.cfl, st.rho, st.T, st.mom, st.U, st.U2)
         st.U, st.U2 = st.U2, st.U
     return st, dt_dev, hist
+
+
+def run_rk2(g, w, nsteps, st=None):
+    """nsteps RK2 steps through rt_rk2_step (time step resident on the device).  Returns (state, dt history tensor)."""
+    st = st if st is not None else DeviceState(g, w)
+    W2 = [t.clone() for t in st.U]
+    dt_dev = torch.zeros(1, dtype=torch.float64, device=g.device)
+    hist = torch.zeros(nsteps, dtype=torch.float64, device=g.device)
+    g.cfl_dt_async(st.U, w.cfl, dt_dev)
+    for s in range(nsteps):
+        hist[s:s + 1].copy_(dt_dev)
+        g.rk2_step(dt_dev, w.cfl, st.rho, st.T, st.mom, st.U, st.U2, W2)
+    return st, hist

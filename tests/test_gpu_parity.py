@@ -367,6 +367,30 @@ def test_implicit_step_cfl_equals_implicit_then_cfl(rt):
     assert g.cfl_dt(a.U, 0.4) == float(dtn.item())
 
 
+# ----------------------------------------------------------------------------- RK2
+@pytest.mark.parametrize("case", ["3d-fused", "3d-spherical-tables", "1d", "2d-cyl"])
+def test_rk2_step_matches_the_oracle_composition(rt, case):
+    """rt_rk2_step = two sub-steps at one dt + the average of U, T, m (L107, L256); 4 steps against
+    oracle.ort.run_rk2, every dt (produced on the device) against the oracle's"""
+    if case == "3d-fused":
+        w = random_workload(W.CARTESIAN, (70, 33, 12), W.SOLVER_HLL, 1, seed=51, fmax=0.9)
+    elif case == "3d-spherical-tables":
+        w = random_workload(W.SPHERICAL, (45, 20, 11), W.SOLVER_GLF, 1, seed=52, fmax=0.9, table=True)
+    elif case == "1d":
+        w = random_workload(W.CARTESIAN, (300, 1, 1), W.SOLVER_HLL, 0, seed=53, fmax=0.95)
+    else:
+        w = random_workload(W.CYLINDRICAL, (33, 17, 1), W.SOLVER_HLL, 1, seed=54, fmax=0.9, bc=(2, 1, 0, 0, 1, 1))
+    og = ort.grid_from_workload(w)
+    refU, refT, refm, dts = ort.run_rk2(og, w, 4)
+    g = rt.grid_from_workload(w)
+    st, hist = rt.run_rk2(g, w, 4)
+    torch.cuda.synchronize()
+    errs = field_errors(w, to_host(st.U), refU, st.T.cpu().numpy(), refT, to_host(st.mom), refm)
+    assert_below(errs, 8 * TOL1, "RK2, " + case)
+    used = hist.cpu().numpy()
+    assert np.all(np.abs(used - np.array(dts)) <= 1e-12 * np.array(dts)), (used, dts)
+
+
 # ----------------------------------------------------------------------------- a11: CFL
 @pytest.mark.parametrize("geometry,n", [(W.CARTESIAN, (141, 37, 35)), (W.SPHERICAL, (67, 33, 18)), (W.CARTESIAN, (300, 1, 1)),
                                         (W.CYLINDRICAL, (1 + 32, 7, 1))])

@@ -205,3 +205,22 @@ def test_cfl_takes_the_worst_cell_and_curvilinear_lengths():
             s = (1 / (r[i + 1] - r[i]) + 1 / (rc[i] * (th[1] - th[0])) + 1 / (rc[i] * math.sin(thc[j]) * (ph[1] - ph[0])))
             rate = max(rate, s / math.sqrt(3))
     assert g.cfl_dt(U, 0.4) == pytest.approx(0.4 / rate, rel=1e-14)
+
+
+# ----------------------------------------------------------------------------- RK2 composition (L107, L256)
+def test_rk2_composition_conserves_the_coupled_energy_and_keeps_a_uniform_state_uniform():
+    """ort.run_rk2 = two Euler sub-steps at one dt and the average of E, F, T, m.  Each sub-step conserves
+    C_v T + (c/chat) E per cell exactly for a uniform state (no transport), so the average does; a uniform state
+    stays uniform."""
+    import rt_workloads as W
+    w = W.c1b()
+    g = ort.grid_from_workload(w)
+    p = w.params
+    it = g.interior
+    tot0 = w.rho[it] * p["c_v"] * w.T[it] + (p["c"] / p["chat"]) * w.U[0][it]
+    U, T, mom, dts = ort.run_rk2(g, w, 5)
+    tot = w.rho[it] * p["c_v"] * T[it] + (p["c"] / p["chat"]) * U[0][it]
+    assert np.all(np.abs(tot - tot0) <= 1e-13 * np.abs(tot0))
+    for a in (U[0][it], T[it]):
+        assert np.ptp(a) <= 1e-14 * np.abs(a).max()
+    assert len(dts) == 5 and all(d > 0 for d in dts)
