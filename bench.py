@@ -143,6 +143,19 @@ class ClockSampler(threading.Thread):
                 "samples": len(s)}
 
 
+def replicas_throughput(ms_local, cells, steps, world, device=None):
+    """whole-job throughput of `world` independent replicas (DESIGN.md Sect. 9: the path does not shard): every rank
+    runs `steps` sub-steps over `cells` cells in ms_local milliseconds; the job takes the slowest rank's time.
+    Returns (cell-updates/s over all ranks, max-over-ranks ms).  Uses the initialised process group when world > 1."""
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([ms_local], dtype=torch.float64, device=device)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms_max = float(t.item())
+    return world * cells * steps / (ms_max * 1e-3), ms_max
+
+
 # ------------------------------------------------------------------------------------------ native arm
 def one_substep(rt, g, w, st, step_index):
     """the whole hot path once"""
@@ -211,11 +224,7 @@ def run_native(args):
     clocks = sampler.stop()
     launches = g.launch_count() - l0
     ms = e0.elapsed_time(e1)
-    t = torch.tensor([ms], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms_max = float(t.item())
-    value = world * w.ncells * K / (ms_max * 1e-3)
+    value, ms_max = replicas_throughput(ms, w.ncells, K, world, dev)
 
     # ---- per-kernel device times over the same K steps (second, instrumented pass): roofline
     g.set_profiling(True)
@@ -373,12 +382,9 @@ def run_e2e(rt, g, w, st, K, world, dev, barrier):
     drain()                                       # the timed region ends when the last result is in host memory
     e1.record(cs)
     barrier()
-    t = torch.tensor([e0.elapsed_time(e1)], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms = float(t.item())
+    value, ms = replicas_throughput(e0.elapsed_time(e1), w.ncells, Ke, world, dev)
     del sets
-    return {"value": world * w.ncells * Ke / (ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+    return {"value": value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
             "steps": Ke, "ms_per_step": ms / Ke,
             "note": "pinned host buffers -> device -> C-ABI sub-step -> pinned host buffers; two device buffer sets, "
                     "copy-in / sub-step / copy-out of consecutive steps overlap on three streams"}
