@@ -241,11 +241,16 @@ struct LogRT {
 // x^(m2/2) for 0 <= m2 <= 15, m2 uniform over the launch: binary powering with uniform predicates (no jump table,
 // no loop), one optional square root
 __device__ __forceinline__ double pow_half_small(double x, int m2) {
-    const double x2 = x * x;
-    double r = (m2 & 2) ? x : 1.0;
-    if (m2 & 4) r *= x2;
-    if (m2 & 8) r *= x2 * x2;
-    if (m2 & 1) r *= fsqrt(x);
+    // the empty asm statements keep these launch-uniform tests real (uniform) branches: if-converted, each costs a
+    // multiplication plus two FSEL per cell whether taken or not
+    double r = 1.0;
+    if (m2 & 2) { r = x; asm volatile(""); }
+    if (m2 & 12) {
+        const double x2 = x * x;
+        if (m2 & 4) { r *= x2; asm volatile(""); }
+        if (m2 & 8) { r *= x2 * x2; asm volatile(""); }
+    }
+    if (m2 & 1) { r *= fsqrt(x); asm volatile(""); }
     return r;
 }
 
@@ -256,10 +261,10 @@ __device__ __forceinline__ double power_law_fast_v(double kappa0, double irho0, 
                                                    double kmax, double rho, double T) {
     const double pr = pow_half_small(rho * irho0, na < 0 ? -na : na);
     const double pt = pow_half_small(T * iT0, nb < 0 ? -nb : nb);
-    double num = kappa0, den = 1.0;
-    if (na < 0) den = pr; else num *= pr;
-    if (nb < 0) den *= pt; else num *= pt;
-    if ((na | nb) < 0) num *= frcp(den);
+    double num = kappa0, den = 1.0;   // launch-uniform tests kept as uniform branches (see pow_half_small)
+    if (na < 0) { den = pr; asm volatile(""); } else { num *= pr; asm volatile(""); }
+    if (nb < 0) { den *= pt; asm volatile(""); } else { num *= pt; asm volatile(""); }
+    if ((na | nb) < 0) { num *= frcp(den); asm volatile(""); }
     return dmin(dmax(num, kmin), kmax);
 }
 __device__ __forceinline__ double power_law_fast(const OpacDev& o, double rho, double T) {
