@@ -247,7 +247,7 @@ __global__ void __launch_bounds__(FNT, FUSED_MINB)
             T_f = a.im.T[id];
             if (THICK) kpr_f = __ldg(a.kpr + id);
         }
-        double invEc;
+        double invEc, Ec2, F2c;
         // ---------------------------------------------------------------- Z
         {
             const double* pm = planes + ((c + 3) & 3) * (FNARR * FPS);
@@ -260,8 +260,10 @@ __global__ void __launch_bounds__(FNT, FUSED_MINB)
                 dp[q] = pp[q * FPS + o] - q0[q];
             }
             State lo, hi;
-            invEc = frcp(q0[0]);  // shared by the three directions of this cell
-            cell_faces<2, HLL, true>(q0, dm, dp, true, true, lo, hi, invEc);  // both always: one basic block, two independent chains
+            invEc = frcp(q0[0]);  // 1/E_c, E_c^2, |F_c|^2: shared by the three directions of this cell
+            Ec2 = q0[0] * q0[0];
+            F2c = fma(q0[3], q0[3], fma(q0[2], q0[2], q0[1] * q0[1]));
+            cell_faces<2, HLL, true>(q0, dm, dp, true, true, lo, hi, invEc, Ec2, F2c);  // both always: one basic block, two independent chains
             double flz[4] = {0.0, 0.0, 0.0, 0.0};
             if (c >= ka) {
                 State L;
@@ -324,7 +326,7 @@ __global__ void __launch_bounds__(FNT, FUSED_MINB)
                 dp[q] = pc[q * FPS + o + 1] - qc[q];
             }
             State lo, hi;
-            cell_faces<0, HLL, true>(qc, dm, dp, true, true, lo, hi, invEc);
+            cell_faces<0, HLL, true>(qc, dm, dp, true, true, lo, hi, invEc, Ec2, F2c);
             State L;
 #pragma unroll
             for (int q = 0; q < 4; ++q) {
@@ -379,7 +381,7 @@ __global__ void __launch_bounds__(FNT, FUSED_MINB)
                 dp[q] = pc[q * FPS + o + FPW] - qc[q];
             }
             State hi;
-            cell_faces<1, HLL, true>(qc, dm, dp, true, true, ylo, hi, invEc);
+            cell_faces<1, HLL, true>(qc, dm, dp, true, true, ylo, hi, invEc, Ec2, F2c);
             if (ly < FTY - 1) {
                 state_store<HLL, FNT>(yex, tid, hi);
                 pair_arrive(1 + ly);

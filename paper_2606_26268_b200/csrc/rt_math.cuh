@@ -155,8 +155,11 @@ template <bool HLL>
 __device__ __forceinline__ void riemann(const State& L, const State& R, double limd, double flux[4]) {
     double sR, sL;
     if (HLL) {
-        sL = dmin(dmin(L.lm, R.lm), 0.0);
-        sR = dmax(dmax(L.lp, R.lp), 0.0);
+        // S_L = min(lm_L, lm_R, 0), S_R = max(lp_L, lp_R, 0) (R-G6), clamped by -+limd (Eq. 25-26), then kept off zero
+        // (R-G8).  The last clamp subsumes the "0" of the first (a positive min ends at -tiny either way), so the
+        // comparison against 0 is not spelled out.
+        sL = dmin(L.lm, R.lm);
+        sR = dmax(L.lp, R.lp);
         sL = dmax(sL, -limd);
         sR = dmin(sR, limd);
         sL = dmin(sL, -kTinySpeed);
@@ -177,16 +180,17 @@ __device__ __forceinline__ void riemann(const State& L, const State& R, double l
 // Both face states of one cell along D from the cell value q0 and the two one-sided differences.
 // lo = state at the cell's lower face (RIGHT state of face c-1/2), hi = state at its upper face
 // (LEFT state of face c+1/2).  WANT_LO / WANT_HI are warp-uniform run-time flags.
-// KNOWN: the caller passes 1/E_c (the three directions of one cell share it).
+// KNOWN: the caller passes 1/E_c, E_c^2 and |F_c|^2 (the three directions of one cell share them).
 template <int D, bool HLL, bool KNOWN = false>
 __device__ __forceinline__ void cell_faces(const double q0[4], const double dm[4], const double dp[4], bool want_lo,
-                                           bool want_hi, State& lo, State& hi, double invEc_known = 0.0) {
+                                           bool want_hi, State& lo, State& hi, double invEc_known = 0.0,
+                                           double Ec2_known = 0.0, double F2c_known = 0.0) {
     double h[4];
 #pragma unroll
     for (int q = 0; q < 4; ++q) h[q] = half_slope(dm[q], dp[q]);
     const double Ec = q0[0];
-    const double Ec2 = Ec * Ec;
-    const double F2c = fma(q0[3], q0[3], fma(q0[2], q0[2], q0[1] * q0[1]));
+    const double Ec2 = KNOWN ? Ec2_known : Ec * Ec;
+    const double F2c = KNOWN ? F2c_known : fma(q0[3], q0[3], fma(q0[2], q0[2], q0[1] * q0[1]));
     const double invEc = KNOWN ? invEc_known : frcp(Ec);
     if (want_lo) {
 #pragma unroll
