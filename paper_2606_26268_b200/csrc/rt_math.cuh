@@ -56,15 +56,14 @@ __device__ __forceinline__ void fsqrt_rsqrt(double x, double& s, double& rs) {
     rs = h + h;
 }
 
-// sqrt(x) alone (7 fp64 ops); x must be > 0 (callers clamp at a tiny positive number).
+// sqrt(x) alone (6 fp64 ops): one third-order step, no residual step (<= ~1 ulp; exactness for perfect squares is
+// not needed where this is used: zeta and the CFL rate); x must be > 0 (callers clamp at a tiny positive number).
 __device__ __forceinline__ double fsqrt(double x) {
-    double y = rsqrt_seed(x);
-    double g = x * y, h = 0.5 * y;
-    double t = fma(-h, g, 0.5);
-    g = fma(g, t, g);
-    h = fma(h, t, h);
-    double d = fma(-g, g, x);
-    return fma(d, h, g);
+    const double y = rsqrt_seed(x);
+    const double g = x * y, h = 0.5 * y;
+    const double t = fma(-h, g, 0.5);
+    const double p = fma(1.5 * t, t, t);
+    return fma(g, p, g);
 }
 
 __device__ __forceinline__ double dmin(double a, double b) { return a < b ? a : b; }
