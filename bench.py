@@ -36,8 +36,8 @@ FP64_PEAK_TINST = 148 * 64 * 1.965e9 / 1e12
 # Algorithmic fp64-pipe instructions (DFMA/DMUL/DADD/DSETP) per cell-update of k_substep_fused: ncu's executed count of
 # the committed capture (profiles/r1_ncu_full_fused.md) x the useful-lane fraction of the launch (30 of 32 lanes along
 # x1 and the ragged last tile, edge-row extras, segment ends) -- derivation in DESIGN.md Sect. 5.
-FUSED_FP64_PER_CELL = {"C4": 0.5 * (710.0 + 594.0),   # HLL / GLF alternate
-                       "C5": 755.0}                    # HLL, spherical (opacity tables are evaluated in the pre-pass)
+FUSED_FP64_PER_CELL = {"C4": 0.5 * (692.0 + 588.0),   # HLL / GLF alternate
+                       "C5": 741.0}                    # HLL, spherical (opacity tables are evaluated in the pre-pass)
 
 
 # Algorithmic bytes per interior cell and launch: 8 B x (fields read + written)
