@@ -113,7 +113,8 @@ int32_t rt_implicit_step_cfl(rt_grid* g, double dt, const double* rho, double* T
  * rt_cfl_dt_async).  No host synchronisation anywhere: a sequence of sub-steps can be enqueued back to back or
  * captured in a CUDA graph.  rho and T are required.  Same argument errors as the two halves.  On 3-D grids the
  * whole sub-step is one fused kernel (rt_set_tuning) and step 1 fills the face-normal ghosts of U_in only: edge and
- * corner ghosts, which no stencil of the scheme reads, are left as they were. */
+ * corner ghosts, which no stencil of the scheme reads, are left as they were.  Handle-owned scratch (thick-limit and
+ * rho kappa_P arrays) is allocated on the first call: capture a graph after one eager call. */
 int32_t rt_substep(rt_grid* g, double* dt_device, double cfl, const double* rho, double* T,
                    double* const mom[3], double* const U_in[4], double* const U_out[4]);
 

@@ -716,11 +716,12 @@ static int fused_segment_length(const rt_grid* g, int tiles) {
     if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
     const double slots = 2.0 * nsm;
     // measured on B200 (C4): segments of 32-43 planes beat 64-128 by ~2.5 % (finer tail), shorter ones pay the two
-    // half-work planes at the segment ends; among lengths 28..44 take the best wave fill x end overhead
-    if (n3 <= 24) return n3;
-    int best = 32;
+    // half-work planes at the segment ends; among lengths 12..48 take the best wave fill x end overhead
+    if (n3 <= 12) return n3;
+    int best = n3 < 32 ? n3 : 32;
     double best_score = -1.0;
-    for (int len = 28; len <= 44 && len <= n3; ++len) {
+    // 12..48: small grids (C3: 80 tiles) need short segments to fill the machine, large ones are flat in this range
+    for (int len = 12; len <= 48 && len <= n3; ++len) {
         const int ns = (n3 + len - 1) / len;
         const double ctas = (double)tiles * ns;
         const double fill = ctas / (ceil(ctas / slots) * slots);                 // tail effect
