@@ -367,6 +367,44 @@ def test_implicit_step_cfl_equals_implicit_then_cfl(rt):
     assert g.cfl_dt(a.U, 0.4) == float(dtn.item())
 
 
+# ----------------------------------------------------------------------------- streams and CUDA graphs
+def test_substeps_on_a_side_stream_and_replayed_from_a_cuda_graph(rt):
+    """rt_substep enqueues on the stream given at rt_grid_create and never synchronises: (a) a grid created on a side
+    stream gives the same bits as one on the default stream; (b) two sub-steps captured into a CUDA graph (after one
+    eager pair, which allocates the handle's scratch) and replayed give the same bits as the eager calls."""
+    w = random_workload(W.CARTESIAN, (64, 20, 16), W.SOLVER_HLL, 1, seed=61, fmax=0.9)
+
+    def eager(nsub):
+        g = rt.grid_from_workload(w)
+        st, dtn, _ = rt.run_substeps_fused(g, w, nsub)
+        torch.cuda.synchronize()
+        return [t.clone() for t in st.U], st.T.clone(), float(dtn.item())
+
+    refU, refT, refdt = eager(4)
+
+    side = torch.cuda.Stream()
+    with torch.cuda.stream(side):
+        g = rt.grid_from_workload(w)                 # the handle's stream = the side stream
+        st = rt.DeviceState(g, w)
+        dt_dev = torch.zeros(1, dtype=torch.float64, device="cuda")
+        g.cfl_dt_async(st.U, w.cfl, dt_dev)
+        # eager pair: first use of the fused kernel allocates scratch and sets its attributes
+        g.substep(dt_dev, w.cfl, st.rho, st.T, st.mom, st.U, st.U2)
+        g.substep(dt_dev, w.cfl, st.rho, st.T, st.mom, st.U2, st.U)
+        side.synchronize()
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(graph, stream=side):
+            g.substep(dt_dev, w.cfl, st.rho, st.T, st.mom, st.U, st.U2)
+            g.substep(dt_dev, w.cfl, st.rho, st.T, st.mom, st.U2, st.U)
+        graph.replay()                               # sub-steps 3 and 4
+        side.synchronize()
+    torch.cuda.synchronize()
+    for q in range(4):
+        assert torch.equal(st.U[q], refU[q]), q
+    assert torch.equal(st.T, refT)
+    assert float(dt_dev.item()) == refdt
+
+
 # ----------------------------------------------------------------------------- RK2 (SURVEY 8(f) NEXT-1)
 @pytest.mark.parametrize("case", ["3d-fused", "3d-spherical-tables", "1d", "2d-cyl"])
 def test_rk2_step_matches_the_oracle_composition(rt, case):
