@@ -488,7 +488,18 @@ static int32_t launch_thick_limit(rt_grid* g, const double* rho, const double* T
     const GridDev& D = g->dev;
     if (!g->lim) RT_CUDA(g, cudaMalloc(&g->lim, (size_t)D.ntot * sizeof(double)));
     if (with_kp && !g->kpr) RT_CUDA(g, cudaMalloc(&g->kpr, (size_t)D.ntot * sizeof(double)));
-    const int bx = 128;
+    // block width (<= 128, a multiple of 32) that wastes the fewest lanes on a row of nt1 cells: 260 -> 96 (3 x 96 = 288)
+    int bx = 128;
+    {
+        long long best = -1;
+        for (int cand = 128; cand >= 64; cand -= 32) {
+            const long long lanes = (long long)((D.nt[0] + cand - 1) / cand) * cand;
+            if (best < 0 || lanes < best) {
+                best = lanes;
+                bx = cand;
+            }
+        }
+    }
     dim3 grid((D.nt[1] + kThickRows - 1) / kThickRows, D.nt[2]);
     {
         ProfScope ps(g, RT_K_THICK);
