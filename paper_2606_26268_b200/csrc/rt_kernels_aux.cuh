@@ -370,6 +370,7 @@ __global__ void __launch_bounds__(128) k_thick_limit(const __grid_constant__ Gri
         const double* __restrict__ rrow = rho + srow;
         const double* __restrict__ trow = T + srow;
         double* __restrict__ lrow = lim + jj * g.stride[1] + kk * g.stride[2];
+        double* __restrict__ krow = kpr ? kpr + jj * g.stride[1] + kk * g.stride[2] : nullptr;
         double l12[3];  // the x2 and x3 factors of the three cell lengths (0 for an inactive direction)
 #pragma unroll
         for (int d = 0; d < 3; ++d) l12[d] = g.gh[d] > 0 ? __ldg(g.len[d][1] + c1) * __ldg(g.len[d][2] + c2) : 0.0;
@@ -389,7 +390,7 @@ __global__ void __launch_bounds__(128) k_thick_limit(const __grid_constant__ Gri
                 chi = kR + opacity_eval_shared(oS, r, t, share, l);
                 if (kpr) kP = same_PR ? kR : opacity_eval_shared(oP, r, t, share, l);
             }
-            if (kpr) kpr[jj * g.stride[1] + kk * g.stride[2] + ii] = kP * r;
+            if (kpr) krow[ii] = kP * r;
             double dx = 0.0;
 #pragma unroll
             for (int d = 0; d < 3; ++d)
