@@ -35,7 +35,8 @@ extern "C" {
 enum { RT_OK = 0, RT_ERR_INVALID_ARG = 1, RT_ERR_BAD_STATE = 2, RT_ERR_CUDA = 3, RT_ERR_NOT_FINITE = 4 };
 enum { RT_CARTESIAN = 0, RT_CYLINDRICAL = 1 /* (R,phi,z) */, RT_SPHERICAL = 2 /* (r,theta,phi) */ };
 enum { RT_BC_PERIODIC = 0, RT_BC_OUTFLOW = 1, RT_BC_REFLECT = 2, RT_BC_FIXED = 3 /* ghosts left as the caller wrote them */ };
-enum { RT_SOLVER_HLL = 0, RT_SOLVER_GLF = 1 };
+enum { RT_SOLVER_HLL = 0, RT_SOLVER_GLF = 1 /* global bound alpha = chat */,
+       RT_SOLVER_RUSANOV = 2 /* local bound alpha = chat max |lambda_1,3| of the two face states (L150; R-G5) */ };
 enum { RT_OPAC_PLANCK = 0, RT_OPAC_ROSSELAND = 1, RT_OPAC_SCATTER = 2 };
 
 typedef struct rt_grid rt_grid; /* opaque */

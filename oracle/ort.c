@@ -130,7 +130,9 @@ static void physical_flux(const double U[4], int d, double chat, double flux[4])
  * S_L = chat min(lam1(U_L), lam1(U_R), 0), S_R = chat max(lam3(U_L), lam3(U_R), 0) (R-G6),
  * then Eq. 25-26: S_L = max(S_L, -lim), S_R = min(S_R, lim), lim = 4 chat/(3 tau) (R-G7).
  * den = S_R - S_L; den > 0 ? HLL formula : plain average (R-G8).
- * GLF: 1/2 (F_L + F_R) - 1/2 alpha (U_R - U_L), alpha = min(chat, lim). */
+ * GLF: 1/2 (F_L + F_R) - 1/2 alpha (U_R - U_L), alpha = min(chat, lim).
+ * Rusanov ("Lax-Friedrichs-Rusanov", L150; DESIGN R-G5): the same form with the LOCAL bound
+ * alpha = min(chat max(|lam1(U_L)|, |lam3(U_L)|, |lam1(U_R)|, |lam3(U_R)|), lim). */
 void ort_riemann_flux(const double UL[4], const double UR[4], int32_t d, double chat, int32_t solver,
                       double lim, double flux[4]) {
     double FL[4], FR[4];
@@ -144,6 +146,12 @@ void ort_riemann_flux(const double UL[4], const double UR[4], int32_t d, double 
     double lamL[3], lamR[3];
     ort_wave_speeds(UL[0], &UL[1], d, lamL);
     ort_wave_speeds(UR[0], &UR[1], d, lamR);
+    if (solver == ORT_SOLVER_RUSANOV) {
+        double alpha = fmax(fmax(fabs(lamL[0]), fabs(lamL[2])), fmax(fabs(lamR[0]), fabs(lamR[2]))) * chat;
+        if (alpha > lim) alpha = lim;
+        for (int q = 0; q < 4; ++q) flux[q] = 0.5 * (FL[q] + FR[q]) - 0.5 * alpha * (UR[q] - UL[q]);
+        return;
+    }
     double SL = fmin(fmin(lamL[0], lamR[0]), 0.0) * chat;
     double SR = fmax(fmax(lamL[2], lamR[2]), 0.0) * chat;
     if (SL < -lim) SL = -lim;
@@ -346,7 +354,7 @@ int32_t ort_set_params(ort_grid* g, const ort_params* p) {
     if (!g || !p) return ORT_ERR_INVALID_ARG;
     if (!(p->chat > 0.0) || !(p->c > 0.0) || !(p->a_R >= 0.0) || !(p->c_v > 0.0) || !(p->E_floor >= 0.0))
         return ORT_ERR_INVALID_ARG;
-    if (p->solver != ORT_SOLVER_HLL && p->solver != ORT_SOLVER_GLF) return ORT_ERR_INVALID_ARG;
+    if (p->solver != ORT_SOLVER_HLL && p->solver != ORT_SOLVER_GLF && p->solver != ORT_SOLVER_RUSANOV) return ORT_ERR_INVALID_ARG;
     g->par = *p;
     g->have_par = 1;
     return ORT_OK;

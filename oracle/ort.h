@@ -22,7 +22,7 @@ extern "C" {
 enum { ORT_OK = 0, ORT_ERR_INVALID_ARG = 1, ORT_ERR_BAD_STATE = 2 };
 enum { ORT_CARTESIAN = 0, ORT_CYLINDRICAL = 1 /* (R,phi,z) */, ORT_SPHERICAL = 2 /* (r,theta,phi) */ };
 enum { ORT_BC_PERIODIC = 0, ORT_BC_OUTFLOW = 1, ORT_BC_REFLECT = 2, ORT_BC_FIXED = 3 };
-enum { ORT_SOLVER_HLL = 0, ORT_SOLVER_GLF = 1 };
+enum { ORT_SOLVER_HLL = 0, ORT_SOLVER_GLF = 1, ORT_SOLVER_RUSANOV = 2 };
 enum { ORT_OPAC_PLANCK = 0, ORT_OPAC_ROSSELAND = 1, ORT_OPAC_SCATTER = 2 };
 
 typedef struct {

@@ -294,7 +294,8 @@ extern "C" int32_t rt_set_params(rt_grid* g, const rt_params* p) {
     if (!(p->chat > 0.0) || !(p->c > 0.0) || !(p->a_R >= 0.0) || !(p->c_v > 0.0) || !(p->E_floor >= 0.0) ||
         !isfinite(p->chat) || !isfinite(p->c) || !isfinite(p->a_R) || !isfinite(p->c_v) || !isfinite(p->E_floor))
         return fail(g, RT_ERR_INVALID_ARG, "rt_set_params: chat, c, c_v must be > 0 and a_R, E_floor >= 0");
-    if (p->solver != RT_SOLVER_HLL && p->solver != RT_SOLVER_GLF) return fail(g, RT_ERR_INVALID_ARG, "rt_set_params: unknown solver");
+    if (p->solver != RT_SOLVER_HLL && p->solver != RT_SOLVER_GLF && p->solver != RT_SOLVER_RUSANOV)
+        return fail(g, RT_ERR_INVALID_ARG, "rt_set_params: unknown solver");
     g->par = *p;
     g->have_par = 1;
     return RT_OK;
@@ -549,7 +550,8 @@ static int32_t explicit_impl(rt_grid* g, double dt, const double* dt_dev, const 
     a.dtc = dt * g->par.chat;
     a.dt_dev = dt_dev;
     a.chat = g->par.chat;
-    const bool hll = g->par.solver == RT_SOLVER_HLL;
+    a.rusanov = g->par.solver == RT_SOLVER_RUSANOV;
+    const bool hll = g->par.solver != RT_SOLVER_GLF;  // HLL and Rusanov need the wave speeds
     const bool curvi = D.geometry != RT_CARTESIAN;
     if (D.gh[0] == 0) {
         // no x1 sweep: start the accumulation from a copy of U^n (rare: grids with n1 == 1)
@@ -804,7 +806,7 @@ static int32_t fused_impl(rt_grid* g, double* dt_device, double cfl, const doubl
     a.use_tma = (g->fused_tma_off == 0 && fused_make_maps(g, a, thick ? 5 : 4, &maps)) ? 1 : 0;
     {
         ProfScope ps(g, RT_K_FUSED);
-        cudaError_t e = launch_fused(g, g->par.solver == RT_SOLVER_HLL, thick, D.geometry != RT_CARTESIAN, feedback, P, a, maps, grid, seglen);
+        cudaError_t e = launch_fused(g, g->par.solver != RT_SOLVER_GLF, thick, D.geometry != RT_CARTESIAN, feedback, P, a, maps, grid, seglen);
         if (e != cudaSuccess) return fail(g, RT_ERR_CUDA, "k_substep_fused attribute: %s", cudaGetErrorString(e));
     }
     RT_LAUNCH_CHECK(g);

@@ -158,6 +158,7 @@ __global__ void __launch_bounds__(FNT, FUSED_MINB)
     const int ic = min(max(i, 0), g.n[0] - 1), jc = min(j, g.n[1] - 1);
     const int o = (ly + 2) * FPW + lx + 1;  // this thread's cell inside a staged plane
     const bool tma = a.use_tma != 0;
+    const bool rus = HLL && par.solver == 2;  // RT_SOLVER_RUSANOV
     const double dt = a.im.dt_dev ? __ldg(a.im.dt_dev) : a.im.dt;
     const double dtc = dt * a.chat;
 
@@ -269,7 +270,7 @@ __global__ void __launch_bounds__(FNT, FUSED_MINB)
                 State L;
                 state_load<HLL, FNT>(zhi, tid, L);
                 const double limd = THICK ? dmax(pm[4 * FPS + o], pc[4 * FPS + o]) : kInf;
-                riemann<HLL>(L, lo, limd, flz);
+                riemann<HLL>(L, lo, limd, flz, rus);
                 if (CURVI) {
                     const double w = g.wf[2][c];
 #pragma unroll
@@ -339,7 +340,7 @@ __global__ void __launch_bounds__(FNT, FUSED_MINB)
             }
             double fl[4];
             const double limd = THICK ? dmax(pc[4 * FPS + o - 1], pc[4 * FPS + o]) : kInf;
-            riemann<HLL>(L, lo, limd, fl);
+            riemann<HLL>(L, lo, limd, fl, rus);
             if (CURVI) {
 #pragma unroll
                 for (int q = 0; q < 4; ++q) fl[q] *= wx;
@@ -398,7 +399,7 @@ __global__ void __launch_bounds__(FNT, FUSED_MINB)
                 cell_faces<1, HLL>(qa, dma, dpa, true, false, loa, hia);
                 const double limd = THICK ? dmax(pc[4 * FPS + o], pc[4 * FPS + o + FPW]) : kInf;
                 double fup[4];
-                riemann<HLL>(hi, loa, limd, fup);
+                riemann<HLL>(hi, loa, limd, fup, rus);
 #pragma unroll
                 for (int q = 0; q < 4; ++q) yex[q * FNT + tid] = CURVI ? fup[q] * wyhi : fup[q];
             }
@@ -423,7 +424,7 @@ __global__ void __launch_bounds__(FNT, FUSED_MINB)
             }
             const double limd = THICK ? dmax(pc[4 * FPS + o - FPW], pc[4 * FPS + o]) : kInf;
             double fly[4];
-            riemann<HLL>(L, ylo, limd, fly);
+            riemann<HLL>(L, ylo, limd, fly, rus);
             const double cy = ky * g.cg[1][2][c];
 #pragma unroll
             for (int q = 0; q < 4; ++q) {

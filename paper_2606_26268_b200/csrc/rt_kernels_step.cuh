@@ -22,6 +22,7 @@ struct SweepArgs {
     double dtc;         // dt * chat (host-supplied dt)
     const double* dt_dev;  // device-resident dt (rt_substep) or nullptr; then dt * chat = *dt_dev * chat
     double chat;
+    int rusanov;  // RT_SOLVER_RUSANOV (the HLL instantiation computes the wave speeds it needs)
 };
 
 __device__ __forceinline__ double sweep_dtc(const SweepArgs& a) { return a.dt_dev ? __ldg(a.dt_dev) * a.chat : a.dtc; }
@@ -78,7 +79,7 @@ __global__ void __launch_bounds__(128) k_sweep_x(const __grid_constant__ GridDev
         L.lp = __shfl_up_sync(0xffffffffu, hi.lp, 1);
     }
     double fl[4];
-    riemann<HLL>(L, lo, limd, fl);
+    riemann<HLL>(L, lo, limd, fl, a.rusanov != 0);
     if (CURVI) {
         const double w = g.wf[0][ic < 0 ? 0 : ic];
 #pragma unroll
@@ -176,7 +177,7 @@ __global__ void __launch_bounds__(128) k_sweep_march(const __grid_constant__ Gri
         cell_faces<D, HLL>(qc, dm, dp, c >= ca, c < cb, lo, hi);
         if (c >= ca) {
             double fl[4];
-            riemann<HLL>(hiPrev, lo, THICK ? dmax(limp, limc) : kInf, fl);
+            riemann<HLL>(hiPrev, lo, THICK ? dmax(limp, limc) : kInf, fl, a.rusanov != 0);
             if (CURVI) {
                 const double w = wfd[c];
 #pragma unroll

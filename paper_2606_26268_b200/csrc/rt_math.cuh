@@ -150,8 +150,10 @@ __device__ __forceinline__ void fpreserve(State& st, const double Uc[4], double 
 
 // Riemann flux (L150; R-G5, G6, G8) divided by chat, from left state L and right state R.
 // limd = 4/(3 tau_face) (Eq. 25-26 in units of chat; +inf when the thick limit is off).
+// rusanov (launch-uniform, HLL instantiation only): the local Lax-Friedrichs bound alpha = max |lambda_{1,3}| of the
+// two states, clamped by limd: S_R = -S_L = alpha turns the two-wave formula into 1/2(F_L+F_R) - 1/2 alpha (U_R-U_L).
 template <bool HLL>
-__device__ __forceinline__ void riemann(const State& L, const State& R, double limd, double flux[4]) {
+__device__ __forceinline__ void riemann(const State& L, const State& R, double limd, double flux[4], bool rusanov = false) {
     double sR, sL;
     if (HLL) {
         // S_L = min(lm_L, lm_R, 0), S_R = max(lp_L, lp_R, 0) (R-G6), clamped by -+limd (Eq. 25-26), then kept off zero
@@ -159,6 +161,10 @@ __device__ __forceinline__ void riemann(const State& L, const State& R, double l
         // comparison against 0 is not spelled out.
         sL = dmin(L.lm, R.lm);
         sR = dmax(L.lp, R.lp);
+        if (rusanov) {
+            sR = dmax(-sL, sR);
+            sL = -sR;
+        }
         sL = dmax(sL, -limd);
         sR = dmin(sR, limd);
         sL = dmin(sL, -kTinySpeed);

@@ -16,7 +16,7 @@ from . import build as _build
 
 CARTESIAN, CYLINDRICAL, SPHERICAL = 0, 1, 2
 BC_PERIODIC, BC_OUTFLOW, BC_REFLECT, BC_FIXED = 0, 1, 2, 3
-SOLVER_HLL, SOLVER_GLF = 0, 1
+SOLVER_HLL, SOLVER_GLF, SOLVER_RUSANOV = 0, 1, 2
 OPAC_PLANCK, OPAC_ROSSELAND, OPAC_SCATTER = 0, 1, 2
 OK, ERR_INVALID_ARG, ERR_BAD_STATE, ERR_CUDA, ERR_NOT_FINITE = 0, 1, 2, 3, 4
 NGHOST = 2

@@ -156,7 +156,7 @@ def random_workload(geometry, n, solver, thick, seed, fmax=1.0, bc=None, feedbac
 # sizes span several tiles of every kernel and leave ragged tails: the x1 sweep owns 30 cells per
 # warp, the marching sweeps 128 x 32 (i x march), the per-cell kernels 128 cells per block
 @pytest.mark.parametrize("geometry", [W.CARTESIAN, W.CYLINDRICAL, W.SPHERICAL])
-@pytest.mark.parametrize("solver", [W.SOLVER_HLL, W.SOLVER_GLF])
+@pytest.mark.parametrize("solver", [W.SOLVER_HLL, W.SOLVER_GLF, W.SOLVER_RUSANOV])
 @pytest.mark.parametrize("thick", [0, 1])
 def test_one_substep_random_states_3d(rt, geometry, solver, thick):
     w = random_workload(geometry, (141, 37, 35), solver, thick, seed=100 + 10 * geometry + 2 * solver + thick)
@@ -167,7 +167,7 @@ def test_one_substep_random_states_3d(rt, geometry, solver, thick):
 
 @pytest.mark.parametrize("n", [(257, 1, 1), (5, 1, 1), (2, 2, 2), (1, 40, 1), (1, 9, 33), (64, 1, 7), (31, 65, 1),
                                (300, 3, 2)])
-@pytest.mark.parametrize("solver", [W.SOLVER_HLL, W.SOLVER_GLF])
+@pytest.mark.parametrize("solver", [W.SOLVER_HLL, W.SOLVER_GLF, W.SOLVER_RUSANOV])
 def test_one_substep_degenerate_shapes(rt, n, solver):
     w = random_workload(W.CARTESIAN, n, solver, 1, seed=7 + sum(n))
     errs, counts, _ = run_both(rt, w, 1)
@@ -282,7 +282,7 @@ def test_uniform_state_is_preserved_on_the_gpu(rt):
 # and x2 and has an odd x1 pitch (planes staged by cp.async); the even-pitch shapes below go through TMA.
 # fused_seg = 12 cuts x3 into segments of 12 + 12 + 11, 0 = the library's own choice
 @pytest.mark.parametrize("geometry", [W.CARTESIAN, W.CYLINDRICAL, W.SPHERICAL])
-@pytest.mark.parametrize("solver", [W.SOLVER_HLL, W.SOLVER_GLF])
+@pytest.mark.parametrize("solver", [W.SOLVER_HLL, W.SOLVER_GLF, W.SOLVER_RUSANOV])
 @pytest.mark.parametrize("thick", [0, 1])
 def test_fused_kernel_one_substep_random_states(rt, geometry, solver, thick):
     w = random_workload(geometry, (141, 37, 35), solver, thick, seed=100 + 10 * geometry + 2 * solver + thick)

@@ -184,6 +184,40 @@ def test_hll_equals_glf_when_speeds_are_symmetric():
     assert a[1] == pytest.approx(0.5 * (1.0 / 3 + 1.0), rel=1e-14)
 
 
+def test_rusanov_is_local_lax_friedrichs():
+    """RT/ORT_SOLVER_RUSANOV (L150 "Lax-Friedrichs-Rusanov"; R-G5): 1/2(F_L+F_R) - 1/2 alpha (U_R-U_L) with the LOCAL
+    alpha = chat max |lambda_{1,3}| of the two states.  Pins: consistency; equals GLF when some |lambda| = 1 (a state
+    streaming along the face normal); equals HLL when the speeds are symmetric (f = 0 on both sides); never more
+    diffusive than GLF; alpha recovered from the flux equals max |lambda| of ort.wave_speeds; obeys the thick limit."""
+    chat = 3.0
+    rng = np.random.default_rng(5)
+    for E, F in random_states(40):
+        U = [E] + list(F)
+        for d in range(3):
+            assert np.allclose(ort.riemann_flux(U, U, d, chat, ort.SOLVER_RUSANOV), _phys_flux(U, d, chat), rtol=1e-14, atol=1e-15)
+    states = random_states(40)
+    for (EL, FL), (ER, FR) in zip(states[::2], states[1::2]):
+        UL, UR = [EL] + list(FL), [ER] + list(FR)
+        for d in range(3):
+            fr = np.array(ort.riemann_flux(UL, UR, d, chat, ort.SOLVER_RUSANOV))
+            fg = np.array(ort.riemann_flux(UL, UR, d, chat, ort.SOLVER_GLF))
+            avg = 0.5 * (np.array(_phys_flux(UL, d, chat)) + np.array(_phys_flux(UR, d, chat)))
+            dU = np.array(UR) - np.array(UL)
+            lam = [abs(v) for U in (UL, UR) for v in (ort.wave_speeds(U[0], U[1:], d)[0], ort.wave_speeds(U[0], U[1:], d)[2])]
+            alpha = chat * max(lam)
+            assert np.allclose(fr, avg - 0.5 * alpha * dU, rtol=1e-13, atol=1e-14)
+            assert np.all(np.abs(fr - avg) <= np.abs(fg - avg) + 1e-14)
+            lim = 0.3 * alpha                                  # thick limit below the local speed: alpha = lim
+            fl = np.array(ort.riemann_flux(UL, UR, d, chat, ort.SOLVER_RUSANOV, lim=lim))
+            assert np.allclose(fl, avg - 0.5 * lim * dU, rtol=1e-13, atol=1e-14)
+    # |lambda| = 1: a beam along +x on the left
+    UL, UR = [2.0, 2.0, 0.0, 0.0], [0.7, 0.1, -0.2, 0.05]
+    assert np.allclose(ort.riemann_flux(UL, UR, 0, chat, ort.SOLVER_RUSANOV), ort.riemann_flux(UL, UR, 0, chat, ort.SOLVER_GLF), rtol=1e-14)
+    # symmetric speeds: f = 0 on both sides -> HLL with S_R = -S_L = chat/sqrt(3) is the same formula
+    UL, UR = [1.3, 0.0, 0.0, 0.0], [0.4, 0.0, 0.0, 0.0]
+    assert np.allclose(ort.riemann_flux(UL, UR, 1, chat, ort.SOLVER_RUSANOV), ort.riemann_flux(UL, UR, 1, chat, ort.SOLVER_HLL), rtol=1e-14)
+
+
 def test_riemann_mirror_symmetry():
     for _ in range(50):
         (E1, F1), (E2, F2) = random_states(2)
