@@ -682,9 +682,9 @@ static bool fused_make_maps(const rt_grid* g, const FusedArgs& a, int narr, Fuse
     return true;
 }
 
-template <bool HLL, bool THICK, bool CURVI, bool FEEDBACK>
+template <bool HLL, bool THICK, bool CURVI, bool FEEDBACK, bool RUS = false>
 static cudaError_t launch_fused_t(rt_grid* g, const ParamsDev& P, const FusedArgs& a, const FusedMaps& maps, dim3 grid, int seglen) {
-    auto kern = k_substep_fused<HLL, THICK, CURVI, FEEDBACK>;
+    auto kern = k_substep_fused<HLL, THICK, CURVI, FEEDBACK, RUS>;
     static bool attr_done = false;
     if (!attr_done) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kFusedSmemBytes);
@@ -698,6 +698,20 @@ static cudaError_t launch_fused_t(rt_grid* g, const ParamsDev& P, const FusedArg
 static cudaError_t launch_fused(rt_grid* g, bool hll, bool thick, bool curvi, bool feedback, const ParamsDev& P,
                                 const FusedArgs& a, const FusedMaps& maps, dim3 grid, int seglen) {
     const int key = (hll ? 8 : 0) | (thick ? 4 : 0) | (curvi ? 2 : 0) | (feedback ? 1 : 0);
+    if (g->par.solver == RT_SOLVER_RUSANOV) {
+        switch (key & 7) {
+#define RT_FUSED_CASE(K, B, C_, D_) case K: return launch_fused_t<true, B, C_, D_, true>(g, P, a, maps, grid, seglen);
+            RT_FUSED_CASE(0, false, false, false)
+            RT_FUSED_CASE(1, false, false, true)
+            RT_FUSED_CASE(2, false, true, false)
+            RT_FUSED_CASE(3, false, true, true)
+            RT_FUSED_CASE(4, true, false, false)
+            RT_FUSED_CASE(5, true, false, true)
+            RT_FUSED_CASE(6, true, true, false)
+            default: return launch_fused_t<true, true, true, true, true>(g, P, a, maps, grid, seglen);
+#undef RT_FUSED_CASE
+        }
+    }
     switch (key) {
 #define RT_FUSED_CASE(K, A, B, C_, D_) case K: return launch_fused_t<A, B, C_, D_>(g, P, a, maps, grid, seglen);
         RT_FUSED_CASE(0, false, false, false, false)

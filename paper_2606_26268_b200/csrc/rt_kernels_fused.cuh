@@ -135,7 +135,8 @@ __device__ __forceinline__ void state_load(const double* buf, int t, State& s) {
 
 
 
-template <bool HLL, bool THICK, bool CURVI, bool FEEDBACK>
+// RUS (with HLL = true): RT_SOLVER_RUSANOV, compile-time so that the HLL faces do not pay for the test
+template <bool HLL, bool THICK, bool CURVI, bool FEEDBACK, bool RUS>
 __global__ void __launch_bounds__(FNT, FUSED_MINB)
     k_substep_fused(const __grid_constant__ GridDev g, const __grid_constant__ ParamsDev par, const __grid_constant__ OpacDev oP,
                     const __grid_constant__ OpacDev oR, const __grid_constant__ OpacDev oS, const __grid_constant__ FusedArgs a,
@@ -158,7 +159,7 @@ __global__ void __launch_bounds__(FNT, FUSED_MINB)
     const int ic = min(max(i, 0), g.n[0] - 1), jc = min(j, g.n[1] - 1);
     const int o = (ly + 2) * FPW + lx + 1;  // this thread's cell inside a staged plane
     const bool tma = a.use_tma != 0;
-    const bool rus = HLL && par.solver == 2;  // RT_SOLVER_RUSANOV
+    constexpr bool rus = HLL && RUS;
     const double dt = a.im.dt_dev ? __ldg(a.im.dt_dev) : a.im.dt;
     const double dtc = dt * a.chat;
 

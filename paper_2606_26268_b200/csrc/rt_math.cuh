@@ -161,9 +161,10 @@ __device__ __forceinline__ void riemann(const State& L, const State& R, double l
         // comparison against 0 is not spelled out.
         sL = dmin(L.lm, R.lm);
         sR = dmax(L.lp, R.lp);
-        if (rusanov) {
+        if (rusanov) {  // kept a real (uniform) branch: if-converted it costs every HLL face a compare and two selects
             sR = dmax(-sL, sR);
             sL = -sR;
+            asm volatile("");
         }
         sL = dmax(sL, -limd);
         sR = dmin(sR, limd);
