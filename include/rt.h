@@ -101,6 +101,11 @@ int32_t rt_explicit_step(rt_grid* g, double dt, const double* rho, const double*
 int32_t rt_implicit_step(rt_grid* g, double dt, const double* rho, double* T,
                          double* const mom[3], double* const U[4]);
 
+/* Irradiation (Sect. 2.9, Eq. 34-35): div_firr = DEVICE array (field layout, caller-owned, must stay valid)
+ * of the divergence of a user-defined irradiation flux; every later implicit half adds Q = -div_firr dt to S_1 of
+ * Eq. 33, i.e. to the coupled energy C_v T + (c/chat) E_r (Eq. 34).  NULL switches it off (the default). */
+int32_t rt_set_irradiation(rt_grid* g, const double* div_firr);
+
 /* rt_implicit_step with step 10 (L120; R-G15) fused behind it: the kernel that writes the updated state also
  * reduces the CFL rate of that state (warp shuffles + filtered atomicMax), and a one-thread kernel writes
  * *dt_next_device = cfl / max rate (DEVICE double): bit-identical to rt_cfl_dt_async on the updated U, without

@@ -39,6 +39,7 @@ struct ort_grid {
     double* table[3];
     int have_opac[3];
     long long n_floor, n_clip;
+    const double* div_firr; /* caller-owned, ghosted layout, or NULL (Sect. 2.9) */
 };
 
 /* ------------------------------------------------------------------------------------------ */
@@ -207,9 +208,13 @@ double ort_opacity_eval(const ort_opacity* o, double rho, double T) {
  *   E'  = [E (C_v + 4 g a_R T^3) + g_r C_v a_R T^4] / det,
  *   T'  = [(1 + g_r) C_v T + 3 g a_R T^4 + g E] / det,
  * with g_r = dt chat kappa_P rho (gamma_abs,red), g = dt c kappa_P rho (gamma_abs), C_v = rho c_v.
- * Eq. 30 (L198): F' = F / (1 + dt chat chi rho).  Eq. 28 (L183): m' = m - (F' - F)/chat. */
+ * Eq. 30 (L198): F' = F / (1 + dt chat chi rho).  Eq. 28 (L183): m' = m - (F' - F)/chat.
+ * Irradiation (Sect. 2.9, Eq. 34-35): Q = -div F_irr dt is added to S_1 = C_v T + 3 g a_R T^4 of Eq. 33;
+ * with S_0 = E - 3 g_r a_R T^4 the analytic inverse reads
+ *   E' = [S_0 (C_v + 4 g a_R T^3) + 4 g_r a_R T^3 S_1] / det,   T' = [g S_0 + (1 + g_r) S_1] / det,
+ * which is the form above for Q = 0; it is evaluated as that form plus the two Q terms. */
 void ort_implicit_cell(const ort_params* p, double dt, double rho, double kappaP, double chi,
-                       double* E, double F[3], double* T, double* mom) {
+                       double* E, double F[3], double* T, double* mom, double Q) {
     double T0 = *T, E0 = *E;
     double gr = dt * p->chat * kappaP * rho;
     double g = dt * p->c * kappaP * rho;
@@ -219,6 +224,10 @@ void ort_implicit_cell(const ort_params* p, double dt, double rho, double kappaP
     double det = Cv * (1.0 + gr) + 4.0 * g * aT3;
     *E = (E0 * (Cv + 4.0 * g * aT3) + gr * Cv * aT4) / det;
     *T = ((1.0 + gr) * Cv * T0 + 3.0 * g * aT4 + g * E0) / det;
+    if (Q != 0.0) {
+        *E += 4.0 * gr * aT3 * Q / det;
+        *T += (1.0 + gr) * Q / det;
+    }
     double damp = 1.0 + dt * p->chat * chi * rho;
     for (int q = 0; q < 3; ++q) {
         double Fn = F[q] / damp;
@@ -583,6 +592,13 @@ int32_t ort_explicit_step(ort_grid* g, double dt, const double* rho, const doubl
 /* ------------------------------------------------------------------------------------------ */
 /* step 8: floor / clip, opacities, implicit coupling                                          */
 /* ------------------------------------------------------------------------------------------ */
+/* Sect. 2.9: div F_irr per cell (host, ghosted layout, caller-owned; NULL switches irradiation off) */
+int32_t ort_set_irradiation(ort_grid* g, const double* div_firr) {
+    if (!g) return ORT_ERR_INVALID_ARG;
+    g->div_firr = div_firr;
+    return ORT_OK;
+}
+
 int32_t ort_implicit_step(ort_grid* g, double dt, const double* rho, double* T,
                           double* const mom[3], double* const U[4]) {
     if (!g || !U || !rho || !T) return ORT_ERR_INVALID_ARG;
@@ -612,7 +628,8 @@ int32_t ort_implicit_step(ort_grid* g, double dt, const double* rho, double* T,
                 double m[3] = {0, 0, 0};
                 if (feedback)
                     for (int q = 0; q < 3; ++q) m[q] = mom[q][id];
-                ort_implicit_cell(p, dt, rho[id], kP, chi, &E, F, &Tc, feedback ? m : NULL);
+                double Q = g->div_firr ? -g->div_firr[id] * dt : 0.0; /* Eq. 34-35 */
+                ort_implicit_cell(p, dt, rho[id], kP, chi, &E, F, &Tc, feedback ? m : NULL, Q);
                 U[0][id] = E; U[1][id] = F[0]; U[2][id] = F[1]; U[3][id] = F[2];
                 T[id] = Tc;
                 if (feedback)

@@ -84,8 +84,9 @@ void ort_riemann_flux(const double UL[4], const double UR[4], int32_t d, double 
                       double lim, double flux[4]);
 double ort_opacity_eval(const ort_opacity* o, double rho, double T);       /* L299, L375 */
 /* Eq. 29-33 L195-216 + Eq. 30: in/out E, F[3], T; optional mom[3] (may be NULL) */
+int32_t ort_set_irradiation(ort_grid* g, const double* div_firr);
 void ort_implicit_cell(const ort_params* p, double dt, double rho, double kappaP, double chi,
-                       double* E, double F[3], double* T, double* mom);
+                       double* E, double F[3], double* T, double* mom, double Q);
 
 #ifdef __cplusplus
 }

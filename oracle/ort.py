@@ -73,7 +73,9 @@ def lib():
         L.ort_riemann_flux.argtypes = [_dp, _dp, C.c_int32, C.c_double, C.c_int32, C.c_double, _dp]
         L.ort_implicit_cell.restype = None
         L.ort_implicit_cell.argtypes = [C.POINTER(Params), C.c_double, C.c_double, C.c_double, C.c_double,
-                                        _dp, _dp, _dp, _dp]
+                                        _dp, _dp, _dp, _dp, C.c_double]
+        L.ort_set_irradiation.restype = C.c_int32
+        L.ort_set_irradiation.argtypes = [C.c_void_p, _dp]
         L.ort_grid_create.argtypes = [C.c_int32, C.POINTER(C.c_int32), C.c_int32, _dp, _dp, _dp,
                                       C.POINTER(C.c_int32), C.POINTER(C.c_void_p)]
         L.ort_grid_destroy.argtypes = [C.c_void_p]
@@ -180,11 +182,11 @@ def opacity_eval(o, rho, T):
     return lib().ort_opacity_eval(C.byref(o), float(rho), float(T))
 
 
-def implicit_cell(params, dt, rho, kappaP, chi, E, F, T, mom=None):
+def implicit_cell(params, dt, rho, kappaP, chi, E, F, T, mom=None, Q=0.0):
     Ea, Ta, Fa = np.array([E], dtype=np.float64), np.array([T], dtype=np.float64), _arr(F).copy()
     ma = _arr(mom).copy() if mom is not None else None
     lib().ort_implicit_cell(C.byref(params), float(dt), float(rho), float(kappaP), float(chi),
-                            _p(Ea), _p(Fa), _p(Ta), _p(ma))
+                            _p(Ea), _p(Fa), _p(Ta), _p(ma), float(Q))
     return Ea[0], Fa, Ta[0], ma
 
 
@@ -259,6 +261,15 @@ class Grid:
                                      _ptrs(U))
         if rc != 0:
             raise ValueError("ort_implicit_step failed with status %d" % rc)
+
+    def set_irradiation(self, div_firr):
+        """div F_irr per cell (ghosted float64 array, kept alive by this object) or None (Sect. 2.9, Eq. 34-35)"""
+        if div_firr is not None:
+            _check64(div_firr)
+        self._div_firr = div_firr
+        rc = lib().ort_set_irradiation(self._h, _p(div_firr) if div_firr is not None else None)
+        if rc != 0:
+            raise ValueError("ort_set_irradiation failed with status %d" % rc)
 
     def cfl_dt(self, U, cfl):
         _check64(*U)

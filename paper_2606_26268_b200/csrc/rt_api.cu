@@ -22,6 +22,7 @@ struct rt_grid {
     double* lim;  // thick-limit pre-pass array, ntot doubles (lazily allocated)
     double* rk_save[4];  // rt_rk2_step: T^n, m^n (lazily allocated)
     double* rk_dt;       // rt_rk2_step: the dt each stage reads (and overwrites)
+    const double* divfirr;  // rt_set_irradiation: caller-owned device array or nullptr
     double* kpr;  // rho kappa_P per cell, written by the pre-pass of the fused sub-step (lazily allocated)
     CflScratch* scr;
     double* dt_dev;
@@ -155,6 +156,7 @@ extern "C" int32_t rt_grid_create(int32_t geometry, const int32_t n[3], int32_t 
     g->metric_buf = nullptr;
     g->lim = nullptr;
     g->kpr = nullptr;
+    g->divfirr = nullptr;
     for (int q = 0; q < 4; ++q) g->rk_save[q] = nullptr;
     g->rk_dt = nullptr;
     g->scr = nullptr;
@@ -606,6 +608,7 @@ static int32_t implicit_impl(rt_grid* g, double dt, const double* dt_dev, const 
     }
     a.ichat = 1.0 / g->par.chat;
     a.counters = g->counters;
+    a.divfirr = g->divfirr;
     ParamsDev P = {g->par.chat, g->par.c, g->par.a_R, g->par.c_v, g->par.E_floor, g->par.solver, g->par.thick_limit,
                    g->par.feedback_momentum};
     const int bx = D.n[0] >= 128 ? 128 : ((D.n[0] + 31) / 32) * 32;
@@ -629,6 +632,13 @@ static int32_t implicit_impl(rt_grid* g, double dt, const double* dt_dev, const 
         }
         RT_LAUNCH_CHECK(g);
     }
+    return RT_OK;
+}
+
+extern "C" int32_t rt_set_irradiation(rt_grid* g, const double* div_firr) {
+    if (!g) return RT_ERR_INVALID_ARG;
+    if (div_firr && !aligned8(div_firr)) return fail(g, RT_ERR_INVALID_ARG, "rt_set_irradiation: misaligned pointer");
+    g->divfirr = div_firr;
     return RT_OK;
 }
 
@@ -810,6 +820,7 @@ static int32_t fused_impl(rt_grid* g, double* dt_device, double cfl, const doubl
     }
     a.im.ichat = 1.0 / g->par.chat;
     a.im.counters = g->counters;
+    a.im.divfirr = g->divfirr;
     ParamsDev P = {g->par.chat, g->par.c, g->par.a_R, g->par.c_v, g->par.E_floor, g->par.solver, g->par.thick_limit,
                    g->par.feedback_momentum};
     const int tx = (D.n[0] + FTX - 1) / FTX, ty = (D.n[1] + FTY - 1) / FTY;

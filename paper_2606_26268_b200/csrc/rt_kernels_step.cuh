@@ -223,6 +223,7 @@ struct ImplicitArgs {
     OpacSet os;   // shared log10 inputs of the table opacities
     double ichat; // 1 / chat
     unsigned long long* counters;  // [0] floor activations, [1] clip activations
+    const double* divfirr;         // div F_irr per cell (Sect. 2.9, Eq. 34-35) or nullptr
 };
 
 // CFL = true additionally evaluates the step-10 rate (R-G15) of the UPDATED state of each cell and folds it
@@ -240,6 +241,13 @@ __device__ __forceinline__ double implicit_cell(const GridDev& g, const ParamsDe
                                                 const double il[3] /* 1/dl_d of the cell (CFL only) */, double E, double F[3],
                                                 double rho, double T0, const double m[3], bool& floored, bool& clipped,
                                                 double rhochi_given = 0.0, double rhokp_given = 0.0) {
+    // irradiation (Eq. 34-35): Q = -div F_irr dt joins S_1 of Eq. 33; a launch-uniform branch
+    const bool irr = a.divfirr != nullptr;
+    double Q = 0.0;
+    if (irr) {
+        Q = -__ldg(a.divfirr + id) * dt;
+        asm volatile("");
+    }
     if (E < par.E_floor) {
         E = par.E_floor;
         floored = true;
@@ -271,8 +279,15 @@ __device__ __forceinline__ double implicit_cell(const GridDev& g, const ParamsDe
     const double aT4 = aT3 * T0;
     const double det = fma(Cv, 1.0 + gr, 4.0 * gg * aT3);
     const double idet = frcp(det);
-    const double En = fma(E, fma(4.0 * gg, aT3, Cv), gr * Cv * aT4) * idet;
-    const double Tn = fma((1.0 + gr) * Cv, T0, fma(3.0 * gg, aT4, gg * E)) * idet;
+    double En_ = fma(E, fma(4.0 * gg, aT3, Cv), gr * Cv * aT4) * idet;
+    double Tn_ = fma((1.0 + gr) * Cv, T0, fma(3.0 * gg, aT4, gg * E)) * idet;
+    if (irr) {  // E' += 4 g_r a_R T^3 Q / det,  T' += (1 + g_r) Q / det
+        const double qd = Q * idet;
+        En_ = fma(4.0 * gr * aT3, qd, En_);
+        Tn_ = fma(1.0 + gr, qd, Tn_);
+        asm volatile("");
+    }
+    const double En = En_, Tn = Tn_;
     const double idamp = frcp(fma(dt * par.chat, rhochi, 1.0));
     a.U[0][id] = En;
     a.T[id] = Tn;

@@ -64,6 +64,7 @@ _SIGNATURES = {
                                          C.POINTER(C.c_void_p), C.c_double, C.c_void_p]),
     "rt_substep": (C.c_int32, [C.c_void_p, C.c_void_p, C.c_double, C.c_void_p, C.c_void_p, C.POINTER(C.c_void_p),
                                C.POINTER(C.c_void_p), C.POINTER(C.c_void_p)]),
+    "rt_set_irradiation": (C.c_int32, [C.c_void_p, C.c_void_p]),
     "rt_rk2_step": (C.c_int32, [C.c_void_p, C.c_void_p, C.c_double, C.c_void_p, C.c_void_p, C.POINTER(C.c_void_p),
                                 C.POINTER(C.c_void_p), C.POINTER(C.c_void_p), C.POINTER(C.c_void_p)]),
     "rt_cfl_dt": (C.c_int32, [C.c_void_p, C.POINTER(C.c_void_p), C.c_double, _dp]),
@@ -291,6 +292,15 @@ class Grid:
                               _ptr_array(mom) if mom is not None else None, _ptr_array(U_in), _ptr_array(U_out))
         if rc != OK:
             self._raise("rt_substep", rc)
+
+    def set_irradiation(self, div_firr):
+        """div F_irr per cell (CUDA float64 tensor in the field layout, kept alive by this object) or None"""
+        if div_firr is not None:
+            _check_field(div_firr, self.shape, "div_firr")
+        self._div_firr = div_firr
+        rc = lib().rt_set_irradiation(self._h, div_firr.data_ptr() if div_firr is not None else None)
+        if rc != OK:
+            self._raise("rt_set_irradiation", rc)
 
     def rk2_step(self, dt_device, cfl, rho, T, mom, U, W1, W2):
         _check_field(rho, self.shape, "rho")

@@ -367,6 +367,34 @@ def test_implicit_step_cfl_equals_implicit_then_cfl(rt):
     assert g.cfl_dt(a.U, 0.4) == float(dtn.item())
 
 
+# ----------------------------------------------------------------------------- irradiation
+@pytest.mark.parametrize("n,fused", [((70, 33, 12), True), ((70, 33, 12), False), ((300, 1, 1), False)])
+def test_irradiation_source_in_the_implicit_half(rt, n, fused):
+    """rt_set_irradiation: Q = -div F_irr dt joins S_1 of Eq. 33 (Eq. 34-35); 3 sub-steps against the oracle
+    with the same seeded div F_irr array, through the fused kernel and through rt_implicit_step"""
+    w = random_workload(W.CARTESIAN, n, W.SOLVER_HLL, 1, seed=71, fmax=0.9)
+    rng = np.random.default_rng(72)
+    div = -rng.uniform(0.0, 2.0, size=w.rho.shape) * w.rho * w.T        # heating of the order of the gas energy per unit time
+    og = ort.grid_from_workload(w)
+    og.set_irradiation(div)
+    refU, refT, refm, dts = ort.run_substeps(og, w, 3)
+    og.set_irradiation(None)
+    g = rt.grid_from_workload(w)
+    ddiv = g.to_device(div)
+    g.set_irradiation(ddiv)
+    if fused:
+        st, _, hist = rt.run_substeps_fused(g, w, 3)
+    else:
+        st, _ = rt.run_substeps(g, w, 3, dts=dts)
+    torch.cuda.synchronize()
+    errs = field_errors(w, to_host(st.U), refU, st.T.cpu().numpy(), refT, to_host(st.mom), refm)
+    assert_below(errs, 3 * TOL1, "irradiation")
+    # and it matters: without the source the temperature differs by far more than the gate
+    g2 = rt.grid_from_workload(w)
+    st2, _ = rt.run_substeps(g2, w, 3, dts=dts)
+    assert (st2.T - st.T).abs().max().item() > 1e-6
+
+
 # ----------------------------------------------------------------------------- streams and CUDA graphs
 def test_substeps_on_a_side_stream_and_replayed_from_a_cuda_graph(rt):
     """rt_substep enqueues on the stream given at rt_grid_create and never synchronises: (a) a grid created on a side

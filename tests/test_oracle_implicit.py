@@ -224,3 +224,46 @@ def test_rk2_composition_conserves_the_coupled_energy_and_keeps_a_uniform_state_
     for a in (U[0][it], T[it]):
         assert np.ptp(a) <= 1e-14 * np.abs(a).max()
     assert len(dts) == 5 and all(d > 0 for d in dts)
+
+
+# ----------------------------------------------------------------------------- irradiation (Sect. 2.9, Eq. 34-35)
+def test_irradiation_source_is_the_solution_of_eq33_with_eq35():
+    """Q = -div F_irr dt enters S_1 of Eq. 33 (Eq. 35).  Independent pin: the 2x2 system written out from
+    Eq. 29-32 with the linearised T^4 and solved by numpy.linalg.solve; plus Eq. 34: the coupled energy
+    C_v T + (c/chat) E grows by exactly Q, and Q = 0 changes nothing."""
+    rng = np.random.default_rng(12)
+    for _ in range(200):
+        chat, c = np.exp(rng.uniform(0, 3)), np.exp(rng.uniform(3, 6))
+        p = ort.make_params(chat=chat, c=c, a_R=np.exp(rng.uniform(-2, 2)), c_v=1.5)
+        dt, rho, kP = np.exp(rng.uniform(-4, 1)), np.exp(rng.uniform(-2, 2)), np.exp(rng.uniform(-3, 3))
+        E, T = np.exp(rng.uniform(-2, 2)), np.exp(rng.uniform(-1, 1))
+        Q = rng.uniform(-0.2, 2.0) * rho * 1.5 * T                     # up to twice the gas energy, either sign
+        gr, g, Cv, a = dt * chat * kP * rho, dt * c * kP * rho, rho * 1.5, p.a_R
+        M = np.array([[1 + gr, -4 * gr * a * T ** 3], [-g, Cv + 4 * g * a * T ** 3]])
+        S = np.array([E - 3 * gr * a * T ** 4, Cv * T + 3 * g * a * T ** 4 + Q])
+        En_ref, Tn_ref = np.linalg.solve(M, S)
+        En, _, Tn, _ = ort.implicit_cell(p, dt, rho, kP, 0.0, E, [0.0, 0.0, 0.0], T, Q=Q)
+        assert En == pytest.approx(En_ref, rel=1e-11) and Tn == pytest.approx(Tn_ref, rel=1e-11)
+        assert Cv * Tn + (c / chat) * En == pytest.approx(Cv * T + (c / chat) * E + Q, rel=1e-12)          # Eq. 34
+        E0, _, T0, _ = ort.implicit_cell(p, dt, rho, kP, 0.0, E, [0.0, 0.0, 0.0], T)
+        E1, _, T1, _ = ort.implicit_cell(p, dt, rho, kP, 0.0, E, [0.0, 0.0, 0.0], T, Q=0.0)
+        assert (E0, T0) == (E1, T1)
+
+
+def test_irradiation_array_reaches_the_grid_level_implicit_step():
+    import rt_workloads as W
+    w = W.c1b()
+    g = ort.grid_from_workload(w)
+    it = g.interior
+    p = w.params
+    div = np.zeros(g.shape)
+    div[it] = -0.3 * (1.0 + np.arange(w.n[0]))[None, None, :] / w.n[0]          # heating, growing along x1
+    U = [a.copy() for a in w.U]
+    T = w.T.copy()
+    tot0 = w.rho[it] * p["c_v"] * T[it] + (p["c"] / p["chat"]) * U[0][it]
+    dt = 0.01
+    g.set_irradiation(div)
+    g.implicit_step(dt, w.rho, T, None, U)
+    g.set_irradiation(None)
+    tot1 = w.rho[it] * p["c_v"] * T[it] + (p["c"] / p["chat"]) * U[0][it]
+    assert np.allclose(tot1 - tot0, -div[it] * dt, rtol=1e-10, atol=1e-13)
