@@ -117,7 +117,7 @@ int32_t rt_implicit_step_cfl(rt_grid* g, double dt, const double* rho, double* T
  *   dt = *dt_device  ->  rt_explicit_step(dt, U_in -> U_out)  ->  rt_implicit_step_cfl(dt, U_out)  ->  *dt_device = next dt.
  * dt_device: DEVICE double, read by the kernels of this sub-step and overwritten at its end (seed it with
  * rt_cfl_dt_async).  No host synchronisation anywhere: a sequence of sub-steps can be enqueued back to back or
- * captured in a CUDA graph.  rho and T are required.  Same argument errors as the two halves.  On 3-D grids the
+ * captured in a CUDA graph.  rho and T are required.  Same argument errors as the two halves.  On 2-D and 3-D grids the
  * whole sub-step is one fused kernel (rt_set_tuning) and step 1 fills the face-normal ghosts of U_in only: edge and
  * corner ghosts, which no stencil of the scheme reads, are left as they were.  Handle-owned scratch (thick-limit and
  * rho kappa_P arrays) is allocated on the first call: capture a graph after one eager call. */
@@ -155,7 +155,7 @@ int32_t rt_set_profiling(rt_grid* g, int32_t on);
 int32_t rt_get_kernel_times(rt_grid* g, double ms[RT_NKERNEL_KINDS], int64_t launches[RT_NKERNEL_KINDS]);
 
 /* Launch-shape tuning knobs, not part of the method.  march_len: cells marched per thread along the sweep
- * direction in the x2/x3 sweeps (0 = library default).  fused_seg: rt_substep on 3-D grids runs ONE fused kernel
+ * direction in the x2/x3 sweeps (0 = library default).  fused_seg: rt_substep on 2-D / 3-D grids runs ONE fused kernel
  * (reconstruction ... implicit coupling + CFL rate in a single pass over U^n, x1-x2 tiles marching along x3);
  * 0 = on with an automatic x3 segment length, > 0 = that segment length, -1 = off (per-direction kernels). */
 int32_t rt_set_tuning(rt_grid* g, int32_t march_len, int32_t fused_seg);

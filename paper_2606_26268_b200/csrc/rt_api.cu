@@ -692,9 +692,9 @@ static bool fused_make_maps(const rt_grid* g, const FusedArgs& a, int narr, Fuse
     return true;
 }
 
-template <bool HLL, bool THICK, bool CURVI, bool FEEDBACK, bool RUS = false>
-static cudaError_t launch_fused_t(rt_grid* g, const ParamsDev& P, const FusedArgs& a, const FusedMaps& maps, dim3 grid, int seglen) {
-    auto kern = k_substep_fused<HLL, THICK, CURVI, FEEDBACK, RUS>;
+template <bool HLL, bool THICK, bool CURVI, bool FEEDBACK, bool RUS, bool HASZ>
+static cudaError_t launch_fused_z(rt_grid* g, const ParamsDev& P, const FusedArgs& a, const FusedMaps& maps, dim3 grid, int seglen) {
+    auto kern = k_substep_fused<HLL, THICK, CURVI, FEEDBACK, RUS, HASZ>;
     static bool attr_done = false;
     if (!attr_done) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kFusedSmemBytes);
@@ -703,6 +703,13 @@ static cudaError_t launch_fused_t(rt_grid* g, const ParamsDev& P, const FusedArg
     }
     kern<<<grid, dim3(32, FNY), kFusedSmemBytes, g->stream>>>(g->dev, P, g->opac[0], g->opac[1], g->opac[2], a, maps, seglen);
     return cudaSuccess;
+}
+
+// x3 active (3-D) or not (2-D)
+template <bool HLL, bool THICK, bool CURVI, bool FEEDBACK, bool RUS = false>
+static cudaError_t launch_fused_t(rt_grid* g, const ParamsDev& P, const FusedArgs& a, const FusedMaps& maps, dim3 grid, int seglen) {
+    return g->dev.gh[2] > 0 ? launch_fused_z<HLL, THICK, CURVI, FEEDBACK, RUS, true>(g, P, a, maps, grid, seglen)
+                            : launch_fused_z<HLL, THICK, CURVI, FEEDBACK, RUS, false>(g, P, a, maps, grid, seglen);
 }
 
 static cudaError_t launch_fused(rt_grid* g, bool hll, bool thick, bool curvi, bool feedback, const ParamsDev& P,
@@ -775,7 +782,7 @@ static int fused_segment_length(const rt_grid* g, int tiles) {
 
 static bool fused_eligible(const rt_grid* g) {
     const GridDev& D = g->dev;
-    return g->fused_seg >= 0 && D.gh[0] > 0 && D.gh[1] > 0 && D.gh[2] > 0 && D.ntot < (1LL << 31);  // 32-bit element offsets inside the kernel
+    return g->fused_seg >= 0 && D.gh[0] > 0 && D.gh[1] > 0 && D.ntot < (1LL << 31);  // 32-bit element offsets inside the kernel
 }
 
 static int32_t fused_impl(rt_grid* g, double* dt_device, double cfl, const double* rho, double* T, double* const mom[3],

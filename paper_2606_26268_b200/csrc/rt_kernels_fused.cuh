@@ -136,7 +136,9 @@ __device__ __forceinline__ void state_load(const double* buf, int t, State& s) {
 
 
 // RUS (with HLL = true): RT_SOLVER_RUSANOV, compile-time so that the HLL faces do not pay for the test
-template <bool HLL, bool THICK, bool CURVI, bool FEEDBACK, bool RUS>
+// HASZ = false: 2-D grids (n3 = 1, x3 inactive): one plane, no x3 phase; the march degenerates to the steps
+// c = -1 (nothing), 0 (X, Y), 1 (FIN) and the planes other than 0 are zero-filled by the TMA (clamped in the cp.async path).
+template <bool HLL, bool THICK, bool CURVI, bool FEEDBACK, bool RUS, bool HASZ>
 __global__ void __launch_bounds__(FNT, FUSED_MINB)
     k_substep_fused(const __grid_constant__ GridDev g, const __grid_constant__ ParamsDev par, const __grid_constant__ OpacDev oP,
                     const __grid_constant__ OpacDev oR, const __grid_constant__ OpacDev oS, const __grid_constant__ FusedArgs a,
@@ -184,7 +186,7 @@ __global__ void __launch_bounds__(FNT, FUSED_MINB)
                 for (int arr = 0; arr < NA; ++arr) tma_load_3d(dst + arr * FPS, &maps.m[arr], i0, j0, cc + g.gh[2], mbar + slot);
             }
         } else {
-            const long long zoff = (long long)(cc + g.gh[2]) * g.stride[2];
+            const long long zoff = (long long)min(max(cc + g.gh[2], 0), g.nt[2] - 1) * g.stride[2];
             for (int e = tid; e < NA * FPHW; e += FNT) {
                 const int arr = e / FPHW, r = e - arr * FPHW;
                 const int row = r / FPW, col = r - row * FPW;
@@ -198,15 +200,19 @@ __global__ void __launch_bounds__(FNT, FUSED_MINB)
     auto wait_plane = [&](int p) {
         if (tma) mbar_wait(mbar + ((p + 4) & 3), (unsigned)(((p - ka + 2) >> 2) & 1));
     };
-    load_plane(ka - 2);
-    load_plane(ka - 1);
-    load_plane(ka);
-    wait_plane(ka - 2);
-    wait_plane(ka - 1);
+    if (HASZ) {
+        load_plane(ka - 2);
+        load_plane(ka - 1);
+        load_plane(ka);
+        wait_plane(ka - 2);
+        wait_plane(ka - 1);
+    } else {
+        load_plane(0);  // the only plane of a 2-D grid; it is waited for at the top of step 0
+    }
 
     const double kx = dtc * g.cg[0][0][ic] * g.cg[0][1][jc];
     const double ky = dtc * g.cg[1][0][ic] * g.cg[1][1][jc];
-    const double kz = dtc * g.cg[2][0][ic] * g.cg[2][1][jc];
+    const double kz = HASZ ? dtc * g.cg[2][0][ic] * g.cg[2][1][jc] : 0.0;
     double wx = 1.0, wylo = 1.0, wyhi = 1.0;  // face-area weights of this cell's lower x1 face, lower / upper x2 faces
     if (CURVI) {
         wx = g.wf[0][min(max(i, 0), g.n[0])];
@@ -217,7 +223,7 @@ __global__ void __launch_bounds__(FNT, FUSED_MINB)
     const int zstride = (int)g.stride[2];
     double ilxy[3];  // x1-x2 part of 1/dl_d (CFL)
 #pragma unroll
-    for (int d = 0; d < 3; ++d) ilxy[d] = g.ilen[d][0][ic] * g.ilen[d][1][jc];
+    for (int d = 0; d < 3; ++d) ilxy[d] = (d < 2 || HASZ) ? g.ilen[d][0][ic] * g.ilen[d][1][jc] : 0.0;
 
     double acc[4] = {0.0, 0.0, 0.0, 0.0};  // U^n - dt/V ([AF]_x + [AF]_y) + dt S_geo of the previous plane's cell,
                                            // still missing the flux through its upper x2 face (held by the row above)
@@ -226,10 +232,12 @@ __global__ void __launch_bounds__(FNT, FUSED_MINB)
     double rate = 0.0;
 
 #pragma unroll 1
-    for (int c = ka - 1; c <= kb; ++c) {
-        if (tma) wait_plane(c + 1); else cp_async_wait_all();
+    for (int c = HASZ ? ka - 1 : 0; c <= kb; ++c) {
+        if (HASZ || c == 0) {
+            if (tma) wait_plane(HASZ ? c + 1 : 0); else cp_async_wait_all();
+        }
         __syncthreads();  // plane c+1 visible to all; every warp is done with step c-1
-        if (c + 2 <= kb + 1) load_plane(c + 2);
+        if (HASZ && c + 2 <= kb + 1) load_plane(c + 2);
         const double* pc = planes + ((c + 4) & 3) * (FNARR * FPS);
         if (writer && c < kb) {  // inputs of the implicit half of cell c, needed one step from now
             const int idn = id0 + c * zstride;
@@ -258,16 +266,16 @@ __global__ void __launch_bounds__(FNT, FUSED_MINB)
 #pragma unroll
             for (int q = 0; q < 4; ++q) {
                 q0[q] = pc[q * FPS + o];
-                dm[q] = q0[q] - pm[q * FPS + o];
-                dp[q] = pp[q * FPS + o] - q0[q];
+                dm[q] = HASZ ? q0[q] - pm[q * FPS + o] : 0.0;
+                dp[q] = HASZ ? pp[q * FPS + o] - q0[q] : 0.0;
             }
             State lo, hi;
             invEc = frcp(q0[0]);  // 1/E_c, E_c^2, |F_c|^2: shared by the three directions of this cell
             Ec2 = q0[0] * q0[0];
             F2c = fma(q0[3], q0[3], fma(q0[2], q0[2], q0[1] * q0[1]));
-            cell_faces<2, HLL, true>(q0, dm, dp, true, true, lo, hi, invEc, Ec2, F2c);  // both always: one basic block, two independent chains
+            if (HASZ) cell_faces<2, HLL, true>(q0, dm, dp, true, true, lo, hi, invEc, Ec2, F2c);  // both always: one basic block, two independent chains
             double flz[4] = {0.0, 0.0, 0.0, 0.0};
-            if (c >= ka) {
+            if (HASZ && c >= ka) {
                 State L;
                 state_load<HLL, FNT>(zhi, tid, L);
                 const double limd = THICK ? dmax(pm[4 * FPS + o], pc[4 * FPS + o]) : kInf;
@@ -278,10 +286,10 @@ __global__ void __launch_bounds__(FNT, FUSED_MINB)
                     for (int q = 0; q < 4; ++q) flz[q] *= w;
                 }
             }
-            state_store<HLL, FNT>(zhi, tid, hi);
+            if (HASZ) state_store<HLL, FNT>(zhi, tid, hi);
             // ------------------------------------------------------------ FIN (cell c-1): a8-a11
             if (c > ka) {
-                const double coef = kz * g.cg[2][2][c - 1];
+                const double coef = HASZ ? kz * g.cg[2][2][c - 1] : 0.0;
                 const double cyp = ky * g.cg[1][2][c - 1];
                 double U4[4];
 #pragma unroll
@@ -295,14 +303,16 @@ __global__ void __launch_bounds__(FNT, FUSED_MINB)
                         for (int q = 0; q < 3; ++q) m[q] = a.im.mom[q][id];
                     }
                     double F[3] = {U4[1], U4[2], U4[3]};
-                    const double il[3] = {ilxy[0] * g.ilen[0][2][c - 1], ilxy[1] * g.ilen[1][2][c - 1], ilxy[2] * g.ilen[2][2][c - 1]};
+                    const double il[3] = {ilxy[0] * g.ilen[0][2][c - 1], ilxy[1] * g.ilen[1][2][c - 1],
+                                          HASZ ? ilxy[2] * g.ilen[2][2][c - 1] : 0.0};
                     bool floored = false, clipped = false;
                     // rho chi of the cell from the thick-limit array of this sub-step: lim = 4/(3 rho chi dx), dx = the
                     // cell's largest extent = 1/min_d(1/dl_d); lim = +inf stands for rho chi dx <= 1e-100
                     double rhochi = 0.0;
                     if (THICK) {
                         const double lim = pm[4 * FPS + o];
-                        rhochi = lim > 1.0e300 ? 0.0 : (4.0 / 3.0) * dmin(il[0], dmin(il[1], il[2])) * frcp(lim);
+                        const double ilmin = HASZ ? dmin(il[0], dmin(il[1], il[2])) : dmin(il[0], il[1]);  // active directions
+                        rhochi = lim > 1.0e300 ? 0.0 : (4.0 / 3.0) * ilmin * frcp(lim);
                     }
                     const double r = implicit_cell<FEEDBACK, true, THICK>(g, par, oP, oR, oS, a.im, dt, (long long)id, il, U4[0], F, rho,
                                                                           T0, m, floored, clipped, rhochi, kpr_f);

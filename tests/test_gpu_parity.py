@@ -64,7 +64,11 @@ def run_both(rt, w, nsub, dts=None, fused=False, fused_seg=0):
         g.set_tuning(fused_seg=fused_seg)
         st, _, hist = rt.run_substeps_fused(g, w, nsub)
         used = hist.cpu().numpy()
-        assert np.all(np.abs(used - np.array(dts)) <= (1e-12 if nsub <= 5 else 1e-9) * np.array(dts)), (used, dts)
+        # every dt comes from the device-side CFL reduction of the GPU's own state: round-off-level field differences
+        # feed back into it, amplified where the maximum sits on a state with f -> 1 (d lambda / d f ~ 1/sqrt(1 - f),
+        # DESIGN.md "Tolerances" (i)): 1e-12 over a few sub-steps, 1e-7 over long runs
+        rel = np.abs(used - np.array(dts)) / np.array(dts)
+        assert rel.max() <= (1e-12 if nsub <= 5 else 1e-7), (rel.max(), int(rel.argmax()))
     else:
         st, _ = rt.run_substeps(g, w, nsub, dts=dts)
     torch.cuda.synchronize()
@@ -300,6 +304,19 @@ def test_fused_kernel_small_and_ragged_shapes(rt, n):
     assert counts[0] == counts[1]
 
 
+@pytest.mark.parametrize("geometry,n", [(W.CARTESIAN, (31, 65, 1)), (W.CARTESIAN, (64, 20, 1)), (W.CYLINDRICAL, (40, 33, 1)),
+                                        (W.SPHERICAL, (45, 22, 1)), (W.CARTESIAN, (2, 2, 1)), (W.CARTESIAN, (300, 9, 1))])
+@pytest.mark.parametrize("solver", [W.SOLVER_HLL, W.SOLVER_GLF, W.SOLVER_RUSANOV])
+def test_fused_kernel_2d_grids(rt, geometry, n, solver):
+    """x3 inactive: the same kernel without its x3 phase (one staged plane); odd and even x1 pitches, ragged tiles"""
+    bc = (0, 0, 0, 0, 0, 0) if geometry == W.CARTESIAN else (2, 1, 1, 1, 1, 1)
+    for thick in (0, 1):
+        w = random_workload(geometry, n, solver, thick, seed=300 + sum(n) + solver, bc=bc, table=(geometry == W.SPHERICAL))
+        errs, counts, _ = run_both(rt, w, 2, fused=True)
+        assert_below(errs, 2 * TOL1, "fused kernel, 2-D %s thick %d" % (n, thick))
+        assert counts[0] == counts[1]
+
+
 def test_fused_kernel_tables_boundaries_no_feedback(rt):
     w = random_workload(W.SPHERICAL, (50, 34, 20), W.SOLVER_HLL, 1, seed=5, bc=(3, 1, 2, 1, 0, 0), table=True)
     errs, _, _ = run_both(rt, w, 1, fused=True, fused_seg=7)
@@ -484,16 +501,17 @@ def test_config1_pulse_and_equilibration_100_substeps(rt):
         assert counts[0] == counts[1]
 
 
-def test_config2_beam_shadow_reduced_and_full_width(rt):
+@pytest.mark.parametrize("fused", [False, True])
+def test_config2_beam_shadow_reduced_and_full_width(rt, fused):
     w = W.c2(n1=128, n2=128, nsub=300)
-    errs, counts, _ = run_both(rt, w, 300)
+    errs, counts, _ = run_both(rt, w, 300, fused=fused)
     assert_below(errs, TOL100, "C2 128^2, 300 sub-steps")
     # no floor-count comparison here: the vacuum cells sit exactly ON the floor value, so E* = floor -+ 1 ulp
     # flips the `E < E_floor` predicate without changing the floored result
     w = W.c2()                                  # full 512^2
-    errs1, _, _ = run_both(rt, w, 1)
+    errs1, _, _ = run_both(rt, w, 1, fused=fused)
     assert_below(errs1, TOL1, "C2 512^2 1 sub-step")
-    errs, counts, _ = run_both(rt, w, 100)
+    errs, counts, _ = run_both(rt, w, 100, fused=fused)
     assert_below(errs, TOL100, "C2 512^2 100 sub-steps")
     assert counts[0][1] == counts[1][1]
 
