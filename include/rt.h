@@ -159,6 +159,8 @@ int32_t rt_get_kernel_times(rt_grid* g, double ms[RT_NKERNEL_KINDS], int64_t lau
  * (reconstruction ... implicit coupling + CFL rate in a single pass over U^n, x1-x2 tiles marching along x3);
  * 0 = on with an automatic x3 segment length, > 0 = that segment length, -1 = off (per-direction kernels). */
 int32_t rt_set_tuning(rt_grid* g, int32_t march_len, int32_t fused_seg);
+/* Measurement aid: with RT_M1_NO_TMA=1 in the environment at rt_grid_create the fused kernel stages its planes by
+ * cp.async even where TMA could address them (the path arrays with an odd x1 pitch always take). */
 
 const char* rt_last_error(const rt_grid* g);
 

@@ -1,4 +1,5 @@
-// rt_kernels_fused.cuh — ONE kernel for the whole sub-step on 3-D grids (SURVEY.md Sect. 8(f) NEXT-1):
+// rt_kernels_fused.cuh — ONE kernel for the whole sub-step on 3-D (and, without its x3 phase, 2-D) grids
+// (SURVEY.md Sect. 8(f) NEXT-1):
 // steps 3-8 and the rate of step 10 in a single pass over U^n.
 //
 // Design (DESIGN.md Sect. 5 "Fused sub-step kernel").  A CTA of 32 x FTY threads owns an x1-x2 tile of
