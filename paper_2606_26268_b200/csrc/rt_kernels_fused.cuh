@@ -79,19 +79,27 @@ __device__ __forceinline__ void mbar_expect_tx(unsigned long long* bar, unsigned
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"((unsigned)__cvta_generic_to_shared(bar)), "r"(bytes)
                  : "memory");
 }
-__device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned parity) {
-    const unsigned b = (unsigned)__cvta_generic_to_shared(bar);
+__device__ __forceinline__ bool mbar_try_wait(unsigned bar_smem, unsigned parity) {
+    unsigned ok;
     asm volatile(
         "{\n"
         ".reg .pred p;\n"
-        "WAIT_%=:\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
-        "@p bra DONE_%=;\n"
-        "bra WAIT_%=;\n"
-        "DONE_%=:\n"
-        "}\n" ::"r"(b),
-        "r"(parity)
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+        "selp.u32 %0, 1, 0, p;\n"
+        "}\n"
+        : "=r"(ok)
+        : "r"(bar_smem), "r"(parity)
         : "memory");
+    return ok != 0;
+}
+// Wait for a phase of an mbarrier.  A bulk copy that never completes (a descriptor the hardware rejects) would spin
+// here for ever: after 2^24 failed tries (seconds) the kernel traps instead, and the next API call reports RT_ERR_CUDA.
+__device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned parity) {
+    const unsigned b = (unsigned)__cvta_generic_to_shared(bar);
+    unsigned spins = 0;
+    while (!mbar_try_wait(b, parity)) {
+        if (++spins > (1u << 24)) __trap();  // each failed try already waits a hardware time slice: seconds in total
+    }
 }
 __device__ __forceinline__ void tma_load_3d(double* smem_dst, const CUtensorMap* map, int x, int y, int z, unsigned long long* bar) {
     asm volatile(
