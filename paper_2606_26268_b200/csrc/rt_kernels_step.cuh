@@ -1,5 +1,7 @@
 // rt_kernels_step.cuh — the fused reconstruct -> f-fix -> closure -> Riemann -> divergence sweeps
 // (a2-a7) and the floor + opacity + implicit coupling kernel (a8-a10).  SURVEY.md Sect. 8(a).
+// These per-direction kernels serve rt_explicit_step / rt_implicit_step and 1-D grids; on 2-D / 3-D grids rt_substep
+// runs k_substep_fused (rt_kernels_fused.cuh), which shares implicit_cell() and the arithmetic of rt_math.cuh.
 //
 // Sweep design: face states, face fluxes and wave speeds never touch HBM.
 //  * x1 sweep: one warp owns 32 consecutive cells of one row; every lane builds both face states of
