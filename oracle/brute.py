@@ -45,9 +45,15 @@ def limited_slope(a, b, c):                      # van Leer (L132, R-G3)
     return 2.0 * lo * hi / (lo + hi) if lo * hi > 0.0 else 0.0
 
 
-def face_state(Um, U0, Up, sign):                # Eq. 17-21 (L128-146); sign = +1 upper face, -1 lower face
+def face_state(Um, U0, Up, sign, fix=0):         # Eq. 17-21 (L128-146); sign = +1 upper face, -1 lower face
     R = tuple(U0[q] + sign * 0.5 * limited_slope(Um[q], U0[q], Up[q]) for q in range(4))
     F2f = R[1] ** 2 + R[2] ** 2 + R[3] ** 2
+    if fix == 1:                                 # "PLUTO reconstruction" (L136): flat where ||R(F)|| > R(E)
+        return tuple(U0) if F2f > R[0] ** 2 else R
+    if fix == 2:                                 # Eq. 36-38 (L272-279): rescale R(F) onto ||F_f|| = R(E)
+        if F2f <= R[0] ** 2:
+            return R
+        return (R[0],) + tuple(R[q] * R[0] / math.sqrt(F2f) for q in (1, 2, 3))
     F2c = U0[1] ** 2 + U0[2] ** 2 + U0[3] ** 2
     if F2f <= R[0] ** 2 and F2f * U0[0] ** 2 > F2c * R[0] ** 2:
         return R
@@ -169,8 +175,9 @@ class Brute:
         e = tuple(1 if a == d else 0 for a in range(3))
         sh = lambda s: tuple(key[a] + s * e[a] for a in range(3))
         A_mm, A_m, A_0, A_p = (self.state(U, sh(s)) for s in (-2, -1, 0, 1))
-        UL = face_state(A_mm, A_m, A_0, +1.0)
-        UR = face_state(A_m, A_0, A_p, -1.0)
+        fix = self.p.get("face_fix", 0)
+        UL = face_state(A_mm, A_m, A_0, +1.0, fix)
+        UR = face_state(A_m, A_0, A_p, -1.0, fix)
         lim = math.inf
         if self.p["thick_limit"]:
             tf = min(self.tau(rho, T, sh(-1)), self.tau(rho, T, key))

@@ -40,6 +40,7 @@ struct ort_grid {
     int have_opac[3];
     long long n_floor, n_clip;
     const double* div_firr; /* caller-owned, ghosted layout, or NULL (Sect. 2.9) */
+    int face_fix;           /* ORT_FIX_* (zero-initialised: the f-preserving scheme of Eq. 19-21) */
 };
 
 /* ------------------------------------------------------------------------------------------ */
@@ -114,6 +115,32 @@ void ort_fpreserving_face(const double Uc[4], const double RU[4], double Uf[4]) 
     } else {
         double r = Ef / Ec;
         Uf[1] = Uc[1] * r; Uf[2] = Uc[2] * r; Uf[3] = Uc[3] * r;
+    }
+}
+
+/* The "PLUTO reconstruction scheme" as the paper states it (L136): flat reconstruction, E_f = E_c and
+ * F_f = F_c, whenever ||R(F)|| > R(E); the reconstructed values otherwise.  Squares compared, no division. */
+void ort_pluto_face(const double Uc[4], const double RU[4], double Uf[4]) {
+    double Ef = RU[0];
+    double F2f = RU[1] * RU[1] + RU[2] * RU[2] + RU[3] * RU[3];
+    if (F2f > Ef * Ef) {
+        for (int q = 0; q < 4; ++q) Uf[q] = Uc[q];
+    } else {
+        for (int q = 0; q < 4; ++q) Uf[q] = RU[q];
+    }
+}
+
+/* Eq. 36-38 (L272-279), the scheme of Fig. 5's first panel: E_f = R(E); F_f = R(F) while
+ * ||R(F)||/R(E) <= 1, otherwise R(F) rescaled to ||F_f|| = R(E) (direction kept). */
+void ort_clip_face(const double RU[4], double Uf[4]) {
+    double Ef = RU[0];
+    double F2f = RU[1] * RU[1] + RU[2] * RU[2] + RU[3] * RU[3];
+    Uf[0] = Ef;
+    if (F2f <= Ef * Ef) {
+        Uf[1] = RU[1]; Uf[2] = RU[2]; Uf[3] = RU[3];
+    } else {
+        double r = Ef / sqrt(F2f);
+        Uf[1] = RU[1] * r; Uf[2] = RU[2] * r; Uf[3] = RU[3] * r;
     }
 }
 
@@ -445,12 +472,12 @@ int32_t ort_fill_ghosts(ort_grid* g, double* const U[4]) {
 /* steps 3-7: explicit transport                                                               */
 /* ------------------------------------------------------------------------------------------ */
 
-/* steps 3+4 for one cell and one direction: PLM (Eq. 17-18) then the f-preserving fix (Eq. 19-21)
+/* steps 3+4 for one cell and one direction: PLM (Eq. 17-18) then the f-preserving fix (Eq. 19-21;
+ * or, on request, the flat fallback of L136 / the clip of Eq. 36-38: ort_set_face_fix)
  * for the cell's lower-face state (the RIGHT state of face i-1/2) and upper-face state (the LEFT
  * state of face i+1/2). */
 static void cell_face_states(const ort_grid* g, double* const U[4], long idx, long stride,
                              double Ulo[4], double Uhi[4]) {
-    (void)g;
     double Uc[4], Rlo[4], Rhi[4];
     for (int q = 0; q < 4; ++q) {
         double qm = U[q][idx - stride], q0 = U[q][idx], qp = U[q][idx + stride];
@@ -459,8 +486,16 @@ static void cell_face_states(const ort_grid* g, double* const U[4], long idx, lo
         Rlo[q] = q0 - 0.5 * slope;
         Rhi[q] = q0 + 0.5 * slope;
     }
-    ort_fpreserving_face(Uc, Rlo, Ulo);
-    ort_fpreserving_face(Uc, Rhi, Uhi);
+    if (g->face_fix == ORT_FIX_PLUTO) {
+        ort_pluto_face(Uc, Rlo, Ulo);
+        ort_pluto_face(Uc, Rhi, Uhi);
+    } else if (g->face_fix == ORT_FIX_CLIP) {
+        ort_clip_face(Rlo, Ulo);
+        ort_clip_face(Rhi, Uhi);
+    } else {
+        ort_fpreserving_face(Uc, Rlo, Ulo);
+        ort_fpreserving_face(Uc, Rhi, Uhi);
+    }
 }
 
 /* tau_cell = rho chi dx, dx = the cell's largest physical extent over active dimensions
@@ -592,6 +627,13 @@ int32_t ort_explicit_step(ort_grid* g, double dt, const double* rho, const doubl
 /* ------------------------------------------------------------------------------------------ */
 /* step 8: floor / clip, opacities, implicit coupling                                          */
 /* ------------------------------------------------------------------------------------------ */
+/* Sect. 2.5 / 3.2: which face fix the explicit step applies */
+int32_t ort_set_face_fix(ort_grid* g, int32_t mode) {
+    if (!g || mode < ORT_FIX_FPRESERVING || mode > ORT_FIX_CLIP) return ORT_ERR_INVALID_ARG;
+    g->face_fix = mode;
+    return ORT_OK;
+}
+
 /* Sect. 2.9: div F_irr per cell (host, ghosted layout, caller-owned; NULL switches irradiation off) */
 int32_t ort_set_irradiation(ort_grid* g, const double* div_firr) {
     if (!g) return ORT_ERR_INVALID_ARG;

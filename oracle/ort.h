@@ -24,6 +24,8 @@ enum { ORT_CARTESIAN = 0, ORT_CYLINDRICAL = 1 /* (R,phi,z) */, ORT_SPHERICAL = 2
 enum { ORT_BC_PERIODIC = 0, ORT_BC_OUTFLOW = 1, ORT_BC_REFLECT = 2, ORT_BC_FIXED = 3 };
 enum { ORT_SOLVER_HLL = 0, ORT_SOLVER_GLF = 1, ORT_SOLVER_RUSANOV = 2 };
 enum { ORT_OPAC_PLANCK = 0, ORT_OPAC_ROSSELAND = 1, ORT_OPAC_SCATTER = 2 };
+/* how f <= 1 is enforced on the reconstructed face states (Sect. 2.5, Sect. 3.2 Eq. 36-38) */
+enum { ORT_FIX_FPRESERVING = 0 /* Eq. 19-21 */, ORT_FIX_PLUTO = 1 /* flat fallback, L136 */, ORT_FIX_CLIP = 2 /* Eq. 36-38 */ };
 
 typedef struct {
     double chat;    /* reduced speed of light, PAPER.md:L179 (Sect. 2.7) */
@@ -79,6 +81,12 @@ void ort_wave_speeds(double E, const double F[3], int32_t d, double lam[3]); /* 
 double ort_vanleer_slope(double qm, double q0, double qp);                 /* L132 (R-G3) */
 /* Eq. 19-21: cell value Uc[4], reconstructed RU[4] -> face state Uf[4] */
 void ort_fpreserving_face(const double Uc[4], const double RU[4], double Uf[4]);
+/* "PLUTO reconstruction" L136: U_f = U_c (E and F) whenever ||R(F)|| > R(E), else U_f = R(U) */
+void ort_pluto_face(const double Uc[4], const double RU[4], double Uf[4]);
+/* Eq. 36-38: E_f = R(E); F_f = R(F) if ||R(F)|| <= R(E), else R(F) R(E)/||R(F)|| */
+void ort_clip_face(const double RU[4], double Uf[4]);
+/* which of the three the explicit step applies (default ORT_FIX_FPRESERVING) */
+int32_t ort_set_face_fix(ort_grid* g, int32_t mode);
 /* L150 (R-G5,G6,G8): face flux from the two face states; lim = 4 chat/(3 tau_face) or +inf */
 void ort_riemann_flux(const double UL[4], const double UR[4], int32_t d, double chat, int32_t solver,
                       double lim, double flux[4]);

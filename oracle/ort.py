@@ -19,6 +19,7 @@ _lib = None
 CARTESIAN, CYLINDRICAL, SPHERICAL = 0, 1, 2
 BC_PERIODIC, BC_OUTFLOW, BC_REFLECT, BC_FIXED = 0, 1, 2, 3
 SOLVER_HLL, SOLVER_GLF, SOLVER_RUSANOV = 0, 1, 2
+FIX_FPRESERVING, FIX_PLUTO, FIX_CLIP = 0, 1, 2
 OPAC_PLANCK, OPAC_ROSSELAND, OPAC_SCATTER = 0, 1, 2
 
 _dp = C.POINTER(C.c_double)
@@ -69,6 +70,12 @@ def lib():
         L.ort_wave_speeds.argtypes = [C.c_double, _dp, C.c_int32, _dp]
         L.ort_fpreserving_face.restype = None
         L.ort_fpreserving_face.argtypes = [_dp, _dp, _dp]
+        L.ort_pluto_face.restype = None
+        L.ort_pluto_face.argtypes = [_dp, _dp, _dp]
+        L.ort_clip_face.restype = None
+        L.ort_clip_face.argtypes = [_dp, _dp]
+        L.ort_set_face_fix.restype = C.c_int32
+        L.ort_set_face_fix.argtypes = [C.c_void_p, C.c_int32]
         L.ort_riemann_flux.restype = None
         L.ort_riemann_flux.argtypes = [_dp, _dp, C.c_int32, C.c_double, C.c_int32, C.c_double, _dp]
         L.ort_implicit_cell.restype = None
@@ -140,6 +147,20 @@ def fpreserving_face(Uc, RU):
     a, b = _arr(Uc), _arr(RU)
     out = np.empty(4)
     lib().ort_fpreserving_face(_p(a), _p(b), _p(out))
+    return out
+
+
+def pluto_face(Uc, RU):
+    a, b = _arr(Uc), _arr(RU)
+    out = np.empty(4)
+    lib().ort_pluto_face(_p(a), _p(b), _p(out))
+    return out
+
+
+def clip_face(RU):
+    b = _arr(RU)
+    out = np.empty(4)
+    lib().ort_clip_face(_p(b), _p(out))
     return out
 
 
@@ -261,6 +282,12 @@ class Grid:
                                      _ptrs(U))
         if rc != 0:
             raise ValueError("ort_implicit_step failed with status %d" % rc)
+
+    def set_face_fix(self, mode):
+        """FIX_FPRESERVING (Eq. 19-21, default), FIX_PLUTO (flat fallback, L136) or FIX_CLIP (Eq. 36-38)"""
+        rc = lib().ort_set_face_fix(self._h, int(mode))
+        if rc != 0:
+            raise ValueError("ort_set_face_fix failed with status %d" % rc)
 
     def set_irradiation(self, div_firr):
         """div F_irr per cell (ghosted float64 array, kept alive by this object) or None (Sect. 2.9, Eq. 34-35)"""

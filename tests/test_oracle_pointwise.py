@@ -150,6 +150,47 @@ def test_fpreserving_face_invariant():
         assert fc * (1 - 1e-14) <= ff <= 1 + 1e-14
 
 
+def test_pluto_and_clip_face_cases():
+    """The two comparison schemes of Sect. 2.5 / 3.2: flat fallback (L136) and clip-only (Eq. 36-38)."""
+    Uc = [1.0, 0.2, 0.0, 0.0]
+    # f_face <= 1: both keep the reconstruction (Eq. 37; L136 "whenever ||R(F)|| > R(E)" not met) -- also where the
+    # f-preserving scheme would NOT keep it (f_face < f_cell)
+    for RU in ([1.0, 0.3, 0.1, 0.0], [1.2, 0.1, 0.0, 0.05]):
+        assert np.array_equal(ort.pluto_face(Uc, RU), RU)
+        assert np.array_equal(ort.clip_face(RU), RU)
+    # f_face > 1 (3-4-5 triangle: ||R(F)|| = 1 exactly, R(E) = 0.5)
+    RU = [0.5, 0.6, 0.0, 0.8]
+    assert np.array_equal(ort.pluto_face(Uc, RU), Uc)                       # E_f = E_c AND F_f = F_c (L136)
+    out = ort.clip_face(RU)
+    assert out[0] == 0.5 and np.allclose(out[1:], [0.3, 0.0, 0.4], rtol=0, atol=1e-16)   # Eq. 38
+    # the three schemes are three different answers on this input (a swapped branch in the grid-level switch shows)
+    fp = ort.fpreserving_face(Uc, RU)
+    assert np.allclose(fp, [0.5, 0.1, 0.0, 0.0], atol=1e-16)
+    # equality ||R(F)|| = R(E) belongs to the "keep" side of Eq. 37 and of L136 (strict ">")
+    RU = [1.0, 0.6, 0.0, 0.8]
+    assert np.array_equal(ort.pluto_face(Uc, RU), RU) and np.array_equal(ort.clip_face(RU), RU)
+
+
+def test_pluto_and_clip_face_invariants():
+    # f_face <= 1 afterwards; clip keeps E_f = R(E) and the direction of R(F); PLUTO returns one of its two inputs
+    ncl = 0
+    for E, F in random_states(300):
+        Uc = np.concatenate([[E], F])
+        RU = Uc * (1 + 0.5 * RNG.uniform(-1, 1, 4))
+        RU[0] = abs(RU[0]) + 1e-3
+        over = np.linalg.norm(RU[1:]) > RU[0]
+        ncl += over
+        c = ort.clip_face(RU)
+        assert c[0] == RU[0]
+        assert np.linalg.norm(c[1:]) <= c[0] * (1 + 1e-15)
+        if over:
+            assert np.linalg.norm(c[1:]) == pytest.approx(c[0], rel=1e-15)
+            assert np.allclose(np.cross(c[1:], RU[1:]), 0.0, atol=1e-16 * RU[0] ** 2) and np.dot(c[1:], RU[1:]) > 0
+        p = ort.pluto_face(Uc, RU)
+        assert np.array_equal(p, Uc if over else RU)
+    assert 20 < ncl < 280                                                    # both branches were exercised
+
+
 # ----------------------------------------------------------------------------- Riemann flux
 def test_riemann_consistency_and_closure_flux():
     for E, F in random_states(100):

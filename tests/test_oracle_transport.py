@@ -202,6 +202,75 @@ def test_substep_matches_brute_force(geo, solver, bcset):
             assert abs(mom[q][g.interior][k, j, i] - mb2[key][q]) < 1e-11 * scale
 
 
+@pytest.mark.parametrize("geo", ["cart", "sph", "cart2d"])
+@pytest.mark.parametrize("fix", [ort.FIX_PLUTO, ort.FIX_CLIP])
+def test_face_fix_variants_match_brute_force(geo, fix):
+    """ort_set_face_fix: the explicit step with the flat fallback (L136) / the clip of Eq. 36-38 against the brute-force
+    evaluation; the states are random with f up to 1, so many reconstructed faces exceed f = 1 and the variants differ
+    from the f-preserving default (asserted).
+
+    Tolerance of the clip: Eq. 38 puts the face state ON f = 1 up to rounding, where zeta of Eq. 23 behaves like
+    sqrt(1 - f): one ulp in ||F_f||/E_f moves lambda_1,3 by ~sqrt(2^-53) ~ 1e-8, and the HLL flux with them.  Two
+    correct evaluations therefore agree to ~1e-8 only (measured 4e-10 here); every other scheme keeps 2e-13."""
+    geometry, xf = GEOS[geo]
+    n = tuple(len(x) - 1 for x in xf)
+    bc = (1,) * 6
+    par = dict(chat=2.0, c=50.0, a_R=1.0, c_v=1.5, E_floor=1e-8, solver=ort.SOLVER_HLL, thick_limit=0, feedback_momentum=0)
+    g = ort.Grid(geometry, n, xf[0], xf[1], xf[2], bc)
+    g.set_params(ort.make_params(**par))
+    for which in (ort.OPAC_PLANCK, ort.OPAC_ROSSELAND, ort.OPAC_SCATTER):
+        g.set_opacity(which, ort.make_power_law(0.0))
+    rng = np.random.default_rng(1000 * fix + len(geo))
+    U = W.random_state(rng, n, fmax=1.0)
+    rho, T = np.ones(g.shape), np.ones(g.shape)
+    dt = g.cfl_dt(U, 0.4)
+    ref = [a.copy() for a in U]
+    g.explicit_step(dt, rho, T, U, ref)                                       # default scheme
+    g.set_face_fix(fix)
+    out = [a.copy() for a in U]
+    g.explicit_step(dt, rho, T, U, out)
+    B = brute.Brute(geometry, [list(map(float, x)) for x in xf], bc, dict(par, face_fix=fix), lambda r, t: (0.0, 0.0, 0.0))
+    Ub = B.explicit(_to_dict(g, U), _scalar_dict(g, rho), _scalar_dict(g, T), dt)
+    scale = max(abs(a[g.interior]).max() for a in U)
+    differs = 0.0
+    tol = 1e-8 if fix == ort.FIX_CLIP else 2e-13
+    for key, v in Ub.items():
+        i, j, k = key
+        for q in range(4):
+            got = out[q][g.interior][k, j, i]
+            assert abs(got - v[q]) < tol * scale, (key, q, got, v[q])
+            differs = max(differs, abs(got - ref[q][g.interior][k, j, i]))
+    assert differs > 1e-3 * scale
+    with pytest.raises(ValueError):
+        g.set_face_fix(3)
+
+
+@pytest.mark.parametrize("fix", [ort.FIX_FPRESERVING, ort.FIX_PLUTO, ort.FIX_CLIP])
+def test_face_fix_variants_conserve_energy_and_keep_uniform_states(fix):
+    """Flux form: whatever the face fix, sum E V is unchanged by the explicit step on a periodic grid, and a uniform
+    state (zero slopes: every scheme returns the cell value) stays uniform."""
+    n = (12, 10, 6)
+    xf = [np.linspace(0, 1, m + 1) for m in n]
+    g = ort.Grid(ort.CARTESIAN, n, xf[0], xf[1], xf[2], (0,) * 6)
+    g.set_params(ort.make_params(chat=3.0, c=30.0, a_R=1.0, c_v=1.5, E_floor=1e-12, solver=ort.SOLVER_HLL,
+                                 thick_limit=0, feedback_momentum=0))
+    for which in (ort.OPAC_PLANCK, ort.OPAC_ROSSELAND, ort.OPAC_SCATTER):
+        g.set_opacity(which, ort.make_power_law(0.0))
+    g.set_face_fix(fix)
+    rng = np.random.default_rng(77 + fix)
+    U = W.random_state(rng, n, fmax=1.0)
+    rho, T = np.ones(g.shape), np.ones(g.shape)
+    dt = g.cfl_dt(U, 0.4)
+    out = [a.copy() for a in U]
+    g.explicit_step(dt, rho, T, U, out)
+    assert out[0][g.interior].sum() == pytest.approx(U[0][g.interior].sum(), rel=1e-14)
+    Uu = [np.full(g.shape, v) for v in (2.0, 1.2, -0.9, 0.4)]
+    outu = [a.copy() for a in Uu]
+    g.explicit_step(dt, rho, T, Uu, outu)
+    for a, b in zip(Uu, outu):
+        assert np.abs(b[g.interior] - a[g.interior]).max() <= 4e-16 * 2.0
+
+
 # ----------------------------------------------------------------------------- metrics
 @pytest.mark.parametrize("geo", ["cyl", "sph"])
 def test_metrics_against_numerical_quadrature(geo):
