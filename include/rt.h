@@ -38,6 +38,10 @@ enum { RT_BC_PERIODIC = 0, RT_BC_OUTFLOW = 1, RT_BC_REFLECT = 2, RT_BC_FIXED = 3
 enum { RT_SOLVER_HLL = 0, RT_SOLVER_GLF = 1 /* global bound alpha = chat */,
        RT_SOLVER_RUSANOV = 2 /* local bound alpha = chat max |lambda_1,3| of the two face states (L150; R-G5) */ };
 enum { RT_OPAC_PLANCK = 0, RT_OPAC_ROSSELAND = 1, RT_OPAC_SCATTER = 2 };
+/* how f <= 1 is enforced on the reconstructed face states (rt_set_face_fix) */
+enum { RT_FIX_FPRESERVING = 0 /* Eq. 19-21, the paper's scheme and the default */,
+       RT_FIX_PLUTO = 1 /* flat fallback U_f = U_c whenever |R(F)| > R(E), L136 */,
+       RT_FIX_CLIP = 2 /* Eq. 36-38: F_f = R(F) R(E)/|R(F)| whenever |R(F)| > R(E) */ };
 
 typedef struct rt_grid rt_grid; /* opaque */
 
@@ -100,6 +104,13 @@ int32_t rt_explicit_step(rt_grid* g, double dt, const double* rho, const double*
  * (Eq. 28).  Asynchronous. */
 int32_t rt_implicit_step(rt_grid* g, double dt, const double* rho, double* T,
                          double* const mom[3], double* const U[4]);
+
+/* Face fix of the explicit half (step a3).  The paper's f-preserving scheme (Eq. 19-21) is the default; the two
+ * schemes it is compared with (Sect. 2.5, Sect. 3.2 Eq. 36-38 and Fig. 5) can be selected for the same
+ * comparisons.  They run in the per-direction kernels: with mode != RT_FIX_FPRESERVING rt_substep / rt_rk2_step take
+ * the split path (same results as rt_explicit_step + rt_implicit_step_cfl).  Unknown mode -> RT_ERR_INVALID_ARG, state
+ * unchanged.  Host call, nothing enqueued. */
+int32_t rt_set_face_fix(rt_grid* g, int32_t mode);
 
 /* Irradiation (Sect. 2.9, Eq. 34-35): div_firr = DEVICE array (field layout, caller-owned, must stay valid)
  * of the divergence of a user-defined irradiation flux; every later implicit half adds Q = -div_firr dt to S_1 of

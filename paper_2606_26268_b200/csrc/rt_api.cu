@@ -23,6 +23,7 @@ struct rt_grid {
     double* rk_save[4];  // rt_rk2_step: T^n, m^n (lazily allocated)
     double* rk_dt;       // rt_rk2_step: the dt each stage reads (and overwrites)
     const double* divfirr;  // rt_set_irradiation: caller-owned device array or nullptr
+    int face_fix;  // rt_set_face_fix: RT_FIX_*
     double* kpr;  // rho kappa_P per cell, written by the pre-pass of the fused sub-step (lazily allocated)
     CflScratch* scr;
     double* dt_dev;
@@ -157,6 +158,7 @@ extern "C" int32_t rt_grid_create(int32_t geometry, const int32_t n[3], int32_t 
     g->lim = nullptr;
     g->kpr = nullptr;
     g->divfirr = nullptr;
+    g->face_fix = RT_FIX_FPRESERVING;
     for (int q = 0; q < 4; ++q) g->rk_save[q] = nullptr;
     g->rk_dt = nullptr;
     g->scr = nullptr;
@@ -553,6 +555,7 @@ static int32_t explicit_impl(rt_grid* g, double dt, const double* dt_dev, const 
     a.dt_dev = dt_dev;
     a.chat = g->par.chat;
     a.rusanov = g->par.solver == RT_SOLVER_RUSANOV;
+    a.fix = g->face_fix;
     const bool hll = g->par.solver != RT_SOLVER_GLF;  // HLL and Rusanov need the wave speeds
     const bool curvi = D.geometry != RT_CARTESIAN;
     if (D.gh[0] == 0) {
@@ -632,6 +635,13 @@ static int32_t implicit_impl(rt_grid* g, double dt, const double* dt_dev, const 
         }
         RT_LAUNCH_CHECK(g);
     }
+    return RT_OK;
+}
+
+extern "C" int32_t rt_set_face_fix(rt_grid* g, int32_t mode) {
+    if (!g) return RT_ERR_INVALID_ARG;
+    if (mode < RT_FIX_FPRESERVING || mode > RT_FIX_CLIP) return fail(g, RT_ERR_INVALID_ARG, "rt_set_face_fix: unknown mode %d", mode);
+    g->face_fix = mode;
     return RT_OK;
 }
 
@@ -782,7 +792,9 @@ static int fused_segment_length(const rt_grid* g, int tiles) {
 
 static bool fused_eligible(const rt_grid* g) {
     const GridDev& D = g->dev;
-    return g->fused_seg >= 0 && D.gh[0] > 0 && D.gh[1] > 0 && D.ntot < (1LL << 31);  // 32-bit element offsets inside the kernel
+    // the comparison face fixes (rt_set_face_fix) exist in the per-direction kernels only
+    return g->fused_seg >= 0 && g->face_fix == RT_FIX_FPRESERVING && D.gh[0] > 0 && D.gh[1] > 0 &&
+           D.ntot < (1LL << 31);  // 32-bit element offsets inside the kernel
 }
 
 static int32_t fused_impl(rt_grid* g, double* dt_device, double cfl, const double* rho, double* T, double* const mom[3],

@@ -25,6 +25,7 @@ struct SweepArgs {
     const double* dt_dev;  // device-resident dt (rt_substep) or nullptr; then dt * chat = *dt_dev * chat
     double chat;
     int rusanov;  // RT_SOLVER_RUSANOV (the HLL instantiation computes the wave speeds it needs)
+    int fix;      // RT_FIX_* (rt_set_face_fix): 0 = f-preserving (Eq. 19-21), 1 = flat fallback (L136), 2 = clip (Eq. 36-38)
 };
 
 __device__ __forceinline__ double sweep_dtc(const SweepArgs& a) { return a.dt_dev ? __ldg(a.dt_dev) * a.chat : a.dtc; }
@@ -67,7 +68,7 @@ __global__ void __launch_bounds__(128) k_sweep_x(const __grid_constant__ GridDev
     if (THICK) limd = dmax(a.lim[id - 1], a.lim[id]);
 
     State lo, hi;
-    cell_faces<0, HLL>(q0, dm, dp, true, true, lo, hi);
+    cell_faces<0, HLL>(q0, dm, dp, true, true, lo, hi, 0.0, 0.0, 0.0, a.fix);
 
     // left state of this lane's lower face = upper-face state of the lane below
     State L;
@@ -176,7 +177,7 @@ __global__ void __launch_bounds__(128) k_sweep_march(const __grid_constant__ Gri
 #pragma unroll
         for (int q = 0; q < 4; ++q) dp[q] = qn[q] - qc[q];
         State lo, hi;
-        cell_faces<D, HLL>(qc, dm, dp, c >= ca, c < cb, lo, hi);
+        cell_faces<D, HLL>(qc, dm, dp, c >= ca, c < cb, lo, hi, 0.0, 0.0, 0.0, a.fix);
         if (c >= ca) {
             double fl[4];
             riemann<HLL>(hiPrev, lo, THICK ? dmax(limp, limc) : kInf, fl, a.rusanov != 0);

@@ -148,6 +148,28 @@ __device__ __forceinline__ void fpreserve(State& st, const double Uc[4], double 
     F2f = keep ? F2r : F2c * (r * r);
 }
 
+// The two comparison schemes of Sect. 2.5 / 3.2 (rt_set_face_fix; per-direction kernels only), same contract as fpreserve.
+// fix == 1, "PLUTO reconstruction" (L136): U_f = U_c, E included, whenever |R(F)| > R(E).
+// fix == 2, clip (Eq. 36-38): F_f = R(F) R(E)/|R(F)| whenever |R(F)| > R(E); IEEE sqrt and division (a rare path).
+__device__ __forceinline__ void facefix_variant(int fix, State& st, const double Uc[4], double Ec2, double F2c, double& E2f,
+                                                double& F2f) {
+    const double Ef = st.U[0];
+    E2f = Ef * Ef;
+    F2f = fma(st.U[3], st.U[3], fma(st.U[2], st.U[2], st.U[1] * st.U[1]));
+    if (F2f <= E2f) return;
+    if (fix == 1) {
+#pragma unroll
+        for (int q = 0; q < 4; ++q) st.U[q] = Uc[q];
+        E2f = Ec2;
+        F2f = F2c;
+    } else {
+        const double r = Ef / sqrt(F2f);
+#pragma unroll
+        for (int q = 1; q < 4; ++q) st.U[q] *= r;
+        F2f = fma(st.U[3], st.U[3], fma(st.U[2], st.U[2], st.U[1] * st.U[1]));
+    }
+}
+
 // Riemann flux (L150; R-G5, G6, G8) divided by chat, from left state L and right state R.
 // limd = 4/(3 tau_face) (Eq. 25-26 in units of chat; +inf when the thick limit is off).
 // rusanov (launch-uniform, HLL instantiation only): the local Lax-Friedrichs bound alpha = max |lambda_{1,3}| of the
@@ -187,10 +209,11 @@ __device__ __forceinline__ void riemann(const State& L, const State& R, double l
 // lo = state at the cell's lower face (RIGHT state of face c-1/2), hi = state at its upper face
 // (LEFT state of face c+1/2).  WANT_LO / WANT_HI are warp-uniform run-time flags.
 // KNOWN: the caller passes 1/E_c, E_c^2 and |F_c|^2 (the three directions of one cell share them).
+// fix (launch-uniform; RT_FIX_*): 0 = the f-preserving scheme; the fused kernel never passes anything else.
 template <int D, bool HLL, bool KNOWN = false>
 __device__ __forceinline__ void cell_faces(const double q0[4], const double dm[4], const double dp[4], bool want_lo,
                                            bool want_hi, State& lo, State& hi, double invEc_known = 0.0,
-                                           double Ec2_known = 0.0, double F2c_known = 0.0) {
+                                           double Ec2_known = 0.0, double F2c_known = 0.0, int fix = 0) {
     double h[4];
 #pragma unroll
     for (int q = 0; q < 4; ++q) h[q] = half_slope(dm[q], dp[q]);
@@ -202,14 +225,16 @@ __device__ __forceinline__ void cell_faces(const double q0[4], const double dm[4
 #pragma unroll
         for (int q = 0; q < 4; ++q) lo.U[q] = q0[q] - h[q];
         double E2f, F2f;
-        fpreserve(lo, q0, invEc, Ec2, F2c, E2f, F2f);
+        if (fix == 0) fpreserve(lo, q0, invEc, Ec2, F2c, E2f, F2f);
+        else facefix_variant(fix, lo, q0, Ec2, F2c, E2f, F2f);
         flux_and_speeds<D, HLL>(lo, E2f, F2f);
     }
     if (want_hi) {
 #pragma unroll
         for (int q = 0; q < 4; ++q) hi.U[q] = q0[q] + h[q];
         double E2f, F2f;
-        fpreserve(hi, q0, invEc, Ec2, F2c, E2f, F2f);
+        if (fix == 0) fpreserve(hi, q0, invEc, Ec2, F2c, E2f, F2f);
+        else facefix_variant(fix, hi, q0, Ec2, F2c, E2f, F2f);
         flux_and_speeds<D, HLL>(hi, E2f, F2f);
     }
 }

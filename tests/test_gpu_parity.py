@@ -412,6 +412,49 @@ def test_irradiation_source_in_the_implicit_half(rt, n, fused):
     assert (st2.T - st.T).abs().max().item() > 1e-6
 
 
+# ----------------------------------------------------------------------------- face-fix variants
+TOL_CLIP = 1e-7  # Eq. 38 puts face states ON f = 1 up to rounding, where zeta (Eq. 23) ~ sqrt(1 - f): one ulp in f moves
+                 # lambda_1,3 by ~1e-8 (tests/test_oracle_transport.py: test_face_fix_variants_match_brute_force)
+
+
+@pytest.mark.parametrize("case", ["cart3d", "sph3d", "cyl2d", "cart1d"])
+@pytest.mark.parametrize("fix", [W.FIX_PLUTO, W.FIX_CLIP])
+def test_face_fix_variants(rt, case, fix):
+    """rt_set_face_fix: the flat fallback of L136 and the clip of Eq. 36-38 in the per-direction kernels, 2 sub-steps on
+    random states with f up to 1 against the oracle; rt_substep falls back to the same kernels (bit-identical fields);
+    and the variant is not the default scheme (the fields differ by far more than the gate)."""
+    geometry, n, solver = {"cart3d": (W.CARTESIAN, (70, 33, 12), W.SOLVER_HLL), "sph3d": (W.SPHERICAL, (45, 20, 17), W.SOLVER_RUSANOV),
+                           "cyl2d": (W.CYLINDRICAL, (64, 40, 1), W.SOLVER_GLF), "cart1d": (W.CARTESIAN, (300, 1, 1), W.SOLVER_HLL)}[case]
+    w = random_workload(geometry, n, solver, 1, seed=90 + fix, fmax=1.0)
+    og = ort.grid_from_workload(w)
+    og.set_face_fix(fix)
+    refU, refT, refm, dts = ort.run_substeps(og, w, 2)
+    g = rt.grid_from_workload(w)
+    g.set_face_fix(fix)
+    st, _ = rt.run_substeps(g, w, 2, dts=dts)
+    torch.cuda.synchronize()
+    errs = field_errors(w, to_host(st.U), refU, st.T.cpu().numpy(), refT, to_host(st.mom), refm)
+    assert_below(errs, TOL_CLIP if fix == W.FIX_CLIP else 2 * TOL1, "face fix %d" % fix)
+    if fix == W.FIX_CLIP:  # only cells next to a clipped face see the sqrt(ulp) sensitivity: the bulk passes the one-sub-step gate
+        it = w.interior
+        e = np.abs(st.U[0].cpu().numpy()[it] - refU[0][it]) / np.abs(refU[0][it]).max()
+        assert np.median(e) <= TOL1
+    # rt_substep with a variant selected: the split kernels, with the device-resident dt
+    g2 = rt.grid_from_workload(w)
+    g2.set_face_fix(fix)
+    st2, _, hist = rt.run_substeps_fused(g2, w, 2)
+    torch.cuda.synchronize()
+    assert np.allclose(hist.cpu().numpy(), dts, rtol=TOL_CLIP if fix == W.FIX_CLIP else 1e-12, atol=0)
+    errs2 = field_errors(w, to_host(st2.U), refU, st2.T.cpu().numpy(), refT, to_host(st2.mom), refm)
+    assert_below(errs2, TOL_CLIP if fix == W.FIX_CLIP else 2 * TOL1, "face fix %d through rt_substep" % fix)
+    # not the default scheme
+    g3 = rt.grid_from_workload(w)
+    st3, _ = rt.run_substeps(g3, w, 2, dts=dts)
+    assert (st3.U[0] - st.U[0]).abs().max().item() > 1e-4 * float(np.abs(refU[0]).max())
+    with pytest.raises(Exception):
+        g3.set_face_fix(3)
+
+
 # ----------------------------------------------------------------------------- streams and CUDA graphs
 def test_substeps_on_a_side_stream_and_replayed_from_a_cuda_graph(rt):
     """rt_substep enqueues on the stream given at rt_grid_create and never synchronises: (a) a grid created on a side
