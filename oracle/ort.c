@@ -641,6 +641,34 @@ int32_t ort_set_irradiation(ort_grid* g, const double* div_firr) {
     return ORT_OK;
 }
 
+/* Sect. 3.7 (L379-383), gray (DESIGN R-G21).  Eq. 48: tau_irr(r) = int_{r_in}^{r} kappa rho dr' with rho constant in a
+ * cell: tau at the upper face of cell i = tau at its lower face + kappa rho_i (r_{i+1/2} - r_{i-1/2}).  Eq. 47 with the
+ * frequency integral collapsed to one gray band: F_irr(r) = L0 e^{-tau}/r^2 r_hat, L0 = F_s R_s^2.  Finite-volume
+ * divergence of a purely radial flux in a spherical cell: [A_+ F_+ - A_- F_-]/V = 3 (r_+^2 F_+ - r_-^2 F_-)/(r_+^3 - r_-^3)
+ * = 3 L0 (e^{-tau_+} - e^{-tau_-})/(r_+^3 - r_-^3); the difference of exponentials is written e^{-tau_-} expm1(-dtau)
+ * (the same number, without the cancellation of optically thin cells).  Cartesian: plane-parallel rays along x1,
+ * F_irr = L0 e^{-tau}, div = (F_+ - F_-)/dx. */
+int32_t ort_irradiation_radial(ort_grid* g, double L0, double kappa_irr, double tau_in, const double* rho,
+                               double* tau_hi, double* div_firr) {
+    if (!g || !rho || !div_firr) return ORT_ERR_INVALID_ARG;
+    if (g->geometry == ORT_CYLINDRICAL) return ORT_ERR_INVALID_ARG;
+    if (!(kappa_irr >= 0.0) || !(tau_in >= 0.0) || !isfinite(L0) || !isfinite(kappa_irr) || !isfinite(tau_in)) return ORT_ERR_INVALID_ARG;
+    for (int k = 0; k < g->n[2]; ++k)
+        for (int j = 0; j < g->n[1]; ++j) {
+            double tau_lo = tau_in;
+            for (int i = 0; i < g->n[0]; ++i) {
+                long id = IDX(g, i, j, k);
+                double rm = g->xf[0][i], rp = g->xf[0][i + 1];
+                double dtau = kappa_irr * rho[id] * (rp - rm);
+                double geo = g->geometry == ORT_SPHERICAL ? 3.0 / (rp * rp * rp - rm * rm * rm) : 1.0 / (rp - rm);
+                div_firr[id] = L0 * exp(-tau_lo) * expm1(-dtau) * geo;
+                tau_lo = tau_lo + dtau;
+                if (tau_hi) tau_hi[id] = tau_lo;
+            }
+        }
+    return ORT_OK;
+}
+
 int32_t ort_implicit_step(ort_grid* g, double dt, const double* rho, double* T,
                           double* const mom[3], double* const U[4]) {
     if (!g || !U || !rho || !T) return ORT_ERR_INVALID_ARG;

@@ -93,6 +93,12 @@ void ort_riemann_flux(const double UL[4], const double UR[4], int32_t d, double 
 double ort_opacity_eval(const ort_opacity* o, double rho, double T);       /* L299, L375 */
 /* Eq. 29-33 L195-216 + Eq. 30: in/out E, F[3], T; optional mom[3] (may be NULL) */
 int32_t ort_set_irradiation(ort_grid* g, const double* div_firr);
+/* Sect. 3.7, Eq. 47-48 L379-383 in gray form (DESIGN R-G21): along every x1 ray tau_irr at the radial faces
+ * (tau_in at the inner edge, + kappa_irr rho_i dr_i per cell), F_irr = L0 e^{-tau}/r^2 (spherical; L0 e^{-tau}
+ * along x1 on a Cartesian grid) and its finite-volume divergence.  rho, tau_hi (optional: tau at each cell's
+ * UPPER face), div_firr: host, ghosted field layout; only interior cells are written. */
+int32_t ort_irradiation_radial(ort_grid* g, double L0, double kappa_irr, double tau_in, const double* rho,
+                               double* tau_hi, double* div_firr);
 void ort_implicit_cell(const ort_params* p, double dt, double rho, double kappaP, double chi,
                        double* E, double F[3], double* T, double* mom, double Q);
 

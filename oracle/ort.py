@@ -81,6 +81,8 @@ def lib():
         L.ort_implicit_cell.restype = None
         L.ort_implicit_cell.argtypes = [C.POINTER(Params), C.c_double, C.c_double, C.c_double, C.c_double,
                                         _dp, _dp, _dp, _dp, C.c_double]
+        L.ort_irradiation_radial.restype = C.c_int32
+        L.ort_irradiation_radial.argtypes = [C.c_void_p, C.c_double, C.c_double, C.c_double, _dp, _dp, _dp]
         L.ort_set_irradiation.restype = C.c_int32
         L.ort_set_irradiation.argtypes = [C.c_void_p, _dp]
         L.ort_grid_create.argtypes = [C.c_int32, C.POINTER(C.c_int32), C.c_int32, _dp, _dp, _dp,
@@ -288,6 +290,16 @@ class Grid:
         rc = lib().ort_set_face_fix(self._h, int(mode))
         if rc != 0:
             raise ValueError("ort_set_face_fix failed with status %d" % rc)
+
+    def irradiation_radial(self, L0, kappa_irr, tau_in, rho):
+        """gray Eq. 47-48 along x1 rays: returns (tau at each cell's upper face, div F_irr), ghosted arrays, zero outside
+        the interior"""
+        _check64(rho)
+        tau, div = self.zeros(), self.zeros()
+        rc = lib().ort_irradiation_radial(self._h, float(L0), float(kappa_irr), float(tau_in), _p(rho), _p(tau), _p(div))
+        if rc != 0:
+            raise ValueError("ort_irradiation_radial failed with status %d" % rc)
+        return tau, div
 
     def set_irradiation(self, div_firr):
         """div F_irr per cell (ghosted float64 array, kept alive by this object) or None (Sect. 2.9, Eq. 34-35)"""

@@ -267,3 +267,72 @@ def test_irradiation_array_reaches_the_grid_level_implicit_step():
     g.set_irradiation(None)
     tot1 = w.rho[it] * p["c_v"] * T[it] + (p["c"] / p["chat"]) * U[0][it]
     assert np.allclose(tot1 - tot0, -div[it] * dt, rtol=1e-10, atol=1e-13)
+
+
+# ----------------------------------------------------------------------------- radial irradiation (Sect. 3.7, Eq. 47-48)
+def _sph_grid(n=(40, 6, 5), rin=1.0, rout=50.0):
+    xf = [np.geomspace(rin, rout, n[0] + 1), np.linspace(np.pi / 2 - 0.4, np.pi / 2 + 0.3, n[1] + 1), np.linspace(0.0, 2 * np.pi, n[2] + 1)]
+    return ort.Grid(ort.SPHERICAL, n, xf[0], xf[1], xf[2], (1, 1, 1, 1, 0, 0)), xf
+
+
+def test_irradiation_radial_optical_depth_is_the_analytic_integral_of_eq48():
+    """rho(r) = C(theta, phi) / r^2, fed as its exact cell average in r: Eq. 48 gives tau(r) = tau_in + kappa C (1/r_in - 1/r)
+    at every radial face, per ray; and the flux divergence equals [A+ F+ - A- F-]/V with F = L0 e^{-tau}/r^2 (Eq. 47, gray)
+    built in numpy from the ANALYTIC tau and the oracle's quadrature-pinned face areas and volumes."""
+    g, xf = _sph_grid()
+    r = xf[0]
+    rng = np.random.default_rng(5)
+    Cray = rng.uniform(0.5, 30.0, size=(g.n[2], g.n[1], 1))
+    rho = g.zeros()
+    rho[g.interior] = Cray * ((1.0 / r[:-1] - 1.0 / r[1:]) / np.diff(r))[None, None, :]
+    L0, kap, tau_in = 7.0, 0.8, 0.05
+    tau, div = g.irradiation_radial(L0, kap, tau_in, rho)
+    tau_face = tau_in + kap * Cray * (1.0 / r[0] - 1.0 / r)[None, None, :]          # all n1 + 1 faces
+    assert np.allclose(tau[g.interior], tau_face[..., 1:], rtol=1e-13, atol=0)
+    vol, a1, _, _ = g.metrics()
+    F = L0 * np.exp(-tau_face) / r[None, None, :] ** 2
+    ref = (a1[..., 1:] * F[..., 1:] - a1[..., :-1] * F[..., :-1]) / vol
+    assert np.all(div[g.interior] < 0.0)
+    assert np.allclose(div[g.interior], ref, rtol=2e-12, atol=0)          # the reference differences e^{-tau}: ~1e-14 / dtau
+    # nothing outside the interior is written
+    mask = np.ones(g.shape, bool)
+    mask[g.interior] = False
+    assert not div[mask].any() and not tau[mask].any()
+
+
+def test_irradiation_radial_deposits_exactly_the_luminosity_it_removes():
+    """sum_i div_i V_i over a ray bundle = -(L_in - L_out): the solid angle of the bundle times L0 (e^{-tau_in} - e^{-tau_out}),
+    tau_out from numpy's cumulative sum; and the optically thin limit is div -> -kappa rho F_irr (the continuum equation)."""
+    g, xf = _sph_grid()
+    r = xf[0]
+    rng = np.random.default_rng(6)
+    rho = g.zeros()
+    rho[g.interior] = np.exp(rng.uniform(-3, 1, size=rho[g.interior].shape))
+    L0, kap, tau_in = 3.0, 0.4, 0.0
+    tau, div = g.irradiation_radial(L0, kap, tau_in, rho)
+    vol, _, _, _ = g.metrics()
+    tau_out = tau_in + kap * np.cumsum(rho[g.interior] * np.diff(r)[None, None, :], axis=-1)[..., -1]
+    omega = (np.cos(xf[1][:-1]) - np.cos(xf[1][1:]))[None, :] * np.diff(xf[2])[:, None]      # solid angle per ray
+    assert (div[g.interior] * vol).sum(axis=-1) == pytest.approx(-(L0 * omega * (np.exp(-tau_in) - np.exp(-tau_out))), rel=1e-12)
+    eps = 1e-9
+    _, thin = g.irradiation_radial(L0, eps, 0.0, rho)
+    rc2 = 3.0 * np.diff(r) / np.diff(r ** 3)                                               # <1/r^2> of a shell
+    assert np.allclose(thin[g.interior], -eps * rho[g.interior] * L0 * rc2[None, None, :], rtol=1e-6, atol=0)
+
+
+def test_irradiation_radial_cartesian_slab_and_errors():
+    """plane-parallel rays along x1 on a Cartesian grid, uniform rho: F = L0 e^{-kappa rho x}, cell-averaged dF/dx"""
+    n = (30, 3, 1)
+    xf = [np.linspace(0.0, 2.0, n[0] + 1) ** 1.3, np.linspace(0, 1, n[1] + 1), np.array([0.0, 1.0])]
+    g = ort.Grid(ort.CARTESIAN, n, xf[0], xf[1], xf[2], (1, 1, 0, 0, 0, 0))
+    rho = np.full(g.shape, 2.5)
+    tau, div = g.irradiation_radial(4.0, 1.2, 0.3, rho)
+    x = xf[0]
+    F = 4.0 * np.exp(-(0.3 + 1.2 * 2.5 * x))
+    assert np.allclose(div[g.interior], (np.diff(F) / np.diff(x))[None, None, :], rtol=1e-12, atol=0)
+    assert np.allclose(tau[g.interior], (0.3 + 3.0 * x[1:])[None, None, :], rtol=1e-14, atol=0)
+    gc = ort.Grid(ort.CYLINDRICAL, (4, 4, 1), np.linspace(1, 2, 5), np.linspace(0, 1, 5), np.array([0.0, 1.0]), (1, 1, 1, 1, 0, 0))
+    with pytest.raises(ValueError):
+        gc.irradiation_radial(1.0, 1.0, 0.0, gc.zeros() + 1.0)
+    with pytest.raises(ValueError):
+        g.irradiation_radial(1.0, -1.0, 0.0, rho)
