@@ -117,6 +117,17 @@ int32_t rt_set_face_fix(rt_grid* g, int32_t mode);
  * Eq. 33, i.e. to the coupled energy C_v T + (c/chat) E_r (Eq. 34).  NULL switches it off (the default). */
 int32_t rt_set_irradiation(rt_grid* g, const double* div_firr);
 
+/* The stellar irradiation flux of Sect. 3.7 in gray form (Eq. 47-48; DESIGN R-G21), the "user function" of
+ * Sect. 2.9 for a central source: along every x1 ray tau_irr at the radial faces is tau_in at the inner edge plus
+ * kappa_irr rho_i (r_{i+1/2} - r_{i-1/2}) per cell (Eq. 48, a prefix sum); F_irr = L0 e^{-tau}/r^2 r_hat on a spherical
+ * grid (L0 = F_s R_s^2), L0 e^{-tau} x_hat on a Cartesian one (plane-parallel rays); div_firr = its finite-volume
+ * divergence [A_+ F_+ - A_- F_-]/V per interior cell, ready for rt_set_irradiation.  rho, div_firr and the optional
+ * tau_hi (tau at each cell's UPPER x1 face; NULL allowed): DEVICE, fp64, field layout, caller-owned; only interior
+ * cells are written.  Cylindrical grid, kappa_irr < 0, tau_in < 0 or a non-finite scalar -> RT_ERR_INVALID_ARG.
+ * Asynchronous on the grid's stream. */
+int32_t rt_irradiation_radial(rt_grid* g, double L0, double kappa_irr, double tau_in, const double* rho,
+                              double* tau_hi, double* div_firr);
+
 /* rt_implicit_step with step 10 (L120; R-G15) fused behind it: the kernel that writes the updated state also
  * reduces the CFL rate of that state (warp shuffles + filtered atomicMax), and a one-thread kernel writes
  * *dt_next_device = cfl / max rate (DEVICE double): bit-identical to rt_cfl_dt_async on the updated U, without

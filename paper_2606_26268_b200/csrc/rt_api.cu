@@ -645,6 +645,20 @@ extern "C" int32_t rt_set_face_fix(rt_grid* g, int32_t mode) {
     return RT_OK;
 }
 
+extern "C" int32_t rt_irradiation_radial(rt_grid* g, double L0, double kappa_irr, double tau_in, const double* rho,
+                                         double* tau_hi, double* div_firr) {
+    if (!g) return RT_ERR_INVALID_ARG;
+    if (!aligned8(rho) || !aligned8(div_firr) || (tau_hi && !aligned8(tau_hi)))
+        return fail(g, RT_ERR_INVALID_ARG, "rt_irradiation_radial: null or misaligned pointer");
+    if (g->dev.geometry == RT_CYLINDRICAL) return fail(g, RT_ERR_INVALID_ARG, "rt_irradiation_radial: x1 rays need a spherical or Cartesian grid");
+    if (!isfinite(L0) || !isfinite(kappa_irr) || !isfinite(tau_in) || !(kappa_irr >= 0.0) || !(tau_in >= 0.0))
+        return fail(g, RT_ERR_INVALID_ARG, "rt_irradiation_radial: L0 finite, kappa_irr >= 0 and tau_in >= 0 required");
+    const long long rays = (long long)g->dev.n[1] * g->dev.n[2];
+    k_irradiation_radial<<<(unsigned)((rays + 3) / 4), 128, 0, g->stream>>>(g->dev, L0, kappa_irr, tau_in, rho, tau_hi, div_firr);
+    RT_LAUNCH_CHECK(g);
+    return RT_OK;
+}
+
 extern "C" int32_t rt_set_irradiation(rt_grid* g, const double* div_firr) {
     if (!g) return RT_ERR_INVALID_ARG;
     if (div_firr && !aligned8(div_firr)) return fail(g, RT_ERR_INVALID_ARG, "rt_set_irradiation: misaligned pointer");

@@ -215,6 +215,51 @@ __global__ void __launch_bounds__(128) k_rk2_average(const __grid_constant__ Gri
 }
 
 // ------------------------------------------------------------------------------------------------
+// Radial irradiation (Sect. 3.7, Eq. 47-48, gray: R-G21).  One warp per x1 ray, 32 consecutive cells per
+// pass (coalesced 256-B rows): dtau = kappa rho dr per lane, inclusive scan over the warp by shuffles, the ray's
+// running tau carried from pass to pass in a register.  div F_irr = L0 e^{-tau_-} expm1(-dtau) x 3/(r_+^3 - r_-^3)
+// (spherical: [A_+ F_+ - A_- F_-]/V of F = L0 e^{-tau}/r^2) or x 1/dx (Cartesian, plane-parallel rays along x1).
+// HBM: 8 B read + 8 B written per cell (+ 8 B with tau_hi).
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(128) k_irradiation_radial(const __grid_constant__ GridDev g, double L0, double kappa,
+                                                            double tau_in, const double* __restrict__ rho,
+                                                            double* __restrict__ tau_hi, double* __restrict__ div) {
+    const int lane = threadIdx.x & 31;
+    const long long ray = (long long)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    if (ray >= (long long)g.n[1] * g.n[2]) return;  // whole warps leave together
+    const int j = (int)(ray % g.n[1]), k = (int)(ray / g.n[1]);
+    const long long row = g.gh[0] + (j + g.gh[1]) * g.stride[1] + (k + g.gh[2]) * g.stride[2];
+    const int n1 = g.n[0];
+    const bool sph = g.geometry == 2;
+    double carry = tau_in;
+#pragma unroll 2
+    for (int i0 = 0; i0 < n1; i0 += 32) {
+        const int i = i0 + lane;
+        const bool on = i < n1;
+        double dtau = 0.0, geo = 0.0;
+        if (on) {
+            const double rm = g.xf[0][i], rp = g.xf[0][i + 1];
+            dtau = kappa * rho[row + i] * (rp - rm);
+            geo = sph ? 3.0 / (rp * rp * rp - rm * rm * rm) : 1.0 / (rp - rm);
+        }
+        double incl = dtau;
+#pragma unroll
+        for (int s = 1; s < 32; s <<= 1) {
+            const double up = __shfl_up_sync(0xffffffffu, incl, s);
+            if (lane >= s) incl += up;
+        }
+        double excl = __shfl_up_sync(0xffffffffu, incl, 1);
+        if (lane == 0) excl = 0.0;
+        const double tlo = carry + excl, thi = carry + incl;
+        if (on) {
+            div[row + i] = L0 * exp(-tlo) * expm1(-dtau) * geo;
+            if (tau_hi) tau_hi[row + i] = thi;
+        }
+        carry = __shfl_sync(0xffffffffu, thi, 31);
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
 // a9: opacities.  Power law kappa0 (rho/rho0)^a (T/T0)^b clipped (L299) or bilinear table of
 // log10 kappa on a uniform (log10 rho, log10 T) grid (L375; R-G14).
 // ------------------------------------------------------------------------------------------------

@@ -67,6 +67,7 @@ _SIGNATURES = {
                                C.POINTER(C.c_void_p), C.POINTER(C.c_void_p)]),
     "rt_set_irradiation": (C.c_int32, [C.c_void_p, C.c_void_p]),
     "rt_set_face_fix": (C.c_int32, [C.c_void_p, C.c_int32]),
+    "rt_irradiation_radial": (C.c_int32, [C.c_void_p, C.c_double, C.c_double, C.c_double, C.c_void_p, C.c_void_p, C.c_void_p]),
     "rt_rk2_step": (C.c_int32, [C.c_void_p, C.c_void_p, C.c_double, C.c_void_p, C.c_void_p, C.POINTER(C.c_void_p),
                                 C.POINTER(C.c_void_p), C.POINTER(C.c_void_p), C.POINTER(C.c_void_p)]),
     "rt_cfl_dt": (C.c_int32, [C.c_void_p, C.POINTER(C.c_void_p), C.c_double, _dp]),
@@ -299,6 +300,16 @@ class Grid:
         rc = lib().rt_set_face_fix(self._h, int(mode))
         if rc != OK:
             self._raise("rt_set_face_fix", rc)
+
+    def irradiation_radial(self, L0, kappa_irr, tau_in, rho, tau_hi, div_firr):
+        _check_field(rho, self.shape, "rho")
+        _check_field(div_firr, self.shape, "div_firr")
+        if tau_hi is not None:
+            _check_field(tau_hi, self.shape, "tau_hi")
+        rc = lib().rt_irradiation_radial(self._h, float(L0), float(kappa_irr), float(tau_in), rho.data_ptr(),
+                                         tau_hi.data_ptr() if tau_hi is not None else None, div_firr.data_ptr())
+        if rc != OK:
+            self._raise("rt_irradiation_radial", rc)
 
     def set_irradiation(self, div_firr):
         """div F_irr per cell (CUDA float64 tensor in the field layout, kept alive by this object) or None"""

@@ -412,6 +412,64 @@ def test_irradiation_source_in_the_implicit_half(rt, n, fused):
     assert (st2.T - st.T).abs().max().item() > 1e-6
 
 
+# ----------------------------------------------------------------------------- radial irradiation (Sect. 3.7, Eq. 47-48)
+@pytest.mark.parametrize("geometry,n", [(W.SPHERICAL, (70, 33, 12)), (W.SPHERICAL, (256, 9, 5)), (W.SPHERICAL, (31, 1, 1)),
+                                        (W.CARTESIAN, (97, 14, 1)), (W.SPHERICAL, (300, 7, 3))])
+def test_irradiation_radial_prefix_scan(rt, geometry, n):
+    """rt_irradiation_radial (one warp per x1 ray, shuffle scan) against the oracle's sequential sum: tau at every upper
+    face and div F_irr element by element over rays that run from optically thin to tau ~ 30; row lengths below, at and
+    above a multiple of 32.  Then the same array through rt_set_irradiation and 2 sub-steps."""
+    w = random_workload(geometry, n, W.SOLVER_HLL, 1, seed=123, fmax=0.9, bc=(1, 1, 1, 1, 0, 0) if n[1] > 1 else (1, 1, 0, 0, 0, 0))
+    og = ort.grid_from_workload(w)
+    L0, tau_in = 3.5, 0.01
+    kap = 30.0 / (w.rho[w.interior].mean() * (w.xf[0][-1] - w.xf[0][0]))
+    tau_ref, div_ref = og.irradiation_radial(L0, kap, tau_in, w.rho)
+    g = rt.grid_from_workload(w)
+    drho = g.to_device(w.rho)
+    dtau, ddiv = torch.zeros_like(drho), torch.zeros_like(drho)
+    g.irradiation_radial(L0, kap, tau_in, drho, dtau, ddiv)
+    ddiv2 = torch.zeros_like(drho)
+    g.irradiation_radial(L0, kap, tau_in, drho, None, ddiv2)                  # tau_hi is optional
+    torch.cuda.synchronize()
+    assert torch.equal(ddiv, ddiv2)
+    tau, div = dtau.cpu().numpy(), ddiv.cpu().numpy()
+    it = w.interior
+    assert tau_ref[it].max() > 5.0
+    assert np.allclose(tau[it], tau_ref[it], rtol=1e-13, atol=0)              # summation order: a few ulp
+    # element-wise relative: |d div / div| <= |d tau_lo| + ulps of exp / expm1
+    assert np.allclose(div[it], div_ref[it], rtol=1e-12, atol=0)
+    mask = np.ones(div.shape, bool)
+    mask[it] = False
+    assert not div[mask].any() and not tau[mask].any()                        # only interior cells are written
+    # through the implicit half
+    og.set_irradiation(div_ref)
+    refU, refT, refm, dts = ort.run_substeps(og, w, 2)
+    og.set_irradiation(None)
+    g.set_irradiation(ddiv)
+    st, _ = rt.run_substeps(g, w, 2, dts=dts)
+    torch.cuda.synchronize()
+    errs = field_errors(w, to_host(st.U), refU, st.T.cpu().numpy(), refT, to_host(st.mom), refm)
+    assert_below(errs, 2 * TOL1, "radial irradiation through 2 sub-steps")
+
+
+def test_irradiation_radial_rejects_bad_arguments(rt):
+    w = random_workload(W.CYLINDRICAL, (16, 8, 1), W.SOLVER_HLL, 0, seed=5)
+    g = rt.grid_from_workload(w)
+    d = g.to_device(w.rho)
+    out = torch.zeros_like(d)
+    with pytest.raises(Exception):
+        g.irradiation_radial(1.0, 1.0, 0.0, d, None, out)                      # cylindrical: no x1 rays from a point
+    w2 = random_workload(W.SPHERICAL, (16, 8, 1), W.SOLVER_HLL, 0, seed=5)
+    g2 = rt.grid_from_workload(w2)
+    d2 = g2.to_device(w2.rho)
+    out2 = torch.zeros_like(d2)
+    for bad in ((float("nan"), 1.0, 0.0), (1.0, -1.0, 0.0), (1.0, 1.0, -0.5), (1.0, float("inf"), 0.0)):
+        with pytest.raises(Exception):
+            g2.irradiation_radial(*bad, d2, None, out2)
+    torch.cuda.synchronize()
+    assert not out2.any()
+
+
 # ----------------------------------------------------------------------------- face-fix variants (SURVEY 8(f) NEXT-4)
 TOL_CLIP = 1e-7  # Eq. 38 puts face states ON f = 1 up to rounding, where zeta (Eq. 23) ~ sqrt(1 - f): one ulp in f moves
                  # lambda_1,3 by ~1e-8 (tests/test_oracle_transport.py: test_face_fix_variants_match_brute_force)
