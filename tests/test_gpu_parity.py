@@ -452,6 +452,26 @@ def test_irradiation_radial_prefix_scan(rt, geometry, n):
     assert_below(errs, 2 * TOL1, "radial irradiation through 2 sub-steps")
 
 
+def test_irradiation_radial_full_size_c5_grid(rt):
+    """the C5 grid and density at BASELINE's full size (256 x 128 x 256, 32768 rays of 256 cells; the disc mid-plane reaches
+    tau ~ 100 as in Sect. 3.7, the floor region stays thin): every cell against the oracle"""
+    w = W.c5()
+    og = ort.grid_from_workload(w)
+    it = w.interior
+    r = w.xf[0]
+    kap = 100.0 / float((w.rho[it].max(axis=(0, 1)) * np.diff(r)).sum())      # densest ray: tau_out = 100
+    tau_ref, div_ref = og.irradiation_radial(2.0, kap, 0.0, w.rho)
+    g = rt.grid_from_workload(w)
+    drho = g.to_device(w.rho)
+    dtau, ddiv = torch.zeros_like(drho), torch.zeros_like(drho)
+    g.irradiation_radial(2.0, kap, 0.0, drho, dtau, ddiv)
+    torch.cuda.synchronize()
+    tau, div = dtau.cpu().numpy(), ddiv.cpu().numpy()
+    assert tau_ref[it].max() > 50.0 and tau_ref[it][..., -1].min() < 0.1
+    assert np.allclose(tau[it], tau_ref[it], rtol=1e-13, atol=0)
+    assert np.allclose(div[it], div_ref[it], rtol=1e-12, atol=0)
+
+
 def test_irradiation_radial_rejects_bad_arguments(rt):
     w = random_workload(W.CYLINDRICAL, (16, 8, 1), W.SOLVER_HLL, 0, seed=5)
     g = rt.grid_from_workload(w)
