@@ -414,7 +414,8 @@ def test_irradiation_source_in_the_implicit_half(rt, n, fused):
 
 # ----------------------------------------------------------------------------- radial irradiation (Sect. 3.7, Eq. 47-48)
 @pytest.mark.parametrize("geometry,n", [(W.SPHERICAL, (70, 33, 12)), (W.SPHERICAL, (256, 9, 5)), (W.SPHERICAL, (31, 1, 1)),
-                                        (W.CARTESIAN, (97, 14, 1)), (W.SPHERICAL, (300, 7, 3))])
+                                        (W.CARTESIAN, (97, 14, 1)), (W.SPHERICAL, (300, 7, 3)),
+                                        (W.SPHERICAL, (32, 3, 2)), (W.SPHERICAL, (33, 2, 2)), (W.SPHERICAL, (4, 5, 1))])
 def test_irradiation_radial_prefix_scan(rt, geometry, n):
     """rt_irradiation_radial (one warp per x1 ray, shuffle scan) against the oracle's sequential sum: tau at every upper
     face and div F_irr element by element over rays that run from optically thin to tau ~ 30; row lengths below, at and
