@@ -184,6 +184,13 @@ int32_t rt_set_tuning(rt_grid* g, int32_t march_len, int32_t fused_seg);
 /* Measurement aid: with RT_M1_NO_TMA=1 in the environment at rt_grid_create the fused kernel stages its planes by
  * cp.async even where TMA could address them (the path arrays with an odd x1 pitch always take). */
 
+/* Measurement aid (SURVEY.md Sect. 8(d): "measure its own fp64 peak with a DFMA microbenchmark in the same run"); no grid
+ * handle.  Launches `blocks` x `threads` threads, each running `chains` (1, 2, 4 or 8) independent chains of
+ * 8 * iters dependent DFMAs, twice (the first launch warms up), and writes the CUDA-event duration of the second launch
+ * in milliseconds to *ms_host (HOST).  Thread instructions of that launch = blocks * threads * chains * 8 * iters.
+ * Synchronises the stream.  Bad argument -> RT_ERR_INVALID_ARG; no device / launch failure -> RT_ERR_CUDA. */
+int32_t rt_measure_fp64(void* cuda_stream, int32_t blocks, int32_t threads, int32_t chains, int32_t iters, double* ms_host);
+
 const char* rt_last_error(const rt_grid* g);
 
 #ifdef __cplusplus

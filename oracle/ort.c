@@ -11,9 +11,12 @@
  * No tiling, no fusion, no algebraic shortcuts: every face flux is stored in a full array and the
  * divergence is taken with full 3-D face areas and volumes.  "R-Gn" = reading Gn of DESIGN.md.
  *
- * Parity pins live in tests/test_oracle_*.py.  Conventions that nothing outside this file fixes
- * (R-G7 tau_face and its dx, R-G9 source form, R-G11 floor placement, R-G15 CFL formula) are
- * "parity unpinned" beyond self-consistency and the physics checks listed in DESIGN.md.
+ * Parity pins live in tests/test_oracle_*.py.  Readings that nothing outside this repo fixes (R-G7 tau_face = min
+ * of the two cells and dx = the cell's largest extent, R-G9 source form, R-G11 floor placement, R-G15 CFL formula)
+ * stay conventions; what IS pinned is that the code implements them as stated: tau_cell and the Eq. 25-26 wiring by
+ * the hand-worked interface fluxes and the clamp-active diffusion rates of tests/test_oracle_thick_limit.py (each
+ * mutation of that block turns one of them red: DESIGN.md Sect. 7), the sources by the curvilinear residual tests,
+ * the CFL form by its two closed forms.
  *
  * Build: gcc -O2 -ffp-contract=off -fopenmp -shared -fPIC oracle/ort.c -o oracle/libort.so -lm
  */

@@ -370,9 +370,10 @@ def run_substeps(g, w, nsub, dts=None, state=None):
     return U, T, mom, used
 
 
-def run_rk2(g, w, nsteps):
+def run_rk2(g, w, nsteps, t_end=None):
     """nsteps RK2 steps (two Euler sub-steps and the average of every evolved variable; DESIGN.md
-    R-G10) of workload w on grid g, each with the CFL time step of its starting state.  Returns (U, T, mom, dts)."""
+    R-G10) of workload w on grid g, each with the CFL time step of its starting state.  With t_end the run instead stops
+    at that time (the last step shortened to land on it; nsteps is then ignored).  Returns (U, T, mom, dts)."""
     U = [a.copy() for a in w.U]
     T = w.T.copy()
     mom = [a.copy() for a in w.mom] if w.mom is not None else None
@@ -381,9 +382,13 @@ def run_rk2(g, w, nsteps):
     it = g.interior
     g.set_params(make_params(**w.params))
     used = []
-    for _ in range(nsteps):
+    t = 0.0
+    while (len(used) < nsteps) if t_end is None else (t < t_end - 1e-12):
         dt = g.cfl_dt(U, w.cfl)
+        if t_end is not None:
+            dt = min(dt, t_end - t)
         used.append(dt)
+        t += dt
         T0 = T.copy()
         m0 = [a.copy() for a in mom] if mom is not None else None
         g.explicit_step(dt, w.rho, T, U, U1)

@@ -14,7 +14,7 @@ ROOT = os.path.dirname(HERE)
 LIB_PATH = os.path.join(HERE, "librt_m1.so")
 SOURCES = [os.path.join(HERE, "csrc", "rt_api.cu")]
 HEADERS = [os.path.join(HERE, "csrc", f) for f in ("rt_math.cuh", "rt_types.cuh", "rt_kernels_aux.cuh",
-                                                    "rt_kernels_step.cuh", "rt_kernels_fused.cuh")] + [os.path.join(ROOT, "include", "rt.h")]
+                                                    "rt_kernels_step.cuh", "rt_kernels_fused.cuh", "rt_kernels_measure.cuh")] + [os.path.join(ROOT, "include", "rt.h")]
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-shared", "-Xcompiler", "-fPIC", "-cudart", "static"]

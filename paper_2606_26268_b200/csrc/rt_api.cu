@@ -12,6 +12,7 @@
 
 #include "../../include/rt.h"
 #include "rt_kernels_fused.cuh"
+#include "rt_kernels_measure.cuh"
 
 using namespace rtm1;
 
@@ -981,4 +982,43 @@ extern "C" int32_t rt_get_floor_counts(rt_grid* g, int64_t* n_floor, int64_t* n_
     if (n_floor) *n_floor = (int64_t)g->counters_pinned[0];
     if (n_clip) *n_clip = (int64_t)g->counters_pinned[1];
     return RT_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// Measurement hook (no grid handle): time one launch of the DFMA-chain microbenchmark with CUDA events on `cuda_stream`.
+extern "C" int32_t rt_measure_fp64(void* cuda_stream, int32_t blocks, int32_t threads, int32_t chains, int32_t iters,
+                                   double* ms_host) {
+    if (!ms_host || blocks < 1 || threads < 32 || threads > 1024 || (threads & 31) || iters < 1) return RT_ERR_INVALID_ARG;
+    if (chains != 1 && chains != 2 && chains != 4 && chains != 8 && chains != 101 && chains != 102 && chains != 104) return RT_ERR_INVALID_ARG;
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
+    double* sink = nullptr;
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    int32_t rc = RT_ERR_CUDA;
+    if (cudaMalloc(&sink, sizeof(double)) == cudaSuccess && cudaEventCreate(&e0) == cudaSuccess &&
+        cudaEventCreate(&e1) == cudaSuccess) {
+        const double a = 0.999999, b = 1.0e-6;  // x -> 1: finite for any iteration count
+        for (int pass = 0; pass < 2; ++pass) {  // pass 0 warms up (module load, clocks)
+            cudaEventRecord(e0, st);
+            switch (chains) {
+                case 1: k_dfma_chains<1><<<blocks, threads, 0, st>>>(sink, iters, a, b); break;
+                case 2: k_dfma_chains<2><<<blocks, threads, 0, st>>>(sink, iters, a, b); break;
+                case 4: k_dfma_chains<4><<<blocks, threads, 0, st>>>(sink, iters, a, b); break;
+                case 101: k_dfma_chains<1, 64><<<blocks, threads, 0, st>>>(sink, iters, a, b); break;
+                case 102: k_dfma_chains<2, 64><<<blocks, threads, 0, st>>>(sink, iters, a, b); break;
+                case 104: k_dfma_chains<4, 64><<<blocks, threads, 0, st>>>(sink, iters, a, b); break;
+                default: k_dfma_chains<8><<<blocks, threads, 0, st>>>(sink, iters, a, b); break;
+            }
+            cudaEventRecord(e1, st);
+        }
+        float t = 0.f;
+        if (cudaGetLastError() == cudaSuccess && cudaEventSynchronize(e1) == cudaSuccess &&
+            cudaEventElapsedTime(&t, e0, e1) == cudaSuccess) {
+            *ms_host = (double)t;
+            rc = RT_OK;
+        }
+    }
+    if (e0) cudaEventDestroy(e0);
+    if (e1) cudaEventDestroy(e1);
+    cudaFree(sink);
+    return rc;
 }

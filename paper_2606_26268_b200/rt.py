@@ -77,6 +77,7 @@ _SIGNATURES = {
     "rt_set_tuning": (C.c_int32, [C.c_void_p, C.c_int32, C.c_int32]),
     "rt_set_profiling": (C.c_int32, [C.c_void_p, C.c_int32]),
     "rt_get_kernel_times": (C.c_int32, [C.c_void_p, _dp, C.POINTER(C.c_int64)]),
+    "rt_measure_fp64": (C.c_int32, [C.c_void_p, C.c_int32, C.c_int32, C.c_int32, C.c_int32, _dp]),
     "rt_last_error": (C.c_char_p, [C.c_void_p]),
 }
 
@@ -151,6 +152,19 @@ def opacity_from_spec(spec):
         return make_power_law(spec["kappa0"], spec["a"], spec["b"], spec["rho0"], spec["T0"], spec["kmin"],
                               spec["kmax"])
     return make_table(spec["log10_kappa"], spec["lrho_range"], spec["lT_range"], spec["rho_unit"], spec["T_unit"])
+
+
+def measure_fp64(blocks, threads, chains, iters, device="cuda:0"):
+    """rt_measure_fp64: milliseconds of one launch of the DFMA-chain microbenchmark and its thread-instruction count"""
+    if not torch.cuda.is_available():
+        raise RuntimeError("no CUDA device: paper_2606_26268_b200 has no CPU path")
+    ms = C.c_double()
+    with torch.cuda.device(torch.device(device)):
+        st = torch.cuda.current_stream()
+        rc = lib().rt_measure_fp64(C.c_void_p(st.cuda_stream), int(blocks), int(threads), int(chains), int(iters), C.byref(ms))
+    if rc != OK:
+        raise RtError("rt_measure_fp64", rc)
+    return ms.value, float(blocks) * threads * chains * 8 * iters
 
 
 class Grid:

@@ -403,27 +403,50 @@ def test_spherical_1d_free_streaming_steady_state_is_inverse_square(golden):
 
 # ----------------------------------------------------------------------------- the paper's shock tubes (Sect. 3.1)
 def _rk2_tube(left, right, N, t_end, cfl):
-    """RK2 = two Euler sub-steps averaged; opacities zero (L244)."""
-    g = cart((N, 1, 1), L=(40.0, 1, 1), x0=(-20.0, 0, 0), bc=(1,) * 6)
-    g.set_params(ort.make_params(chat=1.0, E_floor=1e-30))
-    x = 0.5 * (g.xf[0][1:] + g.xf[0][:-1])
-    U = [g.zeros() for _ in range(4)]
-    for q in range(4):
-        U[q][g.interior] = np.where(x < 0, left[q], right[q])[None, None, :]
-    rho, T = np.ones(g.shape), np.ones(g.shape)
-    U1 = [a.copy() for a in U]
-    U2 = [a.copy() for a in U]
-    t = 0.0
-    while t < t_end - 1e-12:
-        dt = min(g.cfl_dt(U, cfl), t_end - t)
-        g.explicit_step(dt, rho, T, U, U1)
-        g.implicit_step(dt, rho, T, None, U1)
-        g.explicit_step(dt, rho, T, U1, U2)
-        g.implicit_step(dt, rho, T, None, U2)
-        for q in range(4):
-            U[q][g.interior] = 0.5 * (U[q][g.interior] + U2[q][g.interior])
-        t += dt
-    return x, [a[g.interior][0, 0] for a in U]
+    """the paper's tubes through the oracle's own RK2 driver ort.run_rk2 (two Euler sub-steps averaged, PAPER.md:L107,
+    L256); opacities zero (L244), so the implicit half only applies the floor / f <= 1 clip."""
+    n = (N, 1, 1)
+    xf = [np.linspace(-20.0, 20.0, N + 1), np.array([0.0, 1.0]), np.array([0.0, 1.0])]
+    x = 0.5 * (xf[0][1:] + xf[0][:-1])
+    U = [W.embed(n, np.where(x < 0, left[q], right[q]).reshape(1, 1, N)) for q in range(4)]
+    w = W.Workload(name="tube", geometry=W.CARTESIAN, n=n, xf=xf, bc=(W.BC_OUTFLOW,) * 6,
+                   params=W.default_params(chat=1.0, E_floor=1e-30), opacities={}, U=U,
+                   rho=W.embed(n, 1.0, fill=1.0), T=W.embed(n, 1.0, fill=1.0), cfl=cfl)
+    g = ort.grid_from_workload(w)
+    Uo, _, _, dts = ort.run_rk2(g, w, None, t_end=t_end)
+    assert sum(dts) == pytest.approx(t_end, rel=1e-12)
+    return x, [a[g.interior][0, 0] for a in Uo]
+
+
+def test_rk2_driver_is_second_order_in_time_and_its_stages_share_one_dt():
+    """ort.run_rk2 = Heun's method on the semi-discrete transport operator (PAPER.md:L107 "a second-order Runge-Kutta";
+    L256): on a FIXED grid, halving the time step (through the Courant number) must cut the difference to a
+    small-time-step reference by 4, where a single Euler stage, an average taken with a re-evaluated dt, or a missing
+    average would give 2.  Smooth f << 1 wave, transport only (no opacity)."""
+    N = 64
+    n = (N, 1, 1)
+    xf = [np.linspace(0.0, 1.0, N + 1), np.array([0.0, 1.0]), np.array([0.0, 1.0])]
+    x = 0.5 * (xf[0][1:] + xf[0][:-1])
+    E0 = 1.0 + 0.2 * np.sin(2 * np.pi * x)
+    F0 = 0.05 * np.cos(2 * np.pi * x)
+
+    def run(cfl):
+        U = [W.embed(n, E0.reshape(1, 1, N)), W.embed(n, F0.reshape(1, 1, N)), W.embed(n, 0.0), W.embed(n, 0.0)]
+        w = W.Workload(name="wave", geometry=W.CARTESIAN, n=n, xf=xf, bc=(W.BC_PERIODIC,) * 2 + (W.BC_OUTFLOW,) * 4,
+                       params=W.default_params(chat=1.0, solver=W.SOLVER_GLF, E_floor=1e-30), opacities={}, U=U,
+                       rho=W.embed(n, 1.0, fill=1.0), T=W.embed(n, 1.0, fill=1.0), cfl=cfl)
+        g = ort.grid_from_workload(w)
+        t_end = 0.5
+        Uo, _, _, dts = ort.run_rk2(g, w, None, t_end=t_end)
+        return Uo[0][g.interior][0, 0]
+
+    # GLF: alpha = chat whatever the state, and the CFL rate varies by < 1e-2 over the run: dt ~ cfl dx / max lambda
+    # (measured: RK2 1.0e-4, 2.6e-5, 6.5e-6 -> ratios 3.95, 3.91; one Euler stage per step gives 1.1e-3, 5.0e-4, 2.3e-4)
+    ref = run(0.00625)
+    e1 = np.abs(run(0.4) - ref).max()
+    e2 = np.abs(run(0.2) - ref).max()
+    e3 = np.abs(run(0.1) - ref).max()
+    assert 3.5 < e1 / e2 < 4.5 and 3.5 < e2 / e3 < 4.5 and e1 < 2e-4, (e1, e2, e3)
 
 
 def _lambda2_and_Pi(E, Fx, Fy):
