@@ -492,21 +492,28 @@ static void launch_sweep(rt_grid* g, int d, bool hll, bool thick, bool curvi, co
 // with_kp: also write rho kappa_P per cell into g->kpr (fused sub-step: the implicit half then evaluates no opacity)
 static int32_t launch_thick_limit(rt_grid* g, const double* rho, const double* T, bool with_kp = false) {
     const GridDev& D = g->dev;
-    if (!g->lim) RT_CUDA(g, cudaMalloc(&g->lim, (size_t)D.ntot * sizeof(double)));
-    if (with_kp && !g->kpr) RT_CUDA(g, cudaMalloc(&g->kpr, (size_t)D.ntot * sizeof(double)));
-    // block width (<= 128, a multiple of 32) that wastes the fewest lanes on a row of nt1 cells: 260 -> 96 (3 x 96 = 288)
-    int bx = 128;
+    // ghosts the kernel never writes (beyond the first face-normal layer) are never used either: zero them once
+    if (!g->lim) {
+        RT_CUDA(g, cudaMalloc(&g->lim, (size_t)D.ntot * sizeof(double)));
+        RT_CUDA(g, cudaMemsetAsync(g->lim, 0, (size_t)D.ntot * sizeof(double), g->stream));
+    }
+    if (with_kp && !g->kpr) {
+        RT_CUDA(g, cudaMalloc(&g->kpr, (size_t)D.ntot * sizeof(double)));
+        RT_CUDA(g, cudaMemsetAsync(g->kpr, 0, (size_t)D.ntot * sizeof(double), g->stream));
+    }
+    // block width (<= 256, a multiple of 32) that wastes the fewest lanes on a row of n1 cells
+    int bx = 256;
     {
         long long best = -1;
-        for (int cand = 128; cand >= 64; cand -= 32) {
-            const long long lanes = (long long)((D.nt[0] + cand - 1) / cand) * cand;
+        for (int cand = 256; cand >= 64; cand -= 32) {
+            const long long lanes = (long long)((D.n[0] + cand - 1) / cand) * cand;
             if (best < 0 || lanes < best) {
                 best = lanes;
                 bx = cand;
             }
         }
     }
-    dim3 grid((D.nt[1] + kThickRows - 1) / kThickRows, D.nt[2]);
+    dim3 grid((D.n[0] + bx - 1) / bx, (D.n[1] + kThickRows - 1) / kThickRows, D.n[2]);
     {
         ProfScope ps(g, RT_K_THICK);
         const OpacDev &oP = g->opac[RT_OPAC_PLANCK], &oR = g->opac[RT_OPAC_ROSSELAND], &oS = g->opac[RT_OPAC_SCATTER];
@@ -514,12 +521,25 @@ static int32_t launch_thick_limit(rt_grid* g, const double* rho, const double* T
         const int m3[3] = {RT_OPAC_PLANCK, RT_OPAC_ROSSELAND, RT_OPAC_SCATTER};
         const OpacSet os = with_kp ? opac_set(g, m3, 3) : opac_set(g, m2, 2);
         bool lean = oR.set && oR.kind == 0 && oR.fast && !oS.set;
-        if (with_kp) lean = lean && (g->same_PR || (oP.set && oP.kind == 0 && oP.fast));
+        const bool second = with_kp && !g->same_PR;
+        if (second) lean = lean && oP.set && oP.kind == 0 && oP.fast && oP.irho0 == oR.irho0 && oP.iT0 == oR.iT0;
         double* kpr = with_kp ? g->kpr : nullptr;
+        LeanLaws L;
+        memset(&L, 0, sizeof(L));
+        if (lean) {
+            L.irho0 = oR.irho0;
+            L.iT0 = oR.iT0;
+            L.two = second ? 1 : 0;
+            L.k0[0] = oR.kappa0; L.kmin[0] = oR.kmin; L.kmax[0] = oR.kmax; L.na[0] = oR.n2a; L.nb[0] = oR.n2b;
+            if (second) {
+                L.k0[1] = oP.kappa0; L.kmin[1] = oP.kmin; L.kmax[1] = oP.kmax; L.na[1] = oP.n2a; L.nb[1] = oP.n2b;
+                L.same_ab = (oP.n2a == oR.n2a && oP.n2b == oR.n2b) ? 1 : 0;
+            }
+        }
         if (lean)
-            k_thick_limit<true><<<grid, bx, 0, g->stream>>>(D, oR, oS, os, rho, T, g->lim, oP, g->same_PR, kpr);
+            k_thick_limit<true><<<grid, bx, 0, g->stream>>>(D, oR, oS, os, rho, T, g->lim, oP, g->same_PR, kpr, L);
         else
-            k_thick_limit<false><<<grid, bx, 0, g->stream>>>(D, oR, oS, os, rho, T, g->lim, oP, g->same_PR, kpr);
+            k_thick_limit<false><<<grid, bx, 0, g->stream>>>(D, oR, oS, os, rho, T, g->lim, oP, g->same_PR, kpr, L);
     }
     RT_LAUNCH_CHECK(g);
     return RT_OK;

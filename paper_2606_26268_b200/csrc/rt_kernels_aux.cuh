@@ -377,72 +377,153 @@ __device__ __forceinline__ double opacity_eval_shared(const OpacDev& o, double r
 }
 
 // ------------------------------------------------------------------------------------------------
-// Thick-limit pre-pass (Eq. 25-26; R-G7): per ghosted cell
+// Thick-limit pre-pass (Eq. 25-26; R-G7): per interior cell
 //   limd = 4 / (3 tau_cell),  tau_cell = rho chi dx,  chi = kappa_R + sigma (L89),
 //   dx = the cell's largest physical extent over the active dimensions.
-// Ghost cells take the value of the periodic image or of the nearest interior cell, so rho and T
-// ghosts are never read.  The sweeps use lim_face = max(limd_a, limd_b) = 4/(3 min(tau_a, tau_b)).
+// The sweeps use lim_face = max(limd_a, limd_b) = 4/(3 min(tau_a, tau_b)) of the two cells next to a face, so of the
+// ghost layers only the first, face-normal one is ever used: the thread of a boundary cell also writes that ghost
+// (the periodic image, or the copy of the nearest interior cell: rho and T ghosts are never read).  The remaining
+// ghosts of the array keep the zeros of its allocation.
 // ------------------------------------------------------------------------------------------------
-constexpr int kThickRows = 4;  // x2 rows per block: ~200 k one-cell blocks cost more to schedule than to run
-// LEAN: chi is ONE half-integer power law (kappa_R fast, no scattering): its scalars live in registers
-// kpr != nullptr (fused sub-step): the pre-pass also hands rho kappa_P of every cell to the implicit half, so that
-// the fused kernel carries no opacity evaluation at all; oP / same_PR describe kappa_P (same_PR: kappa_P is the
-// same law as kappa_R and costs nothing extra).
+constexpr int kThickRows = 4;  // x2 rows per block: one-row blocks cost more to schedule than to run
+
+// x^(N/2) for a compile-time N: straight-line code, one reciprocal for N < 0, one square root for odd N
+template <int N>
+__device__ __forceinline__ double pow_half_ct(double x) {
+    if (N == 0) return 1.0;
+    constexpr int M = N < 0 ? -N : N;
+    const double b = N < 0 ? frcp(x) : x;
+    double r = 1.0;
+    if (M >> 1) {
+        r = b;                      // b^(M >> 1) by repeated squaring, unrolled at compile time
+        constexpr int K = M >> 1;
+        double acc = 1.0, base = b;
+        bool first = true;
+#pragma unroll
+        for (int bit = 0; bit < 3; ++bit) {
+            if (K & (1 << bit)) {
+                acc = first ? base : acc * base;
+                first = false;
+            }
+            if ((K >> (bit + 1)) != 0) base = base * base;
+        }
+        r = acc;
+    }
+    if (M & 1) {
+        const double root = N < 0 ? fsqrt(x) * b : fsqrt(x);
+        r = (M >> 1) ? r * root : root;
+    }
+    return r;
+}
+
+// x^(n/2) for a LAUNCH-UNIFORM -15 <= n <= 15: one uniform multi-way branch into the straight-line code of that
+// exponent.  (Binary powering behind run-time tests of n cost the pre-pass ~280 instructions per cell, most of them
+// selects and moves; this form costs the branch.)  ~1-2 ulp against libm pow().
+__device__ __forceinline__ double pow_half_uniform(double x, int n) {
+    switch (n) {
+#define RT_PH(N) case N: return pow_half_ct<N>(x);
+        RT_PH(-15) RT_PH(-14) RT_PH(-13) RT_PH(-12) RT_PH(-11) RT_PH(-10) RT_PH(-9) RT_PH(-8) RT_PH(-7) RT_PH(-6) RT_PH(-5)
+        RT_PH(-4) RT_PH(-3) RT_PH(-2) RT_PH(-1) RT_PH(1) RT_PH(2) RT_PH(3) RT_PH(4) RT_PH(5) RT_PH(6) RT_PH(7) RT_PH(8)
+        RT_PH(9) RT_PH(10) RT_PH(11) RT_PH(12) RT_PH(13) RT_PH(14) RT_PH(15)
+#undef RT_PH
+        default: return 1.0;
+    }
+}
+
+// One or two half-integer power laws kappa0 (rho/rho0)^(na/2) (T/T0)^(nb/2) clipped to [kmin, kmax] (L299) that share
+// rho0 and T0; exponents launch-uniform, prepared on the host.
+struct LeanLaws {
+    double irho0, iT0;
+    double k0[2], kmin[2], kmax[2];
+    int na[2], nb[2];  // 2a, 2b (|.| <= 15)
+    int two;           // evaluate the second law (kappa_P) as well
+    int same_ab;       // the second law has the exponents of the first (only kappa0 / the clip differ)
+};
+__device__ __forceinline__ void lean_eval(const LeanLaws& L, double rho, double T, double& k_first, double& k_second) {
+    const double xr = rho * L.irho0, xt = T * L.iT0;
+    const double m0 = pow_half_uniform(xr, L.na[0]) * pow_half_uniform(xt, L.nb[0]);
+    k_first = dmin(dmax(L.k0[0] * m0, L.kmin[0]), L.kmax[0]);
+    k_second = k_first;
+    if (L.two) {
+        const double m1 = L.same_ab ? m0 : pow_half_uniform(xr, L.na[1]) * pow_half_uniform(xt, L.nb[1]);
+        k_second = dmin(dmax(L.k0[1] * m1, L.kmin[1]), L.kmax[1]);
+    }
+}
+
+// LEAN: chi is ONE half-integer power law (kappa_R fast, no scattering) and kappa_P, when asked for (kpr != nullptr:
+// the fused sub-step, whose implicit half then evaluates no opacity at all), is the same law or another fast law with
+// the same rho0, T0.  Otherwise the general evaluation (tables share their log10 inputs: OpacSet).
+// One thread per x1 column of a block of kThickRows x2 rows; the loads of the next row are issued before the
+// arithmetic of the current one.
 template <bool LEAN>
-__global__ void __launch_bounds__(128) k_thick_limit(const __grid_constant__ GridDev g, const __grid_constant__ OpacDev oR,
+__global__ void __launch_bounds__(256) k_thick_limit(const __grid_constant__ GridDev g, const __grid_constant__ OpacDev oR,
                                                      const __grid_constant__ OpacDev oS, const __grid_constant__ OpacSet os,
                                                      const double* __restrict__ rho, const double* __restrict__ T,
                                                      double* __restrict__ lim, const __grid_constant__ OpacDev oP,
-                                                     int same_PR, double* __restrict__ kpr) {
-    const int kk = blockIdx.y;
-    int c2 = kk - g.gh[2];
-    if (c2 < 0) c2 = (g.bc[4] == 0) ? c2 + g.n[2] : 0;
-    else if (c2 >= g.n[2]) c2 = (g.bc[4] == 0) ? c2 - g.n[2] : g.n[2] - 1;
+                                                     int same_PR, double* __restrict__ kpr, const __grid_constant__ LeanLaws laws) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int k = blockIdx.z;
+    if (i >= g.n[0]) return;
     const bool share = os.share != 0;
-    const double k0 = oR.kappa0, ir0 = oR.irho0, it0 = oR.iT0, kmin = oR.kmin, kmax = oR.kmax;
-    const int na = oR.n2a, nb = oR.n2b;
-    const double* __restrict__ len0[3] = {g.len[0][0], g.len[1][0], g.len[2][0]};
-    const int gh0 = g.gh[0], n0 = g.n[0], nt0 = g.nt[0];
-    const bool per0 = g.bc[0] == 0;
-    for (int jr = 0; jr < kThickRows; ++jr) {
-        const int jj = blockIdx.x * kThickRows + jr;
-        if (jj >= g.nt[1]) break;
-        int c1 = jj - g.gh[1];
-        if (c1 < 0) c1 = (g.bc[2] == 0) ? c1 + g.n[1] : 0;
-        else if (c1 >= g.n[1]) c1 = (g.bc[2] == 0) ? c1 - g.n[1] : g.n[1] - 1;
-        // rows are block-uniform: 64-bit row bases once, 32-bit offsets along x1
-        const long long srow = (c1 + g.gh[1]) * g.stride[1] + (c2 + g.gh[2]) * g.stride[2];
-        const double* __restrict__ rrow = rho + srow;
-        const double* __restrict__ trow = T + srow;
-        double* __restrict__ lrow = lim + jj * g.stride[1] + kk * g.stride[2];
-        double* __restrict__ krow = kpr ? kpr + jj * g.stride[1] + kk * g.stride[2] : nullptr;
-        double l12[3];  // the x2 and x3 factors of the three cell lengths (0 for an inactive direction)
+    const int s1 = (int)g.stride[1], s2 = (int)g.stride[2];
+    const int n0 = g.n[0], n1 = g.n[1], n2 = g.n[2];
+    const bool act1 = g.gh[1] > 0, act2 = g.gh[2] > 0;
+    // x1 and x3 factors of the three cell lengths (0 for an inactive direction)
+    double l02[3];
 #pragma unroll
-        for (int d = 0; d < 3; ++d) l12[d] = g.gh[d] > 0 ? __ldg(g.len[d][1] + c1) * __ldg(g.len[d][2] + c2) : 0.0;
-        for (int ii = threadIdx.x; ii < nt0; ii += blockDim.x) {
-            int c0 = ii - gh0;
-            if (c0 < 0) c0 = per0 ? c0 + n0 : 0;
-            else if (c0 >= n0) c0 = per0 ? c0 - n0 : n0 - 1;
-            const double r = __ldg(rrow + c0 + gh0), t = __ldg(trow + c0 + gh0);
-            double chi, kP = 0.0;
-            if (LEAN) {
-                chi = power_law_fast_v(k0, ir0, it0, na, nb, kmin, kmax, r, t);
-                if (kpr) kP = same_PR ? chi : power_law_fast(oP, r, t);
-            } else {
-                LogRT l = {0.0, 0.0};
-                if (share) l = log_inputs(os.src == RT_OPAC_SCATTER_IDX ? oS : (os.src == 1 ? oR : oP), r, t);
-                const double kR = opacity_eval_shared(oR, r, t, share, l);
-                chi = kR + opacity_eval_shared(oS, r, t, share, l);
-                if (kpr) kP = same_PR ? kR : opacity_eval_shared(oP, r, t, share, l);
-            }
-            if (kpr) krow[ii] = kP * r;
-            double dx = 0.0;
-#pragma unroll
-            for (int d = 0; d < 3; ++d)
-                dx = dmax(dx, __ldg(len0[d] + c0) * l12[d]);
-            const double tau = r * chi * dx;
-            // any value >= 1 means "no limit" (|lambda| <= 1, L167): tau -> 0 maps to +inf without a division by zero
-            lrow[ii] = tau > 1.0e-100 ? 4.0 * frcp(3.0 * tau) : __builtin_huge_val();
+    for (int d = 0; d < 3; ++d) l02[d] = g.gh[d] > 0 ? __ldg(g.len[d][0] + i) * __ldg(g.len[d][2] + k) : 0.0;
+    // face-normal ghost this cell also fills along x1 / x3 (offset 0: none): the periodic image or the clamped copy
+    int goff0 = 0, goff2 = 0;
+    if (g.gh[0] > 0) {
+        const bool per = g.bc[0] == 0;
+        if (i == 0) goff0 = per ? n0 : -1;
+        if (i == n0 - 1) goff0 = per ? -n0 : 1;
+    }
+    if (act2) {
+        const bool per = g.bc[4] == 0;
+        if (k == 0) goff2 = (per ? n2 : -1) * s2;
+        if (k == n2 - 1) goff2 = (per ? -n2 : 1) * s2;
+    }
+    const bool per1 = g.bc[2] == 0;
+    const int j0 = blockIdx.y * kThickRows;
+    const int j1 = min(j0 + kThickRows, n1);
+    const double* __restrict__ len01 = g.len[0][1];
+    const double* __restrict__ len11 = g.len[1][1];
+    const double* __restrict__ len21 = g.len[2][1];
+    int id = (i + g.gh[0]) + (j0 + g.gh[1]) * s1 + (k + g.gh[2]) * s2;
+    double r = __ldg(rho + id), t = __ldg(T + id);
+#pragma unroll 1
+    for (int j = j0; j < j1; ++j, id += s1) {
+        const double rc = r, tc = t;
+        if (j + 1 < j1) {
+            r = __ldg(rho + id + s1);
+            t = __ldg(T + id + s1);
+        }
+        double chi, kP;
+        if (LEAN) {
+            lean_eval(laws, rc, tc, chi, kP);
+        } else {
+            LogRT l = {0.0, 0.0};
+            if (share) l = log_inputs(os.src == RT_OPAC_SCATTER_IDX ? oS : (os.src == 1 ? oR : oP), rc, tc);
+            const double kR = opacity_eval_shared(oR, rc, tc, share, l);
+            chi = kR + opacity_eval_shared(oS, rc, tc, share, l);
+            kP = !kpr ? 0.0 : (same_PR ? kR : opacity_eval_shared(oP, rc, tc, share, l));
+        }
+        if (kpr) kpr[id] = kP * rc;
+        double dx = l02[0] * __ldg(len01 + j);
+        if (act1) dx = dmax(dx, l02[1] * __ldg(len11 + j));
+        if (act2) dx = dmax(dx, l02[2] * __ldg(len21 + j));
+        const double tau = rc * chi * dx;
+        // any value >= 1 means "no limit" (|lambda| <= 1, L167): tau -> 0 maps to +inf without a division by zero
+        const double v = tau > 1.0e-100 ? 4.0 * frcp(3.0 * tau) : __builtin_huge_val();
+        lim[id] = v;
+        if (goff0 | goff2) {
+            if (goff0) lim[id + goff0] = v;
+            if (goff2) lim[id + goff2] = v;
+        }
+        if (act1 && (j == 0 || j == n1 - 1)) {
+            if (j == 0) lim[id + (per1 ? n1 : -1) * s1] = v;
+            if (j == n1 - 1) lim[id + (per1 ? -n1 : 1) * s1] = v;
         }
     }
 }
@@ -470,7 +551,7 @@ __device__ __forceinline__ double cell_rate_il(double chat, double E, double F1,
     for (int d = 0; d < 3; ++d) {
         const double b = c.gE * F[d];
         const double z2 = (2.0 * c.dE) * fma(-b, F[d], c.sE);
-        const double z = fsqrt(dmax(z2, kTiny));
+        const double z = fsqrt(fabs(z2) + kTiny);  // see flux_and_speeds
         sum = fma((fabs(F[d]) + z) * c.rsE, il[d], sum);
     }
     return sum * chat;

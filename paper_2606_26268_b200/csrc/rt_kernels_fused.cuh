@@ -160,7 +160,18 @@ __global__ void __launch_bounds__(FNT, FUSED_MINB)
                                                         // that face on the way back down
     unsigned long long* const mbar = (unsigned long long*)(yex + FNST * FNT);  // [FNSLOT]
 
-    const int lx = threadIdx.x, ly = threadIdx.y;
+#ifndef FUSED_ROWSHIFT
+#define FUSED_ROWSHIFT 1
+#endif
+    // Row -> warp map.  Rows 0 and FTY-1 carry the extra edge work of the tile; warp w issues on SM sub-partition w % 4.
+    // Half of the CTAs shift their rows by two warps so that, of two CTAs resident on one SM, the four heavier warps
+    // land on four different sub-partitions instead of two.
+    const int lx = threadIdx.x;
+#if FUSED_ROWSHIFT == 1
+    const int ly = (threadIdx.y + 2 * ((blockIdx.x + blockIdx.y + blockIdx.z) & 1)) % FNY;
+#else
+    const int ly = threadIdx.y;
+#endif
     const int tid = ly * 32 + lx;
     const int i0 = blockIdx.x * FTX, j0 = blockIdx.y * FTY;
     const int ka = blockIdx.z * seglen;

@@ -39,28 +39,34 @@ __device__ __forceinline__ double frcp(double x) {
     return fma(r, t, r);
 }
 
-// s = sqrt(x) and rs = 1/sqrt(x) together (one third-order coupled step + residual step, 8 fp64 ops + 1 for rs;
-// measured on B200 over 2^30 inputs: s correctly rounded, rs <= 1.3 ulp).
-__device__ __forceinline__ void fsqrt_rsqrt(double x, double& s, double& rs) {
-    double y = rsqrt_seed(x);
-    double g = x * y, h = 0.5 * y;
+// y/2 of a NORMAL positive double whose half is normal too (the MUFU seeds below): one integer subtraction on the
+// exponent field instead of a multiplication in the fp64 pipe, which is the unit this library is short of
+__device__ __forceinline__ double half_of_normal(double y) {
+    return __hiloint2double(__double2hiint(y) - 0x00100000, __double2loint(y));
+}
+
+// s = sqrt(x) and hrs = 1/(2 sqrt(x)) together (one third-order coupled step + residual step, 7 fp64 ops;
+// measured on B200 over 2^30 inputs: s correctly rounded, 2 hrs <= 1.3 ulp).
+__device__ __forceinline__ void fsqrt_hrsqrt(double x, double& s, double& hrs) {
+    const double y = rsqrt_seed(x);
+    double g = x * y, h = half_of_normal(y);
     // one third-order step: with 2t = 1 - x y^2,  1/sqrt(1 - 2t) = 1 + t + 3/2 t^2 + O(t^3)
     const double t = fma(-h, g, 0.5);
     const double p = fma(1.5 * t, t, t);
     g = fma(g, p, g);
     h = fma(h, p, h);
-    // residual step: makes s exact for perfect squares (x = E^2 at f = 1 gives s = E, hence
+    // residual step: makes s exact for perfect squares (x = E^2/4 at f = 1 gives s = E/2, hence
     // (1 - xi)/2 = 0 and zeta = 0 exactly: the lambda -> cos(theta) limit of L167)
     const double d = fma(-g, g, x);
     s = fma(d, h, g);
-    rs = h + h;
+    hrs = h;
 }
 
-// sqrt(x) alone (6 fp64 ops): one third-order step, no residual step (<= ~1 ulp; exactness for perfect squares is
-// not needed where this is used: zeta and the CFL rate); x must be > 0 (callers clamp at a tiny positive number).
+// sqrt(x) alone (5 fp64 ops): one third-order step, no residual step (<= ~1 ulp; exactness for perfect squares is
+// not needed where this is used: zeta and the CFL rate); x must be > 0 (callers add a tiny positive number).
 __device__ __forceinline__ double fsqrt(double x) {
     const double y = rsqrt_seed(x);
-    const double g = x * y, h = 0.5 * y;
+    const double g = x * y, h = half_of_normal(y);
     const double t = fma(-h, g, 0.5);
     const double p = fma(1.5 * t, t, t);
     return fma(g, p, g);
@@ -89,13 +95,17 @@ struct Closure {
 
 // E2 = E*E and F2 = |F|^2 are passed in because the callers have them already.
 // f is capped at 1 (Eq. 14; round-off guard, R-G4): |F|^2 enters as min(F2, E2).
+// The square root is taken of (4 E^2 - 3 |F|^2)/4 = E^2 - 3/4 |F|^2 (the scaling by a power of two commutes with every
+// rounding): sE = 2 sqrt(.), 1/sE = the routine's 1/(2 sqrt(.)) as it stands.
 __device__ __forceinline__ Closure closure_of(double E, double E2, double F2) {
     Closure c;
-    double m = dmin(F2, E2);
-    double w = fma(-3.0, m, 4.0 * E2);
-    fsqrt_rsqrt(w, c.sE, c.rsE);
-    c.gE = 3.0 * frcp(fma(2.0, E, c.sE));
-    c.dE = (c.sE - E) * (1.0 / 3.0);
+    const double m = dmin(F2, E2);
+    const double w = fma(-0.75, m, E2);
+    double hs;
+    fsqrt_hrsqrt(w, hs, c.rsE);
+    c.sE = hs + hs;
+    c.gE = 1.5 * frcp(E + hs);               // 3 / (2E + sE)
+    c.dE = fma(2.0, hs, -E) * (1.0 / 3.0);   // (sE - E)/3
     return c;
 }
 
@@ -112,8 +122,11 @@ __device__ __forceinline__ void flux_and_speeds(State& st, double E2, double F2)
     st.G[3] = b * st.U[3];
     st.G[1 + D] += c.dE;
     if (WAVES) {
-        double z2 = (2.0 * c.dE) * fma(-b, Fd, c.sE);  // 2/3 (sE - E)(sE - gE Fd^2)
-        double z = fsqrt(dmax(z2, kTiny));
+        // 2/3 (sE - E)(sE - gE Fd^2) >= 0 up to rounding: it can come out a rounding error below zero only where
+        // sE - E itself is at round-off (f = 1 to the last bits), and it is exactly 0 for f = 1 exactly; |.| + tiny keeps
+        // the square root's argument positive with ONE fp64 operation (a max costs a compare and a chain of selects)
+        const double z2 = (2.0 * c.dE) * fma(-b, Fd, c.sE);
+        const double z = fsqrt(fabs(z2) + kTiny);
         st.lm = (Fd - z) * c.rsE;
         st.lp = (Fd + z) * c.rsE;
     } else {
@@ -130,18 +143,17 @@ __device__ __forceinline__ double half_slope(double dm, double dp) {
 }
 
 // f-preserving face state (Eq. 19-21; R-G4).  Uc = cell value, invEc = 1/E_c,
-// Ec2 = E_c^2, F2c = |F_c|^2; on entry st.U holds the reconstructed R(U); on exit the face state.
-// Returns through E2f/F2f the squares of the final face state.
-__device__ __forceinline__ void fpreserve(State& st, const double Uc[4], double invEc, double Ec2, double F2c,
+// Ec2 = E_c^2, F2c = |F_c|^2; on entry st.U holds the reconstructed R(U) = Uc + sh (sh = the signed half slope, of
+// which dE = sh[0] is passed in); on exit the face state.  Returns through E2f/F2f the squares of the final face state.
+__device__ __forceinline__ void fpreserve(State& st, const double Uc[4], double dE, double invEc, double Ec2, double F2c,
                                           double& E2f, double& F2f) {
     const double Ef = st.U[0];
     E2f = Ef * Ef;
     double F2r = fma(st.U[3], st.U[3], fma(st.U[2], st.U[2], st.U[1] * st.U[1]));
     bool keep = (F2r <= E2f) && (F2r * Ec2 > F2c * E2f);
-    // quotient with one residual step: correctly rounded, so E_f = E_c gives r = 1 EXACTLY and a
-    // cell with f = 1 and zero slopes keeps f_face = 1 exactly (the zeta = 0 limit, L167)
-    double r = Ef * invEc;
-    r = fma(fma(-Uc[0], r, Ef), invEc, r);
+    // E_f/E_c = 1 + dE/E_c in ONE operation (E_f = E_c + dE up to its own rounding: 1-2 ulp on the quotient): a zero
+    // slope gives r = 1 EXACTLY, so a cell with f = 1 and zero slopes keeps f_face = 1 exactly (the zeta = 0 limit, L167)
+    const double r = fma(dE, invEc, 1.0);
     st.U[1] = keep ? st.U[1] : Uc[1] * r;
     st.U[2] = keep ? st.U[2] : Uc[2] * r;
     st.U[3] = keep ? st.U[3] : Uc[3] * r;
@@ -196,6 +208,13 @@ __device__ __forceinline__ void riemann(const State& L, const State& R, double l
         sR = dmax(dmin(1.0, limd), kTinySpeed);  // GLF: alpha = min(chat, 4 chat/(3 tau))
         sL = -sR;
     }
+    if (!HLL) {
+        // alpha = sR = -sL: 1/2 (G_L + G_R) - 1/2 alpha (U_R - U_L) as it is written (L150), no reciprocal
+        const double ha = 0.5 * sR;
+#pragma unroll
+        for (int q = 0; q < 4; ++q) flux[q] = fma(-ha, R.U[q] - L.U[q], 0.5 * (L.G[q] + R.G[q]));
+        return;
+    }
     const double rden = frcp(sR - sL);
     const double sRL = sR * sL;
 #pragma unroll
@@ -225,7 +244,7 @@ __device__ __forceinline__ void cell_faces(const double q0[4], const double dm[4
 #pragma unroll
         for (int q = 0; q < 4; ++q) lo.U[q] = q0[q] - h[q];
         double E2f, F2f;
-        if (fix == 0) fpreserve(lo, q0, invEc, Ec2, F2c, E2f, F2f);
+        if (fix == 0) fpreserve(lo, q0, -h[0], invEc, Ec2, F2c, E2f, F2f);
         else facefix_variant(fix, lo, q0, Ec2, F2c, E2f, F2f);
         flux_and_speeds<D, HLL>(lo, E2f, F2f);
     }
@@ -233,7 +252,7 @@ __device__ __forceinline__ void cell_faces(const double q0[4], const double dm[4
 #pragma unroll
         for (int q = 0; q < 4; ++q) hi.U[q] = q0[q] + h[q];
         double E2f, F2f;
-        if (fix == 0) fpreserve(hi, q0, invEc, Ec2, F2c, E2f, F2f);
+        if (fix == 0) fpreserve(hi, q0, h[0], invEc, Ec2, F2c, E2f, F2f);
         else facefix_variant(fix, hi, q0, Ec2, F2c, E2f, F2f);
         flux_and_speeds<D, HLL>(hi, E2f, F2f);
     }
