@@ -10,8 +10,13 @@
 // stencil value is read from HBM/L2 once per CTA, the loads occupy no registers and no issue slots, and
 // boxes hanging over the array edge are zero-filled by the hardware.  Arrays the TMA cannot address
 // (odd x1 extent => row pitch not a multiple of 16 B, or a base pointer not 16-B aligned) take an
-// 8-byte cp.async loop instead.  Thread (lx, ly) owns cell (i0-1+lx, j0+ly): lanes 0 and 31 are the x1 halo
-// whose face states the tile's outer x1 faces need.  Per plane c, every thread:
+// 8-byte cp.async loop instead.  Thread (lx, ly) owns cell (i0+lx, j0+ly): every lane owns an output cell.  The
+// fluxes through the two OUTER x1 faces of a row (lower face of lane 0, upper face of lane 31) need the face states of
+// the cells i0-1 and i0+32: the 2 x FTY such faces of a plane are one half-filled warp task ("edge task": both face
+// states + Riemann flux of the face), done one step ahead by the warp whose turn it is (rows take turns, so the extra
+// work averages out) and handed over through shared memory.  That costs 3.6 % more warp instructions than the rows
+// alone; halo lanes (30 useful lanes of 32, and a ragged ninth tile on a 256-cell row) cost 12.5 %.
+// Per plane c, every thread:
 //   Z  : both x3 face states of cell c (Eq. 17-21 + closure + speeds), Riemann flux at face c-1/2 against
 //        the upper-face state of cell c-1 kept in this thread's shared-memory slot;
 //   FIN: cell c-1 is complete: U* = acc - dt/V [A F]_z, then floor/clip, opacities, implicit coupling
@@ -24,9 +29,9 @@
 //        it up one plane later (after the per-plane __syncthreads).  The bottom row builds the upper-face state
 //        of the cell below the tile itself, the top row the lower-face state of the cell above and that flux.
 //   acc = U^n - dt/V([AF]_x + [AF]_y) + dt S_geo.
-// One __syncthreads per plane, no idle warps.  Every closure, wave speed and Riemann flux is evaluated once per
-// face inside the tile; the halo costs 32/30 in x1 and one extra face state + flux per edge row in x2.  Face
-// states, fluxes and U* never touch HBM.
+// One __syncthreads per plane, no idle warps, no idle lanes.  Every closure, wave speed and Riemann flux is evaluated
+// once per face inside the tile; the tile boundary costs the edge task in x1 and one extra face state + flux per edge
+// row in x2.  Face states, fluxes and U* never touch HBM.
 #pragma once
 #include <cuda.h>  // CUtensorMap (type only: the encoder is fetched through cudaGetDriverEntryPoint)
 
@@ -34,12 +39,13 @@
 
 namespace rtm1 {
 
-constexpr int FTX = 30;           // output cells per CTA along x1 (32 lanes, 1 halo lane each side)
+constexpr int FTX = 32;           // output cells per CTA along x1 = lanes: no halo lanes (the fluxes through the two outer
+                                  // x1 faces of a row come from the edge task below)
 constexpr int FTY = 8;            // output cells per CTA along x2 = thread rows (no halo rows: rows 0 and FTY-1
                                   // build the face states of the cells below / above the tile themselves)
 constexpr int FNY = FTY;          // thread rows
 constexpr int FNT = 32 * FNY;     // threads per CTA
-constexpr int FPW = 34;           // staged plane width  (cells i0-2 .. i0+31)
+constexpr int FPW = FTX + 4;      // staged plane width  (cells i0-2 .. i0+33)
 constexpr int FPH = FTY + 4;      // staged plane height (cells j0-2 .. j0+FTY+1)
 constexpr int FPHW = FPW * FPH;
 constexpr int FPS = (FPHW + 15) / 16 * 16;  // doubles between staged arrays: every TMA destination 128-B aligned
@@ -49,9 +55,10 @@ constexpr int FNSLOT = 4;
 #define FUSED_MINB 2
 #endif
 constexpr int FNST = 10;          // doubles of an exchanged face state: U[4], G[4], lm, lp
-// staged planes | zhi[FNST][FNT] | yex[FNST][FNT] | mbarriers
+constexpr int FNEDGE = 2 * FNY;   // x1 edge tasks per plane: (lower, upper) outer face of every row
+// staged planes | zhi[FNST][FNT] | yex[FNST][FNT] | xedge[2][4][FNEDGE] | mbarriers
 constexpr size_t kFusedSmemBytes =
-    sizeof(double) * (size_t)(FNSLOT * FNARR * FPS + 2 * FNST * FNT) + FNSLOT * sizeof(unsigned long long);
+    sizeof(double) * (size_t)(FNSLOT * FNARR * FPS + 2 * FNST * FNT + 2 * 4 * FNEDGE) + FNSLOT * sizeof(unsigned long long);
 static_assert(FTY <= 15, "one named barrier per row pair");
 
 struct FusedArgs {
@@ -158,28 +165,19 @@ __global__ void __launch_bounds__(FNT, FUSED_MINB)
     double* const yex = zhi + FNST * FNT;               // [FNST][FNT] x2 exchange, one slot per thread: its upper x2 face
                                                         // state on the way up, then (components 0-3) the flux through
                                                         // that face on the way back down
-    unsigned long long* const mbar = (unsigned long long*)(yex + FNST * FNT);  // [FNSLOT]
+    double* const xedge = yex + FNST * FNT;             // [2 (plane parity)][4][FNEDGE] area-weighted fluxes through the
+                                                        // outer x1 faces: task t = side * FNY + row
+    unsigned long long* const mbar = (unsigned long long*)(xedge + 2 * 4 * FNEDGE);  // [FNSLOT]
 
-#ifndef FUSED_ROWSHIFT
-#define FUSED_ROWSHIFT 1
-#endif
-    // Row -> warp map.  Rows 0 and FTY-1 carry the extra edge work of the tile; warp w issues on SM sub-partition w % 4.
-    // Half of the CTAs shift their rows by two warps so that, of two CTAs resident on one SM, the four heavier warps
-    // land on four different sub-partitions instead of two.
-    const int lx = threadIdx.x;
-#if FUSED_ROWSHIFT == 1
-    const int ly = (threadIdx.y + 2 * ((blockIdx.x + blockIdx.y + blockIdx.z) & 1)) % FNY;
-#else
-    const int ly = threadIdx.y;
-#endif
+    const int lx = threadIdx.x, ly = threadIdx.y;
     const int tid = ly * 32 + lx;
     const int i0 = blockIdx.x * FTX, j0 = blockIdx.y * FTY;
     const int ka = blockIdx.z * seglen;
     const int kb = min(ka + seglen, g.n[2]);
-    const int i = i0 - 1 + lx, j = j0 + ly;
-    const bool writer = lx >= 1 && lx <= FTX && i < g.n[0] && j < g.n[1];
-    const int ic = min(max(i, 0), g.n[0] - 1), jc = min(j, g.n[1] - 1);
-    const int o = (ly + 2) * FPW + lx + 1;  // this thread's cell inside a staged plane
+    const int i = i0 + lx, j = j0 + ly;
+    const bool writer = i < g.n[0] && j < g.n[1];
+    const int ic = min(i, g.n[0] - 1), jc = min(j, g.n[1] - 1);
+    const int o = (ly + 2) * FPW + lx + 2;  // this thread's cell inside a staged plane
     const bool tma = a.use_tma != 0;
     constexpr bool rus = HLL && RUS;
     const double dt = a.im.dt_dev ? __ldg(a.im.dt_dev) : a.im.dt;
@@ -235,7 +233,7 @@ __global__ void __launch_bounds__(FNT, FUSED_MINB)
     const double kz = HASZ ? dtc * g.cg[2][0][ic] * g.cg[2][1][jc] : 0.0;
     double wx = 1.0, wylo = 1.0, wyhi = 1.0;  // face-area weights of this cell's lower x1 face, lower / upper x2 faces
     if (CURVI) {
-        wx = g.wf[0][min(max(i, 0), g.n[0])];
+        wx = g.wf[0][min(i, g.n[0])];
         wylo = g.wf[1][min(j, g.n[1])];
         wyhi = g.wf[1][min(j + 1, g.n[1])];
     }
@@ -251,6 +249,35 @@ __global__ void __launch_bounds__(FNT, FUSED_MINB)
     int nfloor = 0, nclip = 0;             // cells of this thread whose floor / clip fired
     double rate = 0.0;
 
+    // Edge task of plane cc (staged at pe): lanes 0 .. FNEDGE-1 of the calling warp; task t = side * FNY + row computes
+    // the flux through the lower (side 0: cells i0-1 | i0) or upper (side 1: cells i0+31 | i0+32) outer x1 face of that
+    // row from scratch and leaves it, area-weighted, in xedge[cc & 1].  Faces outside the grid produce unused numbers.
+    auto edge_task = [&](int cc, const double* pe) {
+        if (lx < FNEDGE) {
+            const int row = lx % FNY, side = lx / FNY;
+            const int ob = (row + 2) * FPW + 2 + side * FTX;  // cell b = the upper cell of the face; a = b - 1
+            double qa[4], qb[4], dma[4], dpa[4], dpb[4];
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                qa[q] = pe[q * FPS + ob - 1];
+                qb[q] = pe[q * FPS + ob];
+                dma[q] = qa[q] - pe[q * FPS + ob - 2];
+                dpa[q] = qb[q] - qa[q];
+                dpb[q] = pe[q * FPS + ob + 1] - qb[q];
+            }
+            State loa, hia, lob, hib;
+            cell_faces<0, HLL>(qa, dma, dpa, false, true, loa, hia);
+            cell_faces<0, HLL>(qb, dpa, dpb, true, false, lob, hib);
+            const double limd = THICK ? dmax(pe[4 * FPS + ob - 1], pe[4 * FPS + ob]) : kInf;
+            double fe[4];
+            riemann<HLL>(hia, lob, limd, fe, rus);
+            const double w = CURVI ? g.wf[0][min(i0 + side * FTX, g.n[0])] : 1.0;
+            double* dst = xedge + (cc & 1) * (4 * FNEDGE) + lx;
+#pragma unroll
+            for (int q = 0; q < 4; ++q) dst[q * FNEDGE] = fe[q] * w;
+        }
+    };
+
 #pragma unroll 1
     for (int c = HASZ ? ka - 1 : 0; c <= kb; ++c) {
         if (HASZ || c == 0) {
@@ -259,6 +286,14 @@ __global__ void __launch_bounds__(FNT, FUSED_MINB)
         __syncthreads();  // plane c+1 visible to all; every warp is done with step c-1
         if (HASZ && c + 2 <= kb + 1) load_plane(c + 2);
         const double* pc = planes + ((c + 4) & 3) * (FNARR * FPS);
+        if (HASZ) {
+            // outer x1 faces of plane c+1, consumed by the X phase of the next step (behind its barrier); the buffer
+            // written here was last read in the X phase of step c-1, before this step's barrier
+            if (c + 1 < kb && ly == ((c + 1) & (FNY - 1))) edge_task(c + 1, planes + ((c + 5) & 3) * (FNARR * FPS));
+        } else if (c == 0) {
+            if (ly == 0) edge_task(0, pc);   // 2-D: the only plane; one extra barrier
+            __syncthreads();
+        }
         if (writer && c < kb) {  // inputs of the implicit half of cell c, needed one step from now
             const int idn = id0 + c * zstride;
             prefetch_l2(a.im.rho + idn);
@@ -377,9 +412,12 @@ __global__ void __launch_bounds__(FNT, FUSED_MINB)
                 for (int q = 0; q < 4; ++q) fl[q] *= wx;
             }
             const double cx = kx * g.cg[0][2][c];
+            const double* xe = xedge + (c & 1) * (4 * FNEDGE);
 #pragma unroll
             for (int q = 0; q < 4; ++q) {
-                const double fu = __shfl_down_sync(0xffffffffu, fl[q], 1);
+                if (lx == 0) fl[q] = xe[q * FNEDGE + ly];                    // lower outer face of the row
+                double fu = __shfl_down_sync(0xffffffffu, fl[q], 1);
+                if (lx == 31) fu = xe[q * FNEDGE + FNY + ly];                // upper outer face of the row
                 acc[q] = fma(-cx, fu - fl[q], qc[q]);
             }
             if (CURVI) {
@@ -414,10 +452,17 @@ __global__ void __launch_bounds__(FNT, FUSED_MINB)
             }
             State hi;
             cell_faces<1, HLL, true>(qc, dm, dp, true, true, ylo, hi, invEc, Ec2, F2c);
+#ifdef FUSED_EXP_NOEDGE
+            if (true) {
+                state_store<HLL, FNT>(yex, tid, hi);
+                if (ly < FTY - 1) pair_arrive(1 + ly);
+            } else {
+#else
             if (ly < FTY - 1) {
                 state_store<HLL, FNT>(yex, tid, hi);
                 pair_arrive(1 + ly);
             } else {
+#endif
                 // top row: the lower-face state of the cell above the tile, and the flux through the face between them
                 double qa[4], dma[4], dpa[4];
 #pragma unroll
@@ -438,10 +483,17 @@ __global__ void __launch_bounds__(FNT, FUSED_MINB)
         // ---------------------------------------------------------------- Y: flux through the lower x2 face
         {
             State L;
+#ifdef FUSED_EXP_NOEDGE
+            if (true) {
+                if (ly > 0) pair_sync(ly);
+                state_load<HLL, FNT>(yex, ly > 0 ? tid - 32 : tid, L);
+            } else {
+#else
             if (ly > 0) {
                 pair_sync(ly);  // the row below has stored its upper-face state
                 state_load<HLL, FNT>(yex, tid - 32, L);
             } else {
+#endif
                 // bottom row: the upper-face state of the cell below the tile
                 double qb[4], dmb[4], dpb[4];
 #pragma unroll
