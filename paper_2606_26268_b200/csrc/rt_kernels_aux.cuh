@@ -347,13 +347,13 @@ __device__ __forceinline__ double table_eval(const OpacDev& o, const LogRT& l) {
         const double v00 = __ldg(p), v01 = __ldg(p + 1), v10 = __ldg(p + o.n_lrho), v11 = __ldg(p + o.n_lrho + 1);
         val = (1.0 - tv) * ((1.0 - tu) * v00 + tu * v01) + tv * ((1.0 - tu) * v10 + tu * v11);
     }
-    return exp10(val);
+    return fexp10(val);
 }
 
 __device__ __forceinline__ LogRT log_inputs(const OpacDev& o, double rho, double T) {
     LogRT l;
-    l.lT = log10(T * o.T_unit);
-    l.lrho = o.n_lrho > 1 ? log10(rho * o.rho_unit) : 0.0;
+    l.lT = flog10(T * o.T_unit);
+    l.lrho = o.n_lrho > 1 ? flog10(rho * o.rho_unit) : 0.0;
     return l;
 }
 

@@ -306,11 +306,16 @@ __global__ void __launch_bounds__(FNT, FUSED_MINB)
         }
         // gas state of cell c-1 for FIN: issued here so that the x3 phase hides what is left of its latency
         double rho_f = 1.0, T_f = 1.0, kpr_f = 0.0;
+        double m_f[3] = {0.0, 0.0, 0.0};
         if (writer && c > ka) {
             const int id = id0 + (c - 1) * zstride;
             rho_f = __ldg(a.im.rho + id);
             T_f = a.im.T[id];
             if (THICK) kpr_f = __ldg(a.kpr + id);
+            if (FEEDBACK) {
+#pragma unroll
+                for (int q = 0; q < 3; ++q) m_f[q] = a.im.mom[q][id];
+            }
         }
         double invEc, Ec2, F2c;
         // ---------------------------------------------------------------- Z
@@ -352,11 +357,7 @@ __global__ void __launch_bounds__(FNT, FUSED_MINB)
                 if (writer) {
                     const int id = id0 + (c - 1) * zstride;
                     const double rho = rho_f, T0 = T_f;
-                    double m[3] = {0.0, 0.0, 0.0};
-                    if (FEEDBACK) {
-#pragma unroll
-                        for (int q = 0; q < 3; ++q) m[q] = a.im.mom[q][id];
-                    }
+                    const double m[3] = {m_f[0], m_f[1], m_f[2]};
                     double F[3] = {U4[1], U4[2], U4[3]};
                     const double il[3] = {ilxy[0] * g.ilen[0][2][c - 1], ilxy[1] * g.ilen[1][2][c - 1],
                                           HASZ ? ilxy[2] * g.ilen[2][2][c - 1] : 0.0};
@@ -452,17 +453,10 @@ __global__ void __launch_bounds__(FNT, FUSED_MINB)
             }
             State hi;
             cell_faces<1, HLL, true>(qc, dm, dp, true, true, ylo, hi, invEc, Ec2, F2c);
-#ifdef FUSED_EXP_NOEDGE
-            if (true) {
-                state_store<HLL, FNT>(yex, tid, hi);
-                if (ly < FTY - 1) pair_arrive(1 + ly);
-            } else {
-#else
             if (ly < FTY - 1) {
                 state_store<HLL, FNT>(yex, tid, hi);
                 pair_arrive(1 + ly);
             } else {
-#endif
                 // top row: the lower-face state of the cell above the tile, and the flux through the face between them
                 double qa[4], dma[4], dpa[4];
 #pragma unroll
@@ -483,17 +477,10 @@ __global__ void __launch_bounds__(FNT, FUSED_MINB)
         // ---------------------------------------------------------------- Y: flux through the lower x2 face
         {
             State L;
-#ifdef FUSED_EXP_NOEDGE
-            if (true) {
-                if (ly > 0) pair_sync(ly);
-                state_load<HLL, FNT>(yex, ly > 0 ? tid - 32 : tid, L);
-            } else {
-#else
             if (ly > 0) {
                 pair_sync(ly);  // the row below has stored its upper-face state
                 state_load<HLL, FNT>(yex, tid - 32, L);
             } else {
-#endif
                 // bottom row: the upper-face state of the cell below the tile
                 double qb[4], dmb[4], dpb[4];
 #pragma unroll

@@ -72,6 +72,61 @@ __device__ __forceinline__ double fsqrt(double x) {
     return fma(g, p, g);
 }
 
+// log10(x) and 10^v for the opacity tables (L375; R-G14), written out because the pre-pass and the implicit half were
+// spending most of their issue slots inside the library versions (their polynomial coefficients arrive as pairs of
+// 32-bit immediates: two register moves per coefficient).  Same recipe as any libm, no special cases:
+// x = 2^e m, m in [sqrt(1/2), sqrt(2)), log m = 2 atanh(s), s = (m-1)/(m+1), |s| <= 0.1716, series to s^21/21 (next term
+// < 1e-18); 10^v = 2^n 10^r, n = round(v log2 10), |r| <= 0.1506 (two-piece log10 2), 10^r = exp(r ln 10), Taylor to
+// t^13/13! (next term < 5e-18).  <= ~2 ulp each against libm over the table ranges; x must be positive and normal
+// (zero gives -308, below any table edge, like the -inf of the exact function), |v| < 300.
+__device__ __forceinline__ double flog10(double x) {
+    int hi = __double2hiint(x);
+    int e = (hi >> 20) - 1023;
+    hi = (hi & 0x000fffff) | 0x3ff00000;  // m in [1, 2)
+    if (hi >= 0x3ff6a09f) {                // m > sqrt(2): halve it
+        hi -= 0x00100000;
+        e += 1;
+    }
+    const double m = __hiloint2double(hi, __double2loint(x));
+    const double s = (m - 1.0) * frcp(m + 1.0);
+    const double z = s * s;
+    double p = 1.0 / 21.0;
+    p = fma(p, z, 1.0 / 19.0);
+    p = fma(p, z, 1.0 / 17.0);
+    p = fma(p, z, 1.0 / 15.0);
+    p = fma(p, z, 1.0 / 13.0);
+    p = fma(p, z, 1.0 / 11.0);
+    p = fma(p, z, 1.0 / 9.0);
+    p = fma(p, z, 1.0 / 7.0);
+    p = fma(p, z, 1.0 / 5.0);
+    p = fma(p, z, 1.0 / 3.0);
+    p = fma(p * z, s, s);                                          // s (1 + z/3 + z^2/5 + ...)
+    return fma((double)e, 0.3010299956639812, 0.8685889638065036 * p);  // e log10 2 + (2 / ln 10) atanh s
+}
+__device__ __forceinline__ double fexp10(double v) {
+    const double sh = fma(v, 3.321928094887362, 6755399441055744.0);   // round(v log2 10) in the low word
+    const int n = __double2loint(sh);
+    const double nf = sh - 6755399441055744.0;
+    double r = fma(-nf, 0.3010299955494702, v);       // log10 2 in two pieces: the first has 21 trailing zero bits
+    r = fma(-nf, 1.1451100898021838e-10, r);
+    const double t = r * 2.302585092994046;
+    double p = 1.0 / 6227020800.0;
+    p = fma(p, t, 1.0 / 479001600.0);
+    p = fma(p, t, 1.0 / 39916800.0);
+    p = fma(p, t, 1.0 / 3628800.0);
+    p = fma(p, t, 1.0 / 362880.0);
+    p = fma(p, t, 1.0 / 40320.0);
+    p = fma(p, t, 1.0 / 5040.0);
+    p = fma(p, t, 1.0 / 720.0);
+    p = fma(p, t, 1.0 / 120.0);
+    p = fma(p, t, 1.0 / 24.0);
+    p = fma(p, t, 1.0 / 6.0);
+    p = fma(p, t, 0.5);
+    p = fma(p, t, 1.0);
+    p = fma(p, t, 1.0);
+    return __hiloint2double(__double2hiint(p) + (n << 20), __double2loint(p));  // times 2^n: p in [0.7, 1.42]
+}
+
 __device__ __forceinline__ double dmin(double a, double b) { return a < b ? a : b; }
 __device__ __forceinline__ double dmax(double a, double b) { return a > b ? a : b; }
 
