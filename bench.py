@@ -179,6 +179,7 @@ def run_native(args):
     if not torch.cuda.is_available():
         raise RuntimeError("bench.py: no CUDA device; the product has no CPU path")
     from paper_2606_26268_b200 import rt
+    from rt_workloads import drive_rt as drv
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
@@ -192,9 +193,9 @@ def run_native(args):
     FUSED_CFL = args.api == "fused"
     FUSED_KERNEL = FUSED_CFL and args.fused_seg >= 0
     w = make_workload(args.workload, args.size)
-    g = rt.grid_from_workload(w, device=dev)
+    g = drv.grid_from_workload(w, device=dev)
     g.set_tuning(fused_seg=args.fused_seg)
-    st = rt.DeviceState(g, w)
+    st = drv.DeviceState(g, w)
     st.dt_dev = torch.zeros(1, dtype=torch.float64, device=dev)
     g.cfl_dt_async(st.U, w.cfl, st.dt_dev)
     thick, feedback = bool(w.params["thick_limit"]), bool(w.params["feedback_momentum"]) and w.mom is not None

@@ -19,6 +19,7 @@ using namespace rtm1;
 struct rt_grid {
     GridDev dev;
     cudaStream_t stream;
+    int device;                 // the device the handle was created on (every entry point switches to it)
     double* metric_buf;
     double* lim;  // thick-limit pre-pass array, ntot doubles (lazily allocated)
     double* rk_save[4];  // rt_rk2_step: T^n, m^n (lazily allocated)
@@ -52,16 +53,36 @@ struct rt_grid {
 // RAII around one launch: records an event before and after it when profiling is on
 struct ProfScope {
     rt_grid* g;
+    cudaStream_t st;
     cudaEvent_t b;
-    ProfScope(rt_grid* g_, int kind) : g(g_), b(nullptr) {
+    ProfScope(rt_grid* g_, int kind, cudaStream_t st_ = nullptr) : g(g_), st(st_ ? st_ : g_->stream), b(nullptr) {
         if (!g->profiling) return;
         cudaEvent_t a = nullptr;
-        if (cudaEventCreate(&a) != cudaSuccess || cudaEventCreate(&b) != cudaSuccess) { b = nullptr; return; }
-        cudaEventRecord(a, g->stream);
+        if (cudaEventCreate(&a) != cudaSuccess) return;
+        if (cudaEventCreate(&b) != cudaSuccess) {
+            cudaEventDestroy(a);
+            b = nullptr;
+            return;
+        }
+        cudaEventRecord(a, st);
         g->prof.push_back({kind, a, b});
     }
     ~ProfScope() {
-        if (b) cudaEventRecord(b, g->stream);
+        if (b) cudaEventRecord(b, st);
+    }
+};
+
+// Every entry point runs on the device the handle was created on, whatever the caller's current device is, and
+// restores the caller's device on the way out.
+struct DeviceGuard {
+    int prev;
+    bool switched;
+    explicit DeviceGuard(const rt_grid* g) : prev(-1), switched(false) {
+        if (!g) return;
+        if (cudaGetDevice(&prev) == cudaSuccess && prev != g->device) switched = cudaSetDevice(g->device) == cudaSuccess;
+    }
+    ~DeviceGuard() {
+        if (switched) cudaSetDevice(prev);
     }
 };
 
@@ -91,15 +112,18 @@ static int32_t fail(rt_grid* g, int32_t code, const char* fmt, ...) {
 static bool aligned8(const void* p) { return p && (reinterpret_cast<uintptr_t>(p) & 7u) == 0; }
 
 extern "C" const char* rt_last_error(const rt_grid* g) { return g ? g->err : "null grid handle"; }
-extern "C" int64_t rt_get_launch_count(const rt_grid* g) { return g ? g->launches : 0; }
+extern "C" int64_t rt_get_launch_count(const rt_grid* g) {
+    DeviceGuard dg_(g); return g ? g->launches : 0; }
 
 extern "C" int32_t rt_set_profiling(rt_grid* g, int32_t on) {
+    DeviceGuard dg_(g);
     if (!g) return RT_ERR_INVALID_ARG;
     g->profiling = on ? 1 : 0;
     return RT_OK;
 }
 
 extern "C" int32_t rt_get_kernel_times(rt_grid* g, double ms[RT_NKERNEL_KINDS], int64_t launches[RT_NKERNEL_KINDS]) {
+    DeviceGuard dg_(g);
     if (!g || !ms || !launches) return fail(g, RT_ERR_INVALID_ARG, "rt_get_kernel_times: null argument");
     for (int k = 0; k < RT_NKERNEL_KINDS; ++k) {
         ms[k] = 0.0;
@@ -120,6 +144,7 @@ extern "C" int32_t rt_get_kernel_times(rt_grid* g, double ms[RT_NKERNEL_KINDS], 
 }
 
 extern "C" int32_t rt_set_tuning(rt_grid* g, int32_t march_len, int32_t fused_seg) {
+    DeviceGuard dg_(g);
     if (!g || march_len < 0 || fused_seg < -1) return fail(g, RT_ERR_INVALID_ARG, "rt_set_tuning: bad argument");
     g->march_len = march_len;
     g->fused_seg = fused_seg;
@@ -147,6 +172,8 @@ extern "C" int32_t rt_grid_create(int32_t geometry, const int32_t n[3], int32_t 
     if (geometry == RT_SPHERICAL && (x2f[0] < 0.0 || x2f[n[1]] > M_PI)) return RT_ERR_INVALID_ARG;
     // the geometric sources ride on the x1 sweep: curvilinear grids need an active x1
     if (geometry != RT_CARTESIAN && n[0] < 2) return RT_ERR_INVALID_ARG;
+    // x2 / x3 indices ride in gridDim.y / gridDim.z of several launches (limit 65535)
+    if (n[1] > 65535 || n[2] > 65535) return RT_ERR_INVALID_ARG;
 
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) return RT_ERR_CUDA;  // no CPU fallback
@@ -155,6 +182,8 @@ extern "C" int32_t rt_grid_create(int32_t geometry, const int32_t n[3], int32_t 
     if (!g) return RT_ERR_CUDA;
     memset(&g->dev, 0, sizeof(g->dev));
     g->stream = reinterpret_cast<cudaStream_t>(cuda_stream);
+    g->device = 0;
+    cudaGetDevice(&g->device);
     g->metric_buf = nullptr;
     g->lim = nullptr;
     g->kpr = nullptr;
@@ -250,6 +279,7 @@ extern "C" int32_t rt_grid_create(int32_t geometry, const int32_t n[3], int32_t 
 }
 
 extern "C" int32_t rt_grid_destroy(rt_grid* g) {
+    DeviceGuard dg_(g);
     if (!g) return RT_ERR_INVALID_ARG;
     cudaStreamSynchronize(g->stream);
     for (auto& r : g->prof) {
@@ -272,6 +302,7 @@ extern "C" int32_t rt_grid_destroy(rt_grid* g) {
 }
 
 extern "C" int32_t rt_grid_get_metrics(rt_grid* g, double* vol, double* area1, double* area2, double* area3) {
+    DeviceGuard dg_(g);
     if (!g) return RT_ERR_INVALID_ARG;
     const GridDev& D = g->dev;
     const size_t n1 = D.n[0], n2 = D.n[1], n3 = D.n[2];
@@ -295,6 +326,7 @@ extern "C" int32_t rt_grid_get_metrics(rt_grid* g, double* vol, double* area1, d
 }
 
 extern "C" int32_t rt_set_params(rt_grid* g, const rt_params* p) {
+    DeviceGuard dg_(g);
     if (!g || !p) return fail(g, RT_ERR_INVALID_ARG, "rt_set_params: null argument");
     if (!(p->chat > 0.0) || !(p->c > 0.0) || !(p->a_R >= 0.0) || !(p->c_v > 0.0) || !(p->E_floor >= 0.0) ||
         !isfinite(p->chat) || !isfinite(p->c) || !isfinite(p->a_R) || !isfinite(p->c_v) || !isfinite(p->E_floor))
@@ -324,6 +356,7 @@ static bool same_law(const rt_grid* g, int a, int b) {
 }
 
 extern "C" int32_t rt_set_opacity(rt_grid* g, int32_t which, const rt_opacity* o) {
+    DeviceGuard dg_(g);
     if (!g || !o || which < 0 || which > 2) return fail(g, RT_ERR_INVALID_ARG, "rt_set_opacity: bad argument");
     OpacDev d;
     memset(&d, 0, sizeof(d));
@@ -419,7 +452,8 @@ static int32_t launch_fill_ghosts(rt_grid* g, double* const U[4]) {
 }
 
 // face-normal ghosts of all active axes in one launch (the sub-step kernels read nothing else)
-static int32_t launch_fill_faces(rt_grid* g, double* const U[4]) {
+static int32_t launch_fill_faces(rt_grid* g, double* const U[4], cudaStream_t st = nullptr) {
+    if (!st) st = g->stream;
     const GridDev& D = g->dev;
     Fields4 F;
     for (int q = 0; q < 4; ++q) F.q[q] = U[q];
@@ -434,14 +468,15 @@ static int32_t launch_fill_faces(rt_grid* g, double* const U[4]) {
     if (tot == 0) return RT_OK;
     const int nb = (int)((tot + 255) / 256 > 8192 ? 8192 : (tot + 255) / 256);
     {
-        ProfScope ps(g, RT_K_GHOST);
-        k_fill_faces<<<nb, 256, 0, g->stream>>>(D, F);
+        ProfScope ps(g, RT_K_GHOST, st);
+        k_fill_faces<<<nb, 256, 0, st>>>(D, F);
     }
     RT_LAUNCH_CHECK(g);
     return RT_OK;
 }
 
 extern "C" int32_t rt_fill_ghosts(rt_grid* g, double* const U[4]) {
+    DeviceGuard dg_(g);
     if (!g || !U) return fail(g, RT_ERR_INVALID_ARG, "rt_fill_ghosts: null argument");
     for (int q = 0; q < 4; ++q)
         if (!aligned8(U[q])) return fail(g, RT_ERR_INVALID_ARG, "rt_fill_ghosts: U[%d] null or misaligned", q);
@@ -597,6 +632,7 @@ static int32_t explicit_impl(rt_grid* g, double dt, const double* dt_dev, const 
 
 extern "C" int32_t rt_explicit_step(rt_grid* g, double dt, const double* rho, const double* T, double* const U_in[4],
                                     double* const U_out[4]) {
+    DeviceGuard dg_(g);
     return explicit_impl(g, dt, nullptr, rho, T, U_in, U_out);
 }
 
@@ -660,6 +696,7 @@ static int32_t implicit_impl(rt_grid* g, double dt, const double* dt_dev, const 
 }
 
 extern "C" int32_t rt_set_face_fix(rt_grid* g, int32_t mode) {
+    DeviceGuard dg_(g);
     if (!g) return RT_ERR_INVALID_ARG;
     if (mode < RT_FIX_FPRESERVING || mode > RT_FIX_CLIP) return fail(g, RT_ERR_INVALID_ARG, "rt_set_face_fix: unknown mode %d", mode);
     g->face_fix = mode;
@@ -668,6 +705,7 @@ extern "C" int32_t rt_set_face_fix(rt_grid* g, int32_t mode) {
 
 extern "C" int32_t rt_irradiation_radial(rt_grid* g, double L0, double kappa_irr, double tau_in, const double* rho,
                                          double* tau_hi, double* div_firr) {
+    DeviceGuard dg_(g);
     if (!g) return RT_ERR_INVALID_ARG;
     if (!aligned8(rho) || !aligned8(div_firr) || (tau_hi && !aligned8(tau_hi)))
         return fail(g, RT_ERR_INVALID_ARG, "rt_irradiation_radial: null or misaligned pointer");
@@ -681,6 +719,7 @@ extern "C" int32_t rt_irradiation_radial(rt_grid* g, double L0, double kappa_irr
 }
 
 extern "C" int32_t rt_set_irradiation(rt_grid* g, const double* div_firr) {
+    DeviceGuard dg_(g);
     if (!g) return RT_ERR_INVALID_ARG;
     if (div_firr && !aligned8(div_firr)) return fail(g, RT_ERR_INVALID_ARG, "rt_set_irradiation: misaligned pointer");
     g->divfirr = div_firr;
@@ -688,11 +727,13 @@ extern "C" int32_t rt_set_irradiation(rt_grid* g, const double* div_firr) {
 }
 
 extern "C" int32_t rt_implicit_step(rt_grid* g, double dt, const double* rho, double* T, double* const mom[3], double* const U[4]) {
+    DeviceGuard dg_(g);
     return implicit_impl(g, dt, nullptr, rho, T, mom, U, false, 0.0, nullptr);
 }
 
 extern "C" int32_t rt_implicit_step_cfl(rt_grid* g, double dt, const double* rho, double* T, double* const mom[3],
                                         double* const U[4], double cfl, double* dt_next_device) {
+    DeviceGuard dg_(g);
     return implicit_impl(g, dt, nullptr, rho, T, mom, U, true, cfl, dt_next_device);
 }
 
@@ -740,11 +781,13 @@ static bool fused_make_maps(const rt_grid* g, const FusedArgs& a, int narr, Fuse
 template <bool HLL, bool THICK, bool CURVI, bool FEEDBACK, bool RUS, bool HASZ>
 static cudaError_t launch_fused_z(rt_grid* g, const ParamsDev& P, const FusedArgs& a, const FusedMaps& maps, dim3 grid, int seglen) {
     auto kern = k_substep_fused<HLL, THICK, CURVI, FEEDBACK, RUS, HASZ>;
-    static bool attr_done = false;
-    if (!attr_done) {
+    // the attribute is per device (and per instantiation: this function is a template)
+    static bool attr_done[64] = {false};
+    const int dev = g->device >= 0 && g->device < 64 ? g->device : 0;
+    if (!attr_done[dev] || g->device >= 64) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kFusedSmemBytes);
         if (e != cudaSuccess) return e;
-        attr_done = true;
+        attr_done[dev] = true;
     }
     kern<<<grid, dim3(32, FNY), kFusedSmemBytes, g->stream>>>(g->dev, P, g->opac[0], g->opac[1], g->opac[2], a, maps, seglen);
     return cudaSuccess;
@@ -849,6 +892,8 @@ static int32_t fused_impl(rt_grid* g, double* dt_device, double cfl, const doubl
     int32_t rc = launch_fill_faces(g, U_in);
     if (rc != RT_OK) return rc;
     if (thick) {
+        // (running the ghost fill beside the pre-pass on a second stream was measured: no gain, both are short and
+        // memory-bound)
         rc = launch_thick_limit(g, rho, T, true);
         if (rc != RT_OK) return rc;
     }
@@ -899,6 +944,7 @@ static int32_t fused_impl(rt_grid* g, double* dt_device, double cfl, const doubl
 
 extern "C" int32_t rt_substep(rt_grid* g, double* dt_device, double cfl, const double* rho, double* T, double* const mom[3],
                               double* const U_in[4], double* const U_out[4]) {
+    DeviceGuard dg_(g);
     if (!g || !aligned8(dt_device)) return fail(g, RT_ERR_INVALID_ARG, "rt_substep: null or misaligned dt_device");
     if (!(cfl > 0.0) || !isfinite(cfl)) return fail(g, RT_ERR_INVALID_ARG, "rt_substep: cfl must be finite and > 0");
     if (!aligned8(rho) || !aligned8(T)) return fail(g, RT_ERR_INVALID_ARG, "rt_substep: rho / T null or misaligned");
@@ -919,6 +965,7 @@ static int32_t substep_impl(rt_grid* g, double* dt_device, double cfl, const dou
 
 extern "C" int32_t rt_rk2_step(rt_grid* g, double* dt_device, double cfl, const double* rho, double* T, double* const mom[3],
                                double* const U[4], double* const W1[4], double* const W2[4]) {
+    DeviceGuard dg_(g);
     if (!g || !aligned8(dt_device)) return fail(g, RT_ERR_INVALID_ARG, "rt_rk2_step: null or misaligned dt_device");
     if (!(cfl > 0.0) || !isfinite(cfl)) return fail(g, RT_ERR_INVALID_ARG, "rt_rk2_step: cfl must be finite and > 0");
     if (!aligned8(rho) || !aligned8(T) || !U || !W1 || !W2) return fail(g, RT_ERR_INVALID_ARG, "rt_rk2_step: null or misaligned argument");
@@ -968,6 +1015,7 @@ extern "C" int32_t rt_rk2_step(rt_grid* g, double* dt_device, double cfl, const 
 }
 
 extern "C" int32_t rt_cfl_dt_async(rt_grid* g, const double* const U[4], double cfl, double* dt_device) {
+    DeviceGuard dg_(g);
     if (!g || !U || !dt_device) return fail(g, RT_ERR_INVALID_ARG, "rt_cfl_dt: null argument");
     if (!g->have_par) return fail(g, RT_ERR_BAD_STATE, "rt_cfl_dt: rt_set_params has not been called");
     if (!(cfl > 0.0) || !isfinite(cfl)) return fail(g, RT_ERR_INVALID_ARG, "rt_cfl_dt: cfl must be finite and > 0");
@@ -985,6 +1033,7 @@ extern "C" int32_t rt_cfl_dt_async(rt_grid* g, const double* const U[4], double 
 }
 
 extern "C" int32_t rt_cfl_dt(rt_grid* g, const double* const U[4], double cfl, double* dt_host) {
+    DeviceGuard dg_(g);
     if (!dt_host) return fail(g, RT_ERR_INVALID_ARG, "rt_cfl_dt: null argument");
     int32_t rc = rt_cfl_dt_async(g, U, cfl, g ? g->dt_dev : nullptr);
     if (rc != RT_OK) return rc;
@@ -995,6 +1044,7 @@ extern "C" int32_t rt_cfl_dt(rt_grid* g, const double* const U[4], double cfl, d
 }
 
 extern "C" int32_t rt_get_floor_counts(rt_grid* g, int64_t* n_floor, int64_t* n_clip) {
+    DeviceGuard dg_(g);
     if (!g) return RT_ERR_INVALID_ARG;
     RT_CUDA(g, cudaMemcpyAsync(g->counters_pinned, g->counters, 2 * sizeof(unsigned long long), cudaMemcpyDeviceToHost, g->stream));
     RT_CUDA(g, cudaMemsetAsync(g->counters, 0, 2 * sizeof(unsigned long long), g->stream));

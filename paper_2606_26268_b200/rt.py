@@ -103,11 +103,13 @@ def lib():
     return _lib
 
 
-def _check_field(t, shape, name):
+def _check_field(t, shape, name, device=None):
     if not isinstance(t, torch.Tensor):
         raise TypeError("%s must be a torch.Tensor on the GPU" % name)
     if not t.is_cuda:
         raise RuntimeError("%s is not a CUDA tensor: this library has no CPU path" % name)
+    if device is not None and t.device != device:
+        raise ValueError("%s lives on %s but the grid was created on %s" % (name, t.device, device))
     if t.dtype != torch.float64 or not t.is_contiguous() or tuple(t.shape) != tuple(shape):
         raise ValueError("%s must be contiguous float64 of shape %s (got %s %s)" % (name, tuple(shape), t.dtype,
                                                                                      tuple(t.shape)))
@@ -175,6 +177,8 @@ class Grid:
         if not torch.cuda.is_available():
             raise RuntimeError("no CUDA device: paper_2606_26268_b200 has no CPU path")
         self.device = torch.device(device)
+        if self.device.index is None:
+            self.device = torch.device("cuda", torch.cuda.current_device())
         self.n = tuple(int(v) for v in n)
         self.gh = tuple(nghost if v > 1 else 0 for v in self.n)
         self.nt = tuple(v + 2 * g for v, g in zip(self.n, self.gh))
@@ -250,7 +254,7 @@ class Grid:
 
     def fill_ghosts(self, U):
         for q, t in enumerate(U):
-            _check_field(t, self.shape, "U[%d]" % q)
+            _check_field(t, self.shape, "U[%d]" % q, self.device)
         rc = lib().rt_fill_ghosts(self._h, _ptr_array(U))
         if rc != OK:
             self._raise("rt_fill_ghosts", rc)
@@ -258,36 +262,36 @@ class Grid:
     def explicit_step(self, dt, rho, T, U_in, U_out):
         for name, t in (("rho", rho), ("T", T)):
             if t is not None:
-                _check_field(t, self.shape, name)
+                _check_field(t, self.shape, name, self.device)
         for q in range(4):
-            _check_field(U_in[q], self.shape, "U_in[%d]" % q)
-            _check_field(U_out[q], self.shape, "U_out[%d]" % q)
+            _check_field(U_in[q], self.shape, "U_in[%d]" % q, self.device)
+            _check_field(U_out[q], self.shape, "U_out[%d]" % q, self.device)
         rc = lib().rt_explicit_step(self._h, float(dt), rho.data_ptr() if rho is not None else None,
                                     T.data_ptr() if T is not None else None, _ptr_array(U_in), _ptr_array(U_out))
         if rc != OK:
             self._raise("rt_explicit_step", rc)
 
     def implicit_step(self, dt, rho, T, mom, U):
-        _check_field(rho, self.shape, "rho")
-        _check_field(T, self.shape, "T")
+        _check_field(rho, self.shape, "rho", self.device)
+        _check_field(T, self.shape, "T", self.device)
         for q in range(4):
-            _check_field(U[q], self.shape, "U[%d]" % q)
+            _check_field(U[q], self.shape, "U[%d]" % q, self.device)
         if mom is not None:
             for q in range(3):
-                _check_field(mom[q], self.shape, "mom[%d]" % q)
+                _check_field(mom[q], self.shape, "mom[%d]" % q, self.device)
         rc = lib().rt_implicit_step(self._h, float(dt), rho.data_ptr(), T.data_ptr(),
                                     _ptr_array(mom) if mom is not None else None, _ptr_array(U))
         if rc != OK:
             self._raise("rt_implicit_step", rc)
 
     def implicit_step_cfl(self, dt, rho, T, mom, U, cfl, dt_next_device):
-        _check_field(rho, self.shape, "rho")
-        _check_field(T, self.shape, "T")
+        _check_field(rho, self.shape, "rho", self.device)
+        _check_field(T, self.shape, "T", self.device)
         for q in range(4):
-            _check_field(U[q], self.shape, "U[%d]" % q)
+            _check_field(U[q], self.shape, "U[%d]" % q, self.device)
         if mom is not None:
             for q in range(3):
-                _check_field(mom[q], self.shape, "mom[%d]" % q)
+                _check_field(mom[q], self.shape, "mom[%d]" % q, self.device)
         self._check_dt_device(dt_next_device)
         rc = lib().rt_implicit_step_cfl(self._h, float(dt), rho.data_ptr(), T.data_ptr(),
                                         _ptr_array(mom) if mom is not None else None, _ptr_array(U), float(cfl),
@@ -296,14 +300,14 @@ class Grid:
             self._raise("rt_implicit_step_cfl", rc)
 
     def substep(self, dt_device, cfl, rho, T, mom, U_in, U_out):
-        _check_field(rho, self.shape, "rho")
-        _check_field(T, self.shape, "T")
+        _check_field(rho, self.shape, "rho", self.device)
+        _check_field(T, self.shape, "T", self.device)
         for q in range(4):
-            _check_field(U_in[q], self.shape, "U_in[%d]" % q)
-            _check_field(U_out[q], self.shape, "U_out[%d]" % q)
+            _check_field(U_in[q], self.shape, "U_in[%d]" % q, self.device)
+            _check_field(U_out[q], self.shape, "U_out[%d]" % q, self.device)
         if mom is not None:
             for q in range(3):
-                _check_field(mom[q], self.shape, "mom[%d]" % q)
+                _check_field(mom[q], self.shape, "mom[%d]" % q, self.device)
         self._check_dt_device(dt_device)
         rc = lib().rt_substep(self._h, dt_device.data_ptr(), float(cfl), rho.data_ptr(), T.data_ptr(),
                               _ptr_array(mom) if mom is not None else None, _ptr_array(U_in), _ptr_array(U_out))
@@ -316,10 +320,10 @@ class Grid:
             self._raise("rt_set_face_fix", rc)
 
     def irradiation_radial(self, L0, kappa_irr, tau_in, rho, tau_hi, div_firr):
-        _check_field(rho, self.shape, "rho")
-        _check_field(div_firr, self.shape, "div_firr")
+        _check_field(rho, self.shape, "rho", self.device)
+        _check_field(div_firr, self.shape, "div_firr", self.device)
         if tau_hi is not None:
-            _check_field(tau_hi, self.shape, "tau_hi")
+            _check_field(tau_hi, self.shape, "tau_hi", self.device)
         rc = lib().rt_irradiation_radial(self._h, float(L0), float(kappa_irr), float(tau_in), rho.data_ptr(),
                                          tau_hi.data_ptr() if tau_hi is not None else None, div_firr.data_ptr())
         if rc != OK:
@@ -328,22 +332,22 @@ class Grid:
     def set_irradiation(self, div_firr):
         """div F_irr per cell (CUDA float64 tensor in the field layout, kept alive by this object) or None"""
         if div_firr is not None:
-            _check_field(div_firr, self.shape, "div_firr")
+            _check_field(div_firr, self.shape, "div_firr", self.device)
         self._div_firr = div_firr
         rc = lib().rt_set_irradiation(self._h, div_firr.data_ptr() if div_firr is not None else None)
         if rc != OK:
             self._raise("rt_set_irradiation", rc)
 
     def rk2_step(self, dt_device, cfl, rho, T, mom, U, W1, W2):
-        _check_field(rho, self.shape, "rho")
-        _check_field(T, self.shape, "T")
+        _check_field(rho, self.shape, "rho", self.device)
+        _check_field(T, self.shape, "T", self.device)
         for q in range(4):
-            _check_field(U[q], self.shape, "U[%d]" % q)
-            _check_field(W1[q], self.shape, "W1[%d]" % q)
-            _check_field(W2[q], self.shape, "W2[%d]" % q)
+            _check_field(U[q], self.shape, "U[%d]" % q, self.device)
+            _check_field(W1[q], self.shape, "W1[%d]" % q, self.device)
+            _check_field(W2[q], self.shape, "W2[%d]" % q, self.device)
         if mom is not None:
             for q in range(3):
-                _check_field(mom[q], self.shape, "mom[%d]" % q)
+                _check_field(mom[q], self.shape, "mom[%d]" % q, self.device)
         self._check_dt_device(dt_device)
         rc = lib().rt_rk2_step(self._h, dt_device.data_ptr(), float(cfl), rho.data_ptr(), T.data_ptr(),
                                _ptr_array(mom) if mom is not None else None, _ptr_array(U), _ptr_array(W1), _ptr_array(W2))
@@ -357,7 +361,7 @@ class Grid:
 
     def cfl_dt(self, U, cfl):
         for q in range(4):
-            _check_field(U[q], self.shape, "U[%d]" % q)
+            _check_field(U[q], self.shape, "U[%d]" % q, self.device)
         out = C.c_double()
         rc = lib().rt_cfl_dt(self._h, _ptr_array(U), float(cfl), C.byref(out))
         if rc != OK:
@@ -366,7 +370,7 @@ class Grid:
 
     def cfl_dt_async(self, U, cfl, dt_device):
         for q in range(4):
-            _check_field(U[q], self.shape, "U[%d]" % q)
+            _check_field(U[q], self.shape, "U[%d]" % q, self.device)
         if not (dt_device.is_cuda and dt_device.dtype == torch.float64 and dt_device.numel() >= 1):
             raise ValueError("dt_device must be a CUDA float64 tensor")
         rc = lib().rt_cfl_dt_async(self._h, _ptr_array(U), float(cfl), dt_device.data_ptr())
@@ -396,78 +400,3 @@ class Grid:
 
     def launch_count(self):
         return int(lib().rt_get_launch_count(self._h))
-
-
-# ---------------------------------------------------------------------- driving a described workload
-def grid_from_workload(w, device="cuda:0"):
-    g = Grid(w.geometry, w.n, w.xf[0], w.xf[1], w.xf[2], w.bc, device=device)
-    g.set_params(make_params(**w.params))
-    for which, spec in w.opacities.items():
-        g.set_opacity(which, opacity_from_spec(spec))
-    return g
-
-
-class DeviceState:
-    """device-resident copy of a workload's fields: U (two buffers), rho, T, mom"""
-
-    def __init__(self, g, w):
-        self.U = [g.to_device(a) for a in w.U]
-        self.U2 = [t.clone() for t in self.U]  # ghosts of FIXED boundaries must exist in both buffers
-        self.rho = g.to_device(w.rho)
-        self.T = g.to_device(w.T)
-        self.mom = [g.to_device(a) for a in w.mom] if w.mom is not None else None
-
-
-def substep(g, w, st, dt, step_index=0):
-    """one sub-step = rt_explicit_step + rt_implicit_step on the device state (buffers swap)"""
-    if w.solver_schedule:
-        g.set_params(make_params(**dict(w.params, solver=w.solver_at(step_index))))
-    g.explicit_step(dt, st.rho, st.T, st.U, st.U2)
-    g.implicit_step(dt, st.rho, st.T, st.mom, st.U2)
-    st.U, st.U2 = st.U2, st.U
-
-
-def run_substeps(g, w, nsub, dts=None, st=None):
-    """nsub sub-steps of workload w; dts = fixed time steps, else rt_cfl_dt each step.
-    Returns (state, list of dt used)."""
-    st = st if st is not None else DeviceState(g, w)
-    used = []
-    for s in range(nsub):
-        if w.solver_schedule:
-            g.set_params(make_params(**dict(w.params, solver=w.solver_at(s))))
-        dt = float(dts[s]) if dts is not None else g.cfl_dt(st.U, w.cfl)
-        used.append(dt)
-        g.explicit_step(dt, st.rho, st.T, st.U, st.U2)
-        g.implicit_step(dt, st.rho, st.T, st.mom, st.U2)
-        st.U, st.U2 = st.U2, st.U
-    return st, used
-
-
-def run_substeps_fused(g, w, nsub, st=None):
-    """nsub sub-steps through rt_substep: the time step never leaves the device (seeded by rt_cfl_dt_async,
-    then produced by the CFL reduction fused behind each implicit half).  Returns (state, dt tensor of the
-    NEXT sub-step, list of the dt used as a device tensor history)."""
-    st = st if st is not None else DeviceState(g, w)
-    dt_dev = torch.zeros(1, dtype=torch.float64, device=g.device)
-    hist = torch.zeros(nsub, dtype=torch.float64, device=g.device)
-    g.cfl_dt_async(st.U, w.cfl, dt_dev)
-    for s in range(nsub):
-        if w.solver_schedule:
-            g.set_params(make_params(**dict(w.params, solver=w.solver_at(s))))
-        hist[s:s + 1].copy_(dt_dev)
-        g.substep(dt_dev, w.cfl, st.rho, st.T, st.mom, st.U, st.U2)
-        st.U, st.U2 = st.U2, st.U
-    return st, dt_dev, hist
-
-
-def run_rk2(g, w, nsteps, st=None):
-    """nsteps RK2 steps through rt_rk2_step (time step resident on the device).  Returns (state, dt history tensor)."""
-    st = st if st is not None else DeviceState(g, w)
-    W2 = [t.clone() for t in st.U]
-    dt_dev = torch.zeros(1, dtype=torch.float64, device=g.device)
-    hist = torch.zeros(nsteps, dtype=torch.float64, device=g.device)
-    g.cfl_dt_async(st.U, w.cfl, dt_dev)
-    for s in range(nsteps):
-        hist[s:s + 1].copy_(dt_dev)
-        g.rk2_step(dt_dev, w.cfl, st.rho, st.T, st.mom, st.U, st.U2, W2)
-    return st, hist
