@@ -29,15 +29,16 @@ METRIC = "radiation cell-updates/sec (fp64, 1 B200)"
 UNIT = "cell-updates/s"
 
 FUSED_CFL = True
-FUSED_KERNEL = True   # rt_substep runs k_substep_fused (3-D grids, --fused-seg >= 0, --api fused)
+FUSED_KERNEL = True   # rt_substep runs k_substep_fused (2-D / 3-D grids, --fused-seg >= 0, --api fused)
 
-# fp64-pipe roof (DESIGN.md Sect. 5): 148 SMs x 64 fp64 lanes/clk x 1.965 GHz (B200_PROFILING.md unit counts and clock)
-FP64_PEAK_TINST = 148 * 64 * 1.965e9 / 1e12
-# Algorithmic fp64-pipe instructions (DFMA/DMUL/DADD/DSETP) per cell-update of k_substep_fused: ncu's executed count of
-# the committed capture (profiles/r1_ncu_full_fused.md) x the useful-lane fraction of the launch (30 of 32 lanes along
-# x1 and the ragged last tile, edge-row extras, segment ends) -- derivation in DESIGN.md Sect. 5.
-FUSED_FP64_PER_CELL = {"C4": 0.5 * (692.0 + 588.0),   # HLL / GLF alternate
-                       "C5": 741.0}                    # HLL, spherical (opacity tables are evaluated in the pre-pass)
+# fp64-pipe roof by formula, kept beside the MEASURED one (rt_measure_fp64, same process): 148 SMs x 64 lanes/clk x 1.965 GHz
+FP64_FORMULA_TINST = 148 * 64 * 1.965e9 / 1e12
+REGIONS = 5           # timed regions of K steps each; the line reports the median (SURVEY 8(d) "Timing")
+
+
+def method_bytes_per_cell(feedback):
+    """compulsory HBM traffic of one sub-step: read E, F, rho, T (+ m) and write E, F, T (+ m)"""
+    return 88.0 + (48.0 if feedback else 0.0)
 
 
 # Algorithmic bytes per interior cell and launch (DESIGN.md "Kernels and rooflines"): 8 B x (fields read + written)
@@ -67,6 +68,7 @@ def parse_args():
     ap.add_argument("--fused-seg", type=int, default=0, help="rt_set_tuning fused_seg: 0 auto, -1 per-direction kernels, >0 x3 segment")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-also", action="store_true", help="skip the second north_star config (C5 beside C4)")
     return ap.parse_args()
 
 
@@ -172,6 +174,136 @@ def one_substep(rt, g, w, st, step_index):
     return dt
 
 
+def csrc_hash():
+    """sha256 over the CUDA sources: ties the ncu-derived instruction counts under profiles/ to the code they were taken from"""
+    import hashlib
+    h = hashlib.sha256()
+    d = os.path.join(ROOT, "paper_2606_26268_b200", "csrc")
+    for f in sorted(os.listdir(d)):
+        with open(os.path.join(d, f), "rb") as fh:
+            h.update(f.encode() + b"\0" + fh.read())
+    return h.hexdigest()[:16]
+
+
+def load_fp64_counts(workload):
+    """executed fp64-pipe thread instructions per cell-update and ncu's fp64-pipe-active % of k_substep_fused, from
+    profiles/fp64_counts.txt (written by bench_ncu_counts.py from an `ncu --page source/raw --csv` export).  Returns
+    None when the file is missing or was taken from other sources than the ones in the tree (stale)."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "fp64_counts.txt")) as fh:
+            d = json.load(fh)
+    except Exception:
+        return None
+    if d.get("csrc_hash") != csrc_hash():
+        return {"stale": True, "capture_csrc_hash": d.get("csrc_hash"), "tree_csrc_hash": csrc_hash()}
+    return d.get("workloads", {}).get(workload)
+
+
+def measure_fp64_peak(rt, dev):
+    """DFMA microbenchmark in this process (rt_measure_fp64): 8 independent chains per thread, 8 warps per SM
+    sub-partition, ~10 ms.  Thread instructions per second."""
+    best = 0.0
+    for _ in range(3):
+        ms, n = rt.measure_fp64(148 * 4, 256, 8, 20000, device=dev)
+        best = max(best, n / (ms * 1e-3))
+    return best / 1e12
+
+
+def measure_workload(args, rt, drv, w, dev, world, K, Wm, regions, barrier):
+    """the device-resident timing of one workload: returns a dict with value, ms_per_step (median of `regions` timed regions
+    of K sub-steps), per-kernel times, clocks, launches and the live state"""
+    import torch
+    g = drv.grid_from_workload(w, device=dev)
+    g.set_tuning(fused_seg=args.fused_seg)
+    st = drv.DeviceState(g, w)
+    st.dt_dev = torch.zeros(1, dtype=torch.float64, device=dev)
+    g.cfl_dt_async(st.U, w.cfl, st.dt_dev)
+    sampler = ClockSampler(dev.index if dev.index is not None else 0, period=0.002)
+    sampler.start()
+    step = 0
+    for _ in range(Wm):
+        one_substep(rt, g, w, st, step)
+        step += 1
+    ms_regions, launches = [], 0
+    for _ in range(regions):
+        barrier()
+        l0 = g.launch_count()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(K):
+            one_substep(rt, g, w, st, step)
+            step += 1
+        e1.record()
+        barrier()
+        launches = g.launch_count() - l0
+        ms_regions.append(e0.elapsed_time(e1))
+    clocks = sampler.stop()
+    ms_med = sorted(ms_regions)[len(ms_regions) // 2]
+    value, ms_max = replicas_throughput(ms_med, w.ncells, K, world, dev)
+
+    # per-kernel device times over K more steps (instrumented pass): CUDA events on the launching stream, inside the library
+    g.set_profiling(True)
+    for _ in range(K):
+        one_substep(rt, g, w, st, step)
+        step += 1
+    kt = g.kernel_times()
+    g.set_profiling(False)
+    return {"g": g, "st": st, "value": value, "ms_per_step": ms_max / K, "ms_regions": [round(m / K, 5) for m in ms_regions],
+            "kt": kt, "clocks": clocks, "launches": int(launches), "step": step}
+
+
+def roofline_block(w, m, K, world, peaks, fp64_peak):
+    """roofline of the dominant kernel (HBM, on the METHOD's compulsory bytes), every kernel's own figures, the whole
+    sub-step, and the fp64-pipe side block"""
+    thick, feedback = bool(w.params["thick_limit"]), bool(w.params["feedback_momentum"]) and w.mom is not None
+    kt = m["kt"]
+    kernels = {}
+    tot_ms = sum(v[0] for v in kt.values())
+    for name, (tot, cnt) in kt.items():
+        if cnt == 0:
+            continue
+        avg = tot / cnt
+        b = bytes_per_cell(name, thick, feedback) * w.ncells
+        kernels[name] = {"launches_per_step": cnt / K, "avg_ms": round(avg, 5), "share": round(tot / tot_ms, 4),
+                         "alg_bytes": b, "GBps": round(b / (avg * 1e-3) / 1e9, 1) if avg > 0 else None}
+    dom = max(kernels, key=lambda k: kt[k][0])
+    avg_ms = kernels[dom]["avg_ms"]
+    # the method's bytes for the kernel that does the whole sub-step; a per-direction kernel keeps its own algorithmic bytes
+    mb = method_bytes_per_cell(feedback) if dom == "fused" else bytes_per_cell(dom, thick, feedback)
+    alg = mb * w.ncells
+    achieved = alg / (avg_ms * 1e-3) / 1e9
+    sub_bytes = sum(bytes_per_cell(k, thick, feedback) * kernels[k]["launches_per_step"] for k in kernels)
+    sub_GBps = sub_bytes * m["value"] / world / 1e9
+    method_GBps = method_bytes_per_cell(feedback) * m["value"] / world / 1e9
+    roof = {"bound": "hbm", "kernel": dom, "achieved": round(achieved, 1), "peak": peaks["hbm_gbs"], "unit": "GB/s",
+            "frac": round(achieved / peaks["hbm_gbs"], 4), "traffic": load_traffic(dom, w.name),
+            "peak_source": peaks["source"],
+            "bytes_per_cell": mb, "bytes_note": "compulsory bytes of the method for one sub-step (SURVEY 8(d)): read E, F, rho, T"
+            " (+ m), write E, F, T (+ m); the kernel's own algorithmic bytes (adds the lim and rho kappa_P arrays of the"
+            " pre-pass) are in kernels.%s.alg_bytes" % dom,
+            "alg_bytes_per_launch": alg, "avg_launch_ms": avg_ms, "kernels": kernels,
+            "kernel_ms_sum_per_step": round(tot_ms / K, 4),
+            "substep": {"method_bytes_per_cell": method_bytes_per_cell(feedback), "method_GBps": round(method_GBps, 1),
+                        "method_frac": round(method_GBps / peaks["hbm_gbs"], 4),
+                        "alg_bytes_per_cell_all_kernels": sub_bytes, "alg_GBps": round(sub_GBps, 1),
+                        "alg_frac": round(sub_GBps / peaks["hbm_gbs"], 4)}}
+    # fp64 pipe: the roof that binds the fused kernel (DESIGN.md Sect. 5).  Peak MEASURED in this process; executed
+    # instructions per cell from the committed ncu capture of the same sources (refused when stale)
+    alu = {"peak_measured_Tinst": round(fp64_peak, 3), "peak_formula_Tinst": round(FP64_FORMULA_TINST, 3),
+           "peak_source": "rt_measure_fp64 in this run: DFMA chains, 8 per thread, 8 warps per SM sub-partition"}
+    cnt = load_fp64_counts(w.name) if dom == "fused" else None
+    if cnt and not cnt.get("stale"):
+        inst = cnt["fp64_thread_inst_per_cell"]
+        ach = inst * w.ncells / (avg_ms * 1e-3) / 1e12
+        alu.update({"executed_fp64_thread_inst_per_cell": inst, "achieved_Tinst": round(ach, 3),
+                    "frac_of_measured": round(ach / fp64_peak, 4), "ncu_pipe_fp64_active_pct": cnt.get("pipe_fp64_active_pct"),
+                    "counts_source": "profiles/fp64_counts.txt (bench_ncu_counts.py; same csrc hash as the tree)"})
+    elif cnt:
+        alu.update(cnt)
+    roof["alu"] = alu
+    return roof
+
+
 def run_native(args):
     import numpy as np
     import torch
@@ -192,13 +324,6 @@ def run_native(args):
     global FUSED_CFL, FUSED_KERNEL
     FUSED_CFL = args.api == "fused"
     FUSED_KERNEL = FUSED_CFL and args.fused_seg >= 0
-    w = make_workload(args.workload, args.size)
-    g = drv.grid_from_workload(w, device=dev)
-    g.set_tuning(fused_seg=args.fused_seg)
-    st = drv.DeviceState(g, w)
-    st.dt_dev = torch.zeros(1, dtype=torch.float64, device=dev)
-    g.cfl_dt_async(st.U, w.cfl, st.dt_dev)
-    thick, feedback = bool(w.params["thick_limit"]), bool(w.params["feedback_momentum"]) and w.mom is not None
     K, Wm = args.steps, max(args.warmup, 0)
 
     def barrier():
@@ -206,80 +331,34 @@ def run_native(args):
             dist.barrier()
         torch.cuda.synchronize()
 
-    # ---- device-resident timing (value)
-    step = 0
-    for _ in range(Wm):
-        one_substep(rt, g, w, st, step)
-        step += 1
-    barrier()
-    sampler = ClockSampler(local)
-    sampler.start()
-    l0 = g.launch_count()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    e0.record()
-    for _ in range(K):
-        one_substep(rt, g, w, st, step)
-        step += 1
-    e1.record()
-    barrier()
-    clocks = sampler.stop()
-    launches = g.launch_count() - l0
-    ms = e0.elapsed_time(e1)
-    value, ms_max = replicas_throughput(ms, w.ncells, K, world, dev)
-
-    # ---- per-kernel device times over the same K steps (second, instrumented pass): roofline
-    g.set_profiling(True)
-    for _ in range(K):
-        one_substep(rt, g, w, st, step)
-        step += 1
-    kt = g.kernel_times()
-    g.set_profiling(False)
     peaks = load_peaks()
-    kernels = {}
-    for name, (tot, cnt) in kt.items():
-        if cnt == 0:
-            continue
-        avg = tot / cnt
-        b = bytes_per_cell(name, thick, feedback) * w.ncells
-        kernels[name] = {"launches_per_step": cnt / K, "avg_ms": round(avg, 5), "share": None,
-                         "alg_bytes": b, "GBps": round(b / (avg * 1e-3) / 1e9, 1) if avg > 0 else None}
-    tot_ms = sum(v[0] for v in kt.values())
-    for name in kernels:
-        kernels[name]["share"] = round(kt[name][0] / tot_ms, 4)
-    dom = max(kernels, key=lambda k: kt[k][0])
-    achieved = kernels[dom]["GBps"]
-    roofline = {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peaks["hbm_gbs"], "unit": "GB/s",
-                "frac": round(achieved / peaks["hbm_gbs"], 4), "traffic": load_traffic(dom, w.name),
-                "peak_source": peaks["source"], "alg_bytes_per_launch": kernels[dom]["alg_bytes"],
-                "avg_launch_ms": kernels[dom]["avg_ms"], "kernels": kernels,
-                "substep_alg_bytes_per_cell": sum(bytes_per_cell(k, thick, feedback) * kernels[k]["launches_per_step"]
-                                                  for k in kernels),
-                "substep_GBps": None, "kernel_ms_sum_per_step": round(tot_ms / K, 4)}
-    if dom == "fused" and w.name in FUSED_FP64_PER_CELL and not args.size:
-        # the fused kernel is bound by the fp64 pipe, not by HBM (DESIGN.md Sect. 5): report it against that roof and
-        # keep its HBM figure beside it
-        inst = FUSED_FP64_PER_CELL[w.name] * w.ncells
-        ach = inst / (kernels[dom]["avg_ms"] * 1e-3) / 1e12
-        roofline.update({"bound": "alu", "achieved": round(ach, 3), "peak": round(FP64_PEAK_TINST, 3),
-                         "unit": "Tinst/s (fp64 pipe: DFMA/DMUL/DADD/DSETP thread instructions)",
-                         "frac": round(ach / FP64_PEAK_TINST, 4),
-                         "peak_source": "148 SMs x 64 fp64 lanes/clk x 1.965 GHz (B200_PROFILING.md unit counts and clock)",
-                         "alg_fp64_inst_per_cell": FUSED_FP64_PER_CELL[w.name],
-                         "hbm": {"achieved": achieved, "peak": peaks["hbm_gbs"], "unit": "GB/s",
-                                 "frac": round(achieved / peaks["hbm_gbs"], 4), "peak_source": peaks["source"]}})
-    roofline["substep_GBps"] = round(roofline["substep_alg_bytes_per_cell"] * value / world / 1e9, 1)
-    roofline["substep_frac"] = round(roofline["substep_GBps"] / peaks["hbm_gbs"], 4)
-
-    out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
-           "ms_per_step": ms_max / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-           "dtype": "f64", "data": "synthetic", "config": workload_config(w, args), "clocks": clocks,
-           "gpu_launches": int(launches), "roofline": roofline}
+    fp64_peak = measure_fp64_peak(rt, dev)
+    w = make_workload(args.workload, args.size)
+    m = measure_workload(args, rt, drv, w, dev, world, K, Wm, REGIONS, barrier)
+    out = {"metric": METRIC, "value": m["value"], "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
+           "ms_per_step": m["ms_per_step"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+           "dtype": "f64", "data": "synthetic", "config": workload_config(w, args), "clocks": m["clocks"],
+           "gpu_launches": m["launches"], "timing": {"regions": REGIONS, "steps_per_region": K, "reported": "median",
+                                                       "ms_per_step_regions": m["ms_regions"]},
+           "roofline": roofline_block(w, m, K, world, peaks, fp64_peak)}
 
     # ---- end to end: host buffers, copies inside the timed region
     if not args.no_e2e:
-        out["e2e"] = run_e2e(rt, g, w, st, K, world, dev, barrier)
-    del st
+        out["e2e"] = run_e2e(rt, m["g"], w, m["st"], K, world, dev, barrier)
+    del m
     torch.cuda.empty_cache()
+
+    # ---- the other north_star config in the same line (C5 beside C4 and vice versa), same protocol, 3 regions
+    other = {"C4": "C5", "C5": "C4"}.get(args.workload)
+    if other and not args.size and not args.no_also:
+        w2 = make_workload(other)
+        m2 = measure_workload(args, rt, drv, w2, dev, world, K, Wm, 3, barrier)
+        r2 = roofline_block(w2, m2, K, world, peaks, fp64_peak)
+        out["also"] = {other: {"value": m2["value"], "unit": UNIT, "ms_per_step": m2["ms_per_step"],
+                               "ms_per_step_regions": m2["ms_regions"], "config": workload_config(w2, args),
+                               "gpu_launches": m2["launches"], "roofline": r2}}
+        del m2, w2
+        torch.cuda.empty_cache()
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         out["cpu_baseline"] = cpu_baseline(w)
     if world > 1:
@@ -301,17 +380,12 @@ def load_peaks():
 
 
 def load_traffic(kernel, workload):
-    """DRAM bytes per launch of `kernel` from the committed ncu --set full capture (profiles/ncu_traffic.csv,
-    written by hand from the capture named in profiles/ncu_traffic.md), or None"""
-    try:
-        with open(os.path.join(ROOT, "profiles", "ncu_traffic.csv")) as fh:
-            for line in fh.read().splitlines()[1:]:
-                wl, k, b = line.split(",")
-                if wl == workload and k == kernel:
-                    return float(b)
-    except Exception:
-        pass
-    return None
+    """DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) of the fused kernel from the committed ncu
+    capture of the same sources (profiles/fp64_counts.txt), or None (another kernel, no capture, stale capture)"""
+    if kernel != "fused":
+        return None
+    c = load_fp64_counts(workload)
+    return c.get("dram_bytes_per_launch") if c and not c.get("stale") else None
 
 
 def run_e2e(rt, g, w, st, K, world, dev, barrier):
@@ -407,11 +481,20 @@ def time_oracle(w, nsteps, warm=0):
 
 
 def cpu_baseline(w):
+    """the oracle as it stands on the box's host cores: all threads (OpenMP), and one thread (SURVEY 8(d) "Timing")"""
+    from oracle import ort
     n = 2 if w.ncells > 4_000_000 else 5
     v, secs, cores = time_oracle(w, n)
+    ort.set_num_threads(1)
+    try:
+        v1, secs1, _ = time_oracle(w, 1)
+    finally:
+        ort.set_num_threads(cores)
     return {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
             "sample": "%d full sub-steps of the same %s workload (%d cells), %.1f s, OpenMP on %d threads" % (n, w.name, w.ncells,
-                                                                                                            secs, cores)}
+                                                                                                            secs, cores),
+            "single_thread": {"value": v1, "unit": UNIT, "cores": 1,
+                              "sample": "1 full sub-step of the same workload, %.1f s" % secs1}}
 
 
 def run_reference(args):
