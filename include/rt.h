@@ -72,7 +72,9 @@ typedef struct {
  * cuda_stream: a cudaStream_t (NULL = legacy default stream).  Volumes and face areas are the exact
  * finite-volume integrals of R-G9; they are evaluated by a device kernel into separable 1-D factor
  * arrays.  Errors: NULL pointer, n < 1, nghost != 2, non-monotone / non-finite edges, r < 0 or theta
- * outside [0, pi], periodic paired with non-periodic on one axis -> RT_ERR_INVALID_ARG. */
+ * outside [0, pi], periodic paired with non-periodic on one axis, n[1] or n[2] > 65535 (they ride in gridDim.y / .z of
+ * the launches) -> RT_ERR_INVALID_ARG.  The handle belongs to the device that is current at creation: every later call
+ * switches to it for its duration, so a process may hold grids on several GPUs. */
 int32_t rt_grid_create(int32_t geometry, const int32_t n[3], int32_t nghost,
                        const double* x1f, const double* x2f, const double* x3f,
                        const int32_t bc[6], void* cuda_stream, rt_grid** out);
@@ -163,6 +165,12 @@ int32_t rt_cfl_dt_async(rt_grid* g, const double* const U[4], double cfl, double
 /* Activations of the E floor and of the cell-centre f <= 1 clip in rt_implicit_step since the
  * last call (then reset).  Synchronises. */
 int32_t rt_get_floor_counts(rt_grid* g, int64_t* n_floor, int64_t* n_clip);
+
+/* Debug aid (failure detection): counts the interior cells in which E, F1, F2, F3 or (if T != NULL) T is NaN or infinite.
+ * U[4], T: DEVICE, field layout.  *n_bad (HOST, NULL allowed) receives the count; returns RT_ERR_NOT_FINITE when it is not
+ * zero (rt_last_error says how many), RT_OK otherwise.  Synchronises.  The sub-step calls themselves never check: a caller
+ * that wants the check pays for this pass (40 B per cell). */
+int32_t rt_check_finite(rt_grid* g, const double* const U[4], const double* T, int64_t* n_bad);
 
 /* Number of kernel launches the library has enqueued on this grid since creation (bench bookkeeping). */
 int64_t rt_get_launch_count(const rt_grid* g);

@@ -43,10 +43,16 @@ struct rt_grid {
     int fused_tma_off;  // test hook (env RT_M1_NO_TMA at grid creation): stage the planes by cp.async even where TMA could
     int fused_seg;  // rt_set_tuning: 0 auto, -1 never use the fused sub-step kernel, > 0 its x3 segment length
     long long launches;
+    // TMA descriptors of the fused kernel, keyed by the five staged arrays: rt_substep alternates between two buffer
+    // sets, so a handful of entries serves a whole run without re-encoding (the grid shape never changes)
+    struct MapEntry { const double* key[FNARR]; int narr; FusedMaps maps; };
+    std::vector<MapEntry> map_cache;
     // optional per-kernel device timing (rt_set_profiling): one event pair per launch
     int profiling;
     struct ProfRec { int kind; cudaEvent_t a, b; };
     std::vector<ProfRec> prof;
+    double prof_ms[RT_NKERNEL_KINDS];     // sums already folded in by ProfScope::trim
+    long long prof_n[RT_NKERNEL_KINDS];
     char err[256];
 };
 
@@ -66,6 +72,23 @@ struct ProfScope {
         }
         cudaEventRecord(a, st);
         g->prof.push_back({kind, a, b});
+    }
+    // called by the launch sites BEFORE a new scope opens: with too many pairs outstanding, fold the finished ones into the
+    // running sums (synchronises the stream once per kMaxLive launches) so that a long profiled run holds a bounded number
+    static void trim(rt_grid* g) {
+        constexpr size_t kMaxLive = 4096;
+        if (!g->profiling || g->prof.size() < kMaxLive) return;
+        if (cudaStreamSynchronize(g->stream) != cudaSuccess) return;
+        for (auto& r : g->prof) {
+            float t = 0.f;
+            if (cudaEventElapsedTime(&t, r.a, r.b) == cudaSuccess && r.kind >= 0 && r.kind < RT_NKERNEL_KINDS) {
+                g->prof_ms[r.kind] += (double)t;
+                g->prof_n[r.kind] += 1;
+            }
+            cudaEventDestroy(r.a);
+            cudaEventDestroy(r.b);
+        }
+        g->prof.clear();
     }
     ~ProfScope() {
         if (b) cudaEventRecord(b, st);
@@ -126,8 +149,10 @@ extern "C" int32_t rt_get_kernel_times(rt_grid* g, double ms[RT_NKERNEL_KINDS], 
     DeviceGuard dg_(g);
     if (!g || !ms || !launches) return fail(g, RT_ERR_INVALID_ARG, "rt_get_kernel_times: null argument");
     for (int k = 0; k < RT_NKERNEL_KINDS; ++k) {
-        ms[k] = 0.0;
-        launches[k] = 0;
+        ms[k] = g->prof_ms[k];
+        launches[k] = g->prof_n[k];
+        g->prof_ms[k] = 0.0;
+        g->prof_n[k] = 0;
     }
     RT_CUDA(g, cudaStreamSynchronize(g->stream));
     for (auto& r : g->prof) {
@@ -206,6 +231,10 @@ extern "C" int32_t rt_grid_create(int32_t geometry, const int32_t n[3], int32_t 
     }
     g->launches = 0;
     g->profiling = 0;
+    for (int k = 0; k < RT_NKERNEL_KINDS; ++k) {
+        g->prof_ms[k] = 0.0;
+        g->prof_n[k] = 0;
+    }
     g->err[0] = 0;
     for (int w = 0; w < 3; ++w) {
         memset(&g->opac[w], 0, sizeof(OpacDev));
@@ -583,6 +612,7 @@ static int32_t launch_thick_limit(rt_grid* g, const double* rho, const double* T
 // explicit half; the time step is dt (host) or, when dt_dev != nullptr, the device double *dt_dev
 static int32_t explicit_impl(rt_grid* g, double dt, const double* dt_dev, const double* rho, const double* T,
                              double* const U_in[4], double* const U_out[4]) {
+    if (g) ProfScope::trim(g);
     if (!g || !U_in || !U_out) return fail(g, RT_ERR_INVALID_ARG, "rt_explicit_step: null argument");
     if (!g->have_par) return fail(g, RT_ERR_BAD_STATE, "rt_explicit_step: rt_set_params has not been called");
     if (!dt_dev && (!(dt > 0.0) || !isfinite(dt))) return fail(g, RT_ERR_INVALID_ARG, "rt_explicit_step: dt must be finite and > 0");
@@ -877,6 +907,7 @@ static bool fused_eligible(const rt_grid* g) {
 
 static int32_t fused_impl(rt_grid* g, double* dt_device, double cfl, const double* rho, double* T, double* const mom[3],
                           double* const U_in[4], double* const U_out[4]) {
+    ProfScope::trim(g);
     if (!U_in || !U_out) return fail(g, RT_ERR_INVALID_ARG, "rt_substep: null argument");
     if (!g->have_par) return fail(g, RT_ERR_BAD_STATE, "rt_substep: rt_set_params has not been called");
     for (int q = 0; q < 4; ++q)
@@ -927,7 +958,32 @@ static int32_t fused_impl(rt_grid* g, double* dt_device, double cfl, const doubl
     dim3 grid(tx, ty, (D.n[2] + seglen - 1) / seglen);
     FusedMaps maps;
     memset(&maps, 0, sizeof(maps));
-    a.use_tma = (g->fused_tma_off == 0 && fused_make_maps(g, a, thick ? 5 : 4, &maps)) ? 1 : 0;
+    a.use_tma = 0;
+    if (g->fused_tma_off == 0) {
+        const int narr = thick ? 5 : 4;
+        const rt_grid::MapEntry* hit = nullptr;
+        for (const auto& e : g->map_cache) {
+            bool same = e.narr == narr;
+            for (int q = 0; q < narr && same; ++q) same = e.key[q] == a.src[q];
+            if (same) {
+                hit = &e;
+                break;
+            }
+        }
+        if (hit) {
+            maps = hit->maps;
+            a.use_tma = 1;
+        } else if (fused_make_maps(g, a, narr, &maps)) {
+            a.use_tma = 1;
+            if (g->map_cache.size() >= 8) g->map_cache.erase(g->map_cache.begin());
+            rt_grid::MapEntry e;
+            memset(&e, 0, sizeof(e));
+            for (int q = 0; q < narr; ++q) e.key[q] = a.src[q];
+            e.narr = narr;
+            e.maps = maps;
+            g->map_cache.push_back(e);
+        }
+    }
     {
         ProfScope ps(g, RT_K_FUSED);
         cudaError_t e = launch_fused(g, g->par.solver != RT_SOLVER_GLF, thick, D.geometry != RT_CARTESIAN, feedback, P, a, maps, grid, seglen);
@@ -1040,6 +1096,43 @@ extern "C" int32_t rt_cfl_dt(rt_grid* g, const double* const U[4], double cfl, d
     RT_CUDA(g, cudaMemcpyAsync(g->dt_pinned, g->dt_dev, sizeof(double), cudaMemcpyDeviceToHost, g->stream));
     RT_CUDA(g, cudaStreamSynchronize(g->stream));
     *dt_host = *g->dt_pinned;
+    return RT_OK;
+}
+
+extern "C" int32_t rt_check_finite(rt_grid* g, const double* const U[4], const double* T, int64_t* n_bad) {
+    DeviceGuard dg_(g);
+    if (!g || !U) return fail(g, RT_ERR_INVALID_ARG, "rt_check_finite: null argument");
+    FiniteArgs v;
+    memset(&v, 0, sizeof(v));
+    for (int q = 0; q < 4; ++q) {
+        if (!aligned8(U[q])) return fail(g, RT_ERR_INVALID_ARG, "rt_check_finite: U[%d] null or misaligned", q);
+        v.f[q] = U[q];
+    }
+    v.n = 4;
+    if (T) {
+        if (!aligned8(T)) return fail(g, RT_ERR_INVALID_ARG, "rt_check_finite: T misaligned");
+        v.f[v.n++] = T;
+    }
+    const GridDev& D = g->dev;
+    // the clip counter's word serves as scratch: save it, count, restore
+    RT_CUDA(g, cudaMemcpyAsync(g->counters_pinned, g->counters, 2 * sizeof(unsigned long long), cudaMemcpyDeviceToHost, g->stream));
+    RT_CUDA(g, cudaMemsetAsync(g->counters + 1, 0, sizeof(unsigned long long), g->stream));
+    const int bx = D.n[0] >= 128 ? 128 : ((D.n[0] + 31) / 32) * 32;
+    dim3 grid((D.n[0] + bx - 1) / bx, D.n[1], D.n[2]);
+    k_check_finite<<<grid, bx, 0, g->stream>>>(D, v, g->counters + 1);
+    RT_LAUNCH_CHECK(g);
+    unsigned long long saved[2];
+    RT_CUDA(g, cudaStreamSynchronize(g->stream));
+    saved[0] = g->counters_pinned[0];
+    saved[1] = g->counters_pinned[1];
+    RT_CUDA(g, cudaMemcpyAsync(g->counters_pinned, g->counters + 1, sizeof(unsigned long long), cudaMemcpyDeviceToHost, g->stream));
+    RT_CUDA(g, cudaStreamSynchronize(g->stream));
+    const unsigned long long bad = g->counters_pinned[0];
+    g->counters_pinned[0] = saved[1];
+    RT_CUDA(g, cudaMemcpyAsync(g->counters + 1, g->counters_pinned, sizeof(unsigned long long), cudaMemcpyHostToDevice, g->stream));
+    RT_CUDA(g, cudaStreamSynchronize(g->stream));
+    if (n_bad) *n_bad = (int64_t)bad;
+    if (bad) return fail(g, RT_ERR_NOT_FINITE, "rt_check_finite: %llu interior cells hold a non-finite value", bad);
     return RT_OK;
 }
 

@@ -200,6 +200,23 @@ __global__ void k_fill_faces(GridDev g, Fields4 U) {
     }
 }
 
+// Debug aid (SURVEY.md Sect. 5 "failure detection"): count the interior cells in which any of up to five fields is not finite.
+struct FiniteArgs {
+    const double* f[5];
+    int n;
+};
+__global__ void __launch_bounds__(128) k_check_finite(const __grid_constant__ GridDev g, const __grid_constant__ FiniteArgs v,
+                                                      unsigned long long* __restrict__ bad) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    bool b = false;
+    if (i < g.n[0]) {
+        const long long id = (i + g.gh[0]) + (blockIdx.y + g.gh[1]) * g.stride[1] + (blockIdx.z + g.gh[2]) * g.stride[2];
+        for (int q = 0; q < v.n; ++q) b = b || !isfinite(v.f[q][id]);
+    }
+    const unsigned m = __ballot_sync(0xffffffffu, b);
+    if (m && (threadIdx.x & 31) == 0) atomicAdd(bad, (unsigned long long)__popc(m));
+}
+
 // RK2 (L107, L256: two Euler sub-steps and the average of every evolved variable): q <- (q0 + q2)/2 on interior cells.
 // a[] = the fields holding q0 on entry and the average on exit; b[] = q2.  n = 4 (U), 1 (T) or 3 (m) pairs per launch.
 struct AvgArgs {

@@ -152,8 +152,8 @@ __device__ __forceinline__ void state_load(const double* buf, int t, State& s) {
 
 
 // RUS (with HLL = true): RT_SOLVER_RUSANOV, compile-time so that the HLL faces do not pay for the test
-// HASZ = false: 2-D grids (n3 = 1, x3 inactive): one plane, no x3 phase; the march degenerates to the steps
-// c = -1 (nothing), 0 (X, Y), 1 (FIN) and the planes other than 0 are zero-filled by the TMA (clamped in the cp.async path).
+// HASZ = false: 2-D grids (n3 = 1, x3 inactive): one staged plane, no x3 phase; the march degenerates to the steps
+// c = 0 (X, Y) and 1 (FIN, which reads nothing but the thick-limit value of plane 0).
 template <bool HLL, bool THICK, bool CURVI, bool FEEDBACK, bool RUS, bool HASZ>
 __global__ void __launch_bounds__(FNT, FUSED_MINB)
     k_substep_fused(const __grid_constant__ GridDev g, const __grid_constant__ ParamsDev par, const __grid_constant__ OpacDev oP,
@@ -325,7 +325,8 @@ __global__ void __launch_bounds__(FNT, FUSED_MINB)
             double q0[4], dm[4], dp[4];
 #pragma unroll
             for (int q = 0; q < 4; ++q) {
-                q0[q] = pc[q * FPS + o];
+                // 2-D grids stage plane 0 only: step 1 (their FIN step) has no plane of its own to read
+                q0[q] = (HASZ || c == 0) ? pc[q * FPS + o] : 1.0;
                 dm[q] = HASZ ? q0[q] - pm[q * FPS + o] : 0.0;
                 dp[q] = HASZ ? pp[q * FPS + o] - q0[q] : 0.0;
             }

@@ -73,6 +73,7 @@ _SIGNATURES = {
     "rt_cfl_dt": (C.c_int32, [C.c_void_p, C.POINTER(C.c_void_p), C.c_double, _dp]),
     "rt_cfl_dt_async": (C.c_int32, [C.c_void_p, C.POINTER(C.c_void_p), C.c_double, C.c_void_p]),
     "rt_get_floor_counts": (C.c_int32, [C.c_void_p, C.POINTER(C.c_int64), C.POINTER(C.c_int64)]),
+    "rt_check_finite": (C.c_int32, [C.c_void_p, C.POINTER(C.c_void_p), C.c_void_p, C.POINTER(C.c_int64)]),
     "rt_get_launch_count": (C.c_int64, [C.c_void_p]),
     "rt_set_tuning": (C.c_int32, [C.c_void_p, C.c_int32, C.c_int32]),
     "rt_set_profiling": (C.c_int32, [C.c_void_p, C.c_int32]),
@@ -383,6 +384,18 @@ class Grid:
         if rc != OK:
             self._raise("rt_get_floor_counts", rc)
         return a.value, b.value
+
+    def check_finite(self, U, T=None):
+        """rt_check_finite: number of interior cells holding a NaN / inf (raises RtError with status ERR_NOT_FINITE if any)"""
+        for q in range(4):
+            _check_field(U[q], self.shape, "U[%d]" % q, self.device)
+        if T is not None:
+            _check_field(T, self.shape, "T", self.device)
+        n = C.c_int64()
+        rc = lib().rt_check_finite(self._h, _ptr_array(U), T.data_ptr() if T is not None else None, C.byref(n))
+        if rc != OK:
+            self._raise("rt_check_finite", rc)
+        return n.value
 
     def set_profiling(self, on):
         rc = lib().rt_set_profiling(self._h, 1 if on else 0)
