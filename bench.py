@@ -69,6 +69,7 @@ def parse_args():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-also", action="store_true", help="skip the second north_star config (C5 beside C4)")
+    ap.add_argument("--graph", action="store_true", help="replay the sub-steps from a CUDA graph of two (latency-bound grids)")
     return ap.parse_args()
 
 
@@ -211,45 +212,74 @@ def measure_fp64_peak(rt, dev):
 
 def measure_workload(args, rt, drv, w, dev, world, K, Wm, regions, barrier):
     """the device-resident timing of one workload: returns a dict with value, ms_per_step (median of `regions` timed regions
-    of K sub-steps), per-kernel times, clocks, launches and the live state"""
+    of K sub-steps), per-kernel times, clocks, launches and the live state.  --graph: the sub-steps are replayed from a
+    CUDA graph holding two of them (the ping-pong of the two state buffers; K is rounded up to an even number), which is
+    how a launch-latency-bound grid (C1, C2) would be driven; everything then runs on a side stream."""
+    import contextlib
     import torch
-    g = drv.grid_from_workload(w, device=dev)
-    g.set_tuning(fused_seg=args.fused_seg)
-    st = drv.DeviceState(g, w)
-    st.dt_dev = torch.zeros(1, dtype=torch.float64, device=dev)
-    g.cfl_dt_async(st.U, w.cfl, st.dt_dev)
-    sampler = ClockSampler(dev.index if dev.index is not None else 0, period=0.002)
-    sampler.start()
-    step = 0
-    for _ in range(Wm):
-        one_substep(rt, g, w, st, step)
-        step += 1
-    ms_regions, launches = [], 0
-    for _ in range(regions):
-        barrier()
+    side = torch.cuda.Stream(dev) if args.graph else None
+    ctx = torch.cuda.stream(side) if side is not None else contextlib.nullcontext()
+    with ctx:
+        g = drv.grid_from_workload(w, device=dev)
+        g.set_tuning(fused_seg=args.fused_seg)
+        st = drv.DeviceState(g, w)
+        st.dt_dev = torch.zeros(1, dtype=torch.float64, device=dev)
+        g.cfl_dt_async(st.U, w.cfl, st.dt_dev)
+        sampler = ClockSampler(dev.index if dev.index is not None else 0, period=0.002)
+        sampler.start()
+        step = 0
+        for _ in range(Wm + (Wm & 1 if args.graph else 0)):   # an even count keeps the buffer roles of the captured pair
+            one_substep(rt, g, w, st, step)
+            step += 1
+        graph = None
+        if args.graph:
+            K += K & 1
+            torch.cuda.synchronize()
+            graph = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(graph, stream=side):
+                one_substep(rt, g, w, st, step)
+                one_substep(rt, g, w, st, step + 1)
+
+        def run(nsteps):
+            nonlocal step
+            if graph is not None:
+                for _ in range(nsteps // 2):
+                    graph.replay()
+            else:
+                for _ in range(nsteps):
+                    one_substep(rt, g, w, st, step)
+                    step += 1
+
+        ms_regions, launches = [], 0
+        per_step = None
+        for _ in range(regions):
+            barrier()
+            l0 = g.launch_count()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            run(K)
+            e1.record()
+            barrier()
+            launches = g.launch_count() - l0
+            ms_regions.append(e0.elapsed_time(e1))
+        clocks = sampler.stop()
+        ms_med = sorted(ms_regions)[len(ms_regions) // 2]
+        value, ms_max = replicas_throughput(ms_med, w.ncells, K, world, dev)
+
+        # per-kernel device times over K more steps (instrumented pass, eager launches): CUDA events on the launching
+        # stream, inside the library
+        g.set_profiling(True)
         l0 = g.launch_count()
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        e0.record()
         for _ in range(K):
             one_substep(rt, g, w, st, step)
             step += 1
-        e1.record()
-        barrier()
-        launches = g.launch_count() - l0
-        ms_regions.append(e0.elapsed_time(e1))
-    clocks = sampler.stop()
-    ms_med = sorted(ms_regions)[len(ms_regions) // 2]
-    value, ms_max = replicas_throughput(ms_med, w.ncells, K, world, dev)
-
-    # per-kernel device times over K more steps (instrumented pass): CUDA events on the launching stream, inside the library
-    g.set_profiling(True)
-    for _ in range(K):
-        one_substep(rt, g, w, st, step)
-        step += 1
-    kt = g.kernel_times()
-    g.set_profiling(False)
+        eager_launches = g.launch_count() - l0
+        kt = g.kernel_times()
+        g.set_profiling(False)
+        if graph is not None:
+            launches = eager_launches      # kernels per K steps: a replay launches what the capture recorded
     return {"g": g, "st": st, "value": value, "ms_per_step": ms_max / K, "ms_regions": [round(m / K, 5) for m in ms_regions],
-            "kt": kt, "clocks": clocks, "launches": int(launches), "step": step}
+            "kt": kt, "clocks": clocks, "launches": int(launches), "step": step, "K": K}
 
 
 def roofline_block(w, m, K, world, peaks, fp64_peak):
@@ -335,10 +365,11 @@ def run_native(args):
     fp64_peak = measure_fp64_peak(rt, dev)
     w = make_workload(args.workload, args.size)
     m = measure_workload(args, rt, drv, w, dev, world, K, Wm, REGIONS, barrier)
+    K = m["K"]
     out = {"metric": METRIC, "value": m["value"], "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
            "ms_per_step": m["ms_per_step"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
            "dtype": "f64", "data": "synthetic", "config": workload_config(w, args), "clocks": m["clocks"],
-           "gpu_launches": m["launches"], "timing": {"regions": REGIONS, "steps_per_region": K, "reported": "median",
+           "gpu_launches": m["launches"], "timing": {"regions": REGIONS, "steps_per_region": K, "reported": "median", "cuda_graph": bool(args.graph),
                                                        "ms_per_step_regions": m["ms_regions"]},
            "roofline": roofline_block(w, m, K, world, peaks, fp64_peak)}
 

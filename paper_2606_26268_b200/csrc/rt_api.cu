@@ -998,6 +998,82 @@ static int32_t fused_impl(rt_grid* g, double* dt_device, double cfl, const doubl
     return RT_OK;
 }
 
+// Small 1-D grids: the whole sub-step in one launch of one CTA (k_substep_1d)
+static bool oned_eligible(const rt_grid* g) {
+    const GridDev& D = g->dev;
+    return g->fused_seg >= 0 && D.gh[0] > 0 && D.gh[1] == 0 && D.gh[2] == 0 && D.n[0] >= 2 && D.n[0] <= K1D_MAXN;
+}
+
+template <bool HLL, bool THICK, bool CURVI>
+static void launch_1d(rt_grid* g, bool feedback, const ParamsDev& P, const SweepArgs& sw, const ImplicitArgs& im, double cfl,
+                      double* dt_out) {
+    if (feedback)
+        k_substep_1d<HLL, THICK, CURVI, true><<<1, K1D_NT, 0, g->stream>>>(g->dev, P, g->opac[0], g->opac[1], g->opac[2], sw, im, cfl, dt_out);
+    else
+        k_substep_1d<HLL, THICK, CURVI, false><<<1, K1D_NT, 0, g->stream>>>(g->dev, P, g->opac[0], g->opac[1], g->opac[2], sw, im, cfl, dt_out);
+}
+
+static int32_t oned_impl(rt_grid* g, double* dt_device, double cfl, const double* rho, double* T, double* const mom[3],
+                         double* const U_in[4], double* const U_out[4]) {
+    if (!U_in || !U_out) return fail(g, RT_ERR_INVALID_ARG, "rt_substep: null argument");
+    if (!g->have_par) return fail(g, RT_ERR_BAD_STATE, "rt_substep: rt_set_params has not been called");
+    for (int q = 0; q < 4; ++q)
+        if (!aligned8(U_in[q]) || !aligned8(U_out[q]) || U_in[q] == U_out[q])
+            return fail(g, RT_ERR_INVALID_ARG, "rt_substep: U_in/U_out[%d] null, misaligned or aliased", q);
+    const bool feedback = g->par.feedback_momentum && mom != nullptr;
+    if (feedback)
+        for (int q = 0; q < 3; ++q)
+            if (!aligned8(mom[q])) return fail(g, RT_ERR_INVALID_ARG, "rt_substep: mom[%d] null or misaligned", q);
+    const GridDev& D = g->dev;
+    SweepArgs sw;
+    for (int q = 0; q < 4; ++q) {
+        sw.uin[q] = U_in[q];
+        sw.uout[q] = U_out[q];
+    }
+    sw.lim = nullptr;
+    sw.dtc = 0.0;
+    sw.dt_dev = dt_device;
+    sw.chat = g->par.chat;
+    sw.rusanov = g->par.solver == RT_SOLVER_RUSANOV;
+    sw.fix = g->face_fix;
+    ImplicitArgs a;
+    for (int q = 0; q < 4; ++q) a.U[q] = U_out[q];
+    a.rho = rho;
+    a.T = T;
+    for (int q = 0; q < 3; ++q) a.mom[q] = feedback ? mom[q] : nullptr;
+    a.dt = 0.0;
+    a.dt_dev = dt_device;
+    a.scr = g->scr;
+    a.feedback = feedback;
+    a.same_PR = g->same_PR;
+    {
+        const int members[3] = {RT_OPAC_PLANCK, RT_OPAC_ROSSELAND, RT_OPAC_SCATTER};
+        a.os = opac_set(g, members, 3);
+    }
+    a.ichat = 1.0 / g->par.chat;
+    a.counters = g->counters;
+    a.divfirr = g->divfirr;
+    ParamsDev P = {g->par.chat, g->par.c, g->par.a_R, g->par.c_v, g->par.E_floor, g->par.solver, g->par.thick_limit,
+                   g->par.feedback_momentum};
+    const bool hll = g->par.solver != RT_SOLVER_GLF, thick = g->par.thick_limit != 0, curvi = D.geometry != RT_CARTESIAN;
+    {
+        ProfScope ps(g, RT_K_FUSED);
+        const int key = (hll ? 4 : 0) | (thick ? 2 : 0) | (curvi ? 1 : 0);
+        switch (key) {
+            case 0: launch_1d<false, false, false>(g, feedback, P, sw, a, cfl, dt_device); break;
+            case 1: launch_1d<false, false, true>(g, feedback, P, sw, a, cfl, dt_device); break;
+            case 2: launch_1d<false, true, false>(g, feedback, P, sw, a, cfl, dt_device); break;
+            case 3: launch_1d<false, true, true>(g, feedback, P, sw, a, cfl, dt_device); break;
+            case 4: launch_1d<true, false, false>(g, feedback, P, sw, a, cfl, dt_device); break;
+            case 5: launch_1d<true, false, true>(g, feedback, P, sw, a, cfl, dt_device); break;
+            case 6: launch_1d<true, true, false>(g, feedback, P, sw, a, cfl, dt_device); break;
+            default: launch_1d<true, true, true>(g, feedback, P, sw, a, cfl, dt_device); break;
+        }
+    }
+    RT_LAUNCH_CHECK(g);
+    return RT_OK;
+}
+
 extern "C" int32_t rt_substep(rt_grid* g, double* dt_device, double cfl, const double* rho, double* T, double* const mom[3],
                               double* const U_in[4], double* const U_out[4]) {
     DeviceGuard dg_(g);
@@ -1005,6 +1081,7 @@ extern "C" int32_t rt_substep(rt_grid* g, double* dt_device, double cfl, const d
     if (!(cfl > 0.0) || !isfinite(cfl)) return fail(g, RT_ERR_INVALID_ARG, "rt_substep: cfl must be finite and > 0");
     if (!aligned8(rho) || !aligned8(T)) return fail(g, RT_ERR_INVALID_ARG, "rt_substep: rho / T null or misaligned");
     if (fused_eligible(g)) return fused_impl(g, dt_device, cfl, rho, T, mom, U_in, U_out);
+    if (oned_eligible(g)) return oned_impl(g, dt_device, cfl, rho, T, mom, U_in, U_out);
     int32_t rc = explicit_impl(g, 0.0, dt_device, rho, T, U_in, U_out);
     if (rc != RT_OK) return rc;
     return implicit_impl(g, 0.0, dt_device, rho, T, mom, U_out, true, cfl, dt_device);
@@ -1014,6 +1091,7 @@ extern "C" int32_t rt_substep(rt_grid* g, double* dt_device, double cfl, const d
 static int32_t substep_impl(rt_grid* g, double* dt_device, double cfl, const double* rho, double* T, double* const mom[3],
                             double* const U_in[4], double* const U_out[4]) {
     if (fused_eligible(g)) return fused_impl(g, dt_device, cfl, rho, T, mom, U_in, U_out);
+    if (oned_eligible(g)) return oned_impl(g, dt_device, cfl, rho, T, mom, U_in, U_out);
     int32_t rc = explicit_impl(g, 0.0, dt_device, rho, T, U_in, U_out);
     if (rc != RT_OK) return rc;
     return implicit_impl(g, 0.0, dt_device, rho, T, mom, U_out, true, cfl, dt_device);

@@ -327,6 +327,154 @@ __device__ __forceinline__ void implicit_warp_epilogue(const ImplicitArgs& a, do
     }
 }
 
+// ------------------------------------------------------------------------------------------------
+// Small 1-D grids (BASELINE config 1: 256 cells): the WHOLE sub-step in one CTA and one launch — ghost fill (step 1),
+// thick-limit values, face states + Riemann fluxes, divergence (+ geometric sources), floor / clip, opacities, implicit
+// coupling and the new time step (step 10).  Such grids are bound by launch latency, not by any pipe: the five to six
+// launches of the per-direction path cost ~28 us per sub-step, this one a single launch.  One thread per FACE builds
+// both states of its face from the staged row (each cell's slopes are evaluated by its two faces: twice the
+// reconstruction work, which is irrelevant here, and no state exchange), then one thread per CELL finishes it.
+// ------------------------------------------------------------------------------------------------
+constexpr int K1D_MAXN = 512;   // cells: 10.5 doubles of shared memory per cell, 43 KB in all
+constexpr int K1D_NT = 256;
+
+template <bool HLL, bool THICK, bool CURVI, bool FEEDBACK>
+__global__ void __launch_bounds__(K1D_NT) k_substep_1d(const __grid_constant__ GridDev g, const __grid_constant__ ParamsDev par,
+                                                       const __grid_constant__ OpacDev oP, const __grid_constant__ OpacDev oR,
+                                                       const __grid_constant__ OpacDev oS, const __grid_constant__ SweepArgs sw,
+                                                       const __grid_constant__ ImplicitArgs im, double cfl, double* dt_out) {
+    __shared__ double sU[4][K1D_MAXN + 4];
+    __shared__ double sLim[K1D_MAXN + 2];
+    __shared__ double sFl[4][K1D_MAXN + 1];
+    __shared__ double sred[K1D_NT / 32];
+    const int tid = threadIdx.x;
+    const int n = g.n[0], gh = g.gh[0];
+    const double dt = __ldg(im.dt_dev);
+    const double dtc = dt * sw.chat;
+    // step 1 (L111): stage the row with its ghosts; ghosts other than FIXED ones are also written back to U_in
+    for (int e = tid; e < 4 * (n + 4); e += K1D_NT) {
+        const int q = e / (n + 4), c = e - q * (n + 4) - 2;
+        int src = c;
+        bool flip = false;
+        int kind = 3;
+        if (c < 0 || c >= n) {
+            kind = g.bc[c < 0 ? 0 : 1];
+            if (kind == 0) src = c < 0 ? c + n : c - n;
+            else if (kind == 1) src = c < 0 ? 0 : n - 1;
+            else if (kind == 2) {
+                src = c < 0 ? -1 - c : 2 * n - 1 - c;
+                flip = q == 1;
+            }
+        }
+        double v = sw.uin[q][src + gh];
+        if (flip) v = -v;
+        sU[q][c + 2] = v;
+        if (kind != 3) const_cast<double*>(sw.uin[q])[c + gh] = v;
+    }
+    // Eq. 25-26 (R-G7): lim = 4 / (3 rho chi dx) of the cells -1 .. n (ghosts: periodic image or nearest interior cell)
+    if (THICK) {
+        for (int j = tid - 1; j <= n; j += K1D_NT) {
+            int c = j;
+            if (c < 0) c = g.bc[0] == 0 ? c + n : 0;
+            else if (c >= n) c = g.bc[0] == 0 ? c - n : n - 1;
+            const double r = __ldg(im.rho + c + gh), t = im.T[c + gh];
+            const double chi = opacity_eval(oR, r, t) + opacity_eval(oS, r, t);
+            const double tau = r * chi * (g.len[0][0][c] * g.len[0][1][0] * g.len[0][2][0]);
+            sLim[j + 1] = tau > 1.0e-100 ? 4.0 * frcp(3.0 * tau) : kInf;
+        }
+    }
+    __syncthreads();
+    // steps 3-6: the flux through face i (between cells i-1 and i), i = 0 .. n
+    for (int i = tid; i <= n; i += K1D_NT) {
+        double qa[4], qb[4], dma[4], dpa[4], dpb[4];
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            qa[q] = sU[q][i + 1];
+            qb[q] = sU[q][i + 2];
+            dma[q] = qa[q] - sU[q][i];
+            dpa[q] = qb[q] - qa[q];
+            dpb[q] = sU[q][i + 3] - qb[q];
+        }
+        State loa, hia, lob, hib;
+        cell_faces<0, HLL>(qa, dma, dpa, false, true, loa, hia, 0.0, 0.0, 0.0, sw.fix);
+        cell_faces<0, HLL>(qb, dpa, dpb, true, false, lob, hib, 0.0, 0.0, 0.0, sw.fix);
+        const double limd = THICK ? dmax(sLim[i], sLim[i + 1]) : kInf;
+        double fe[4];
+        riemann<HLL>(hia, lob, limd, fe, sw.rusanov != 0);
+        const double w = CURVI ? g.wf[0][i] : 1.0;
+#pragma unroll
+        for (int q = 0; q < 4; ++q) sFl[q][i] = fe[q] * w;
+    }
+    __syncthreads();
+    // step 7 (+ geometric sources, R-G9), then a8-a11 per cell
+    double rate = 0.0;
+    int nfloor = 0, nclip = 0;
+    const double cyz = g.cg[0][1][0] * g.cg[0][2][0];
+    const double il12 = g.ilen[0][1][0] * g.ilen[0][2][0];
+    for (int i = tid; i < n; i += K1D_NT) {
+        const double coef = dtc * g.cg[0][0][i] * cyz;
+        double q0[4], out[4];
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            q0[q] = sU[q][i + 2];
+            out[q] = fma(-coef, sFl[q][i + 1] - sFl[q][i], q0[q]);
+        }
+        if (CURVI) {
+            const double E2 = q0[0] * q0[0];
+            const double F2 = fma(q0[3], q0[3], fma(q0[2], q0[2], q0[1] * q0[1]));
+            const Closure c = closure_of(q0[0], E2, F2);
+            const double s = dtc * g.invr[i];
+            if (g.geometry == 1) {
+                out[1] = fma(s, fma(c.gE * q0[2], q0[2], c.dE), out[1]);
+                out[2] = fma(-s, c.gE * q0[1] * q0[2], out[2]);
+            } else {
+                const double ct = g.cot[0];
+                const double Ptt = fma(c.gE * q0[2], q0[2], c.dE);
+                const double Ppp = fma(c.gE * q0[3], q0[3], c.dE);
+                const double Prt = c.gE * q0[1] * q0[2];
+                const double Prp = c.gE * q0[1] * q0[3];
+                const double Ptp = c.gE * q0[2] * q0[3];
+                out[1] = fma(s, Ptt + Ppp, out[1]);
+                out[2] = fma(s, fma(ct, Ppp, -Prt), out[2]);
+                out[3] = fma(-s, fma(ct, Ptp, Prp), out[3]);
+            }
+        }
+        const long long id = i + gh;
+        double F[3] = {out[1], out[2], out[3]};
+        double m[3] = {0.0, 0.0, 0.0};
+        if (FEEDBACK) {
+#pragma unroll
+            for (int q = 0; q < 3; ++q) m[q] = im.mom[q][id];
+        }
+        const double il[3] = {g.ilen[0][0][i] * il12, 0.0, 0.0};
+        bool floored = false, clipped = false;
+        const double r = implicit_cell<FEEDBACK, true>(g, par, oP, oR, oS, im, dt, id, il, out[0], F, __ldg(im.rho + id), im.T[id], m,
+                                                        floored, clipped);
+        rate = dmax(rate, r);
+        nfloor += floored ? 1 : 0;
+        nclip += clipped ? 1 : 0;
+    }
+    // step 10 (L120; R-G15): dt = cfl / max rate; floor / clip counters
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) rate = dmax(rate, __shfl_xor_sync(0xffffffffu, rate, o));
+    if ((tid & 31) == 0) sred[tid >> 5] = rate;
+    if (__any_sync(0xffffffffu, (nfloor | nclip) != 0)) {
+        nfloor = __reduce_add_sync(0xffffffffu, nfloor);
+        nclip = __reduce_add_sync(0xffffffffu, nclip);
+        if ((tid & 31) == 0) {
+            if (nfloor) atomicAdd(&im.counters[0], (unsigned long long)nfloor);
+            if (nclip) atomicAdd(&im.counters[1], (unsigned long long)nclip);
+        }
+    }
+    __syncthreads();
+    if (tid == 0) {
+        double r = sred[0];
+#pragma unroll
+        for (int k = 1; k < K1D_NT / 32; ++k) r = dmax(r, sred[k]);
+        *dt_out = cfl / r;
+    }
+}
+
 template <bool FEEDBACK, bool CFL>
 __global__ void __launch_bounds__(128) k_implicit(const __grid_constant__ GridDev g, const __grid_constant__ ParamsDev par,
                                                   const __grid_constant__ OpacDev oP, const __grid_constant__ OpacDev oR,
