@@ -109,9 +109,9 @@ int32_t rt_implicit_step(rt_grid* g, double dt, const double* rho, double* T,
 
 /* Face fix of the explicit half (step a3).  The paper's f-preserving scheme (Eq. 19-21) is the default; the two
  * schemes it is compared with (Sect. 2.5, Sect. 3.2 Eq. 36-38 and Fig. 5) can be selected for the same
- * comparisons.  They run in the per-direction kernels: with mode != RT_FIX_FPRESERVING rt_substep / rt_rk2_step take
- * the split path (same results as rt_explicit_step + rt_implicit_step_cfl).  Unknown mode -> RT_ERR_INVALID_ARG, state
- * unchanged.  Host call, nothing enqueued. */
+ * comparisons.  Every path honours the mode (per-direction kernels, the fused 2-D / 3-D kernel, the 1-D kernel); only the
+ * combination with RT_SOLVER_RUSANOV makes rt_substep / rt_rk2_step take the per-direction kernels.  Unknown mode ->
+ * RT_ERR_INVALID_ARG, state unchanged.  Host call, nothing enqueued. */
 int32_t rt_set_face_fix(rt_grid* g, int32_t mode);
 
 /* Irradiation (Sect. 2.9, Eq. 34-35): div_firr = DEVICE array (field layout, caller-owned, must stay valid)

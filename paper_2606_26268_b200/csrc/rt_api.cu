@@ -13,6 +13,16 @@
 #include "../../include/rt.h"
 #include "rt_kernels_fused.cuh"
 #include "rt_kernels_measure.cuh"
+#include "rt_fused_inst.cuh"
+
+// k_substep_fused is instantiated in rt_fused_inst.cu (several translation units, compiled side by side)
+namespace rtm1 {
+#define RT_EXTERN(P, A, B, C_, D_, E_, F_, G_)                                                                                    \
+    extern template __global__ void k_substep_fused<A, B, C_, D_, E_, F_, G_>(const __grid_constant__ GridDev, const __grid_constant__ ParamsDev, const __grid_constant__ OpacDev, \
+        const __grid_constant__ OpacDev, const __grid_constant__ OpacDev, const __grid_constant__ FusedArgs, const __grid_constant__ FusedMaps, int);
+RT_FUSED_INSTANCES(RT_EXTERN)
+#undef RT_EXTERN
+}  // namespace rtm1
 
 using namespace rtm1;
 
@@ -808,9 +818,9 @@ static bool fused_make_maps(const rt_grid* g, const FusedArgs& a, int narr, Fuse
     return true;
 }
 
-template <bool HLL, bool THICK, bool CURVI, bool FEEDBACK, bool RUS, bool HASZ>
+template <bool HLL, bool THICK, bool CURVI, bool FEEDBACK, bool RUS, bool HASZ, bool VARFIX>
 static cudaError_t launch_fused_z(rt_grid* g, const ParamsDev& P, const FusedArgs& a, const FusedMaps& maps, dim3 grid, int seglen) {
-    auto kern = k_substep_fused<HLL, THICK, CURVI, FEEDBACK, RUS, HASZ>;
+    auto kern = k_substep_fused<HLL, THICK, CURVI, FEEDBACK, RUS, HASZ, VARFIX>;
     // the attribute is per device (and per instantiation: this function is a template)
     static bool attr_done[64] = {false};
     const int dev = g->device >= 0 && g->device < 64 ? g->device : 0;
@@ -823,11 +833,14 @@ static cudaError_t launch_fused_z(rt_grid* g, const ParamsDev& P, const FusedArg
     return cudaSuccess;
 }
 
-// x3 active (3-D) or not (2-D)
+// x3 active (3-D) or not (2-D); the comparison face fixes (a.fix != 0; never with the Rusanov solver: fused_eligible)
 template <bool HLL, bool THICK, bool CURVI, bool FEEDBACK, bool RUS = false>
 static cudaError_t launch_fused_t(rt_grid* g, const ParamsDev& P, const FusedArgs& a, const FusedMaps& maps, dim3 grid, int seglen) {
-    return g->dev.gh[2] > 0 ? launch_fused_z<HLL, THICK, CURVI, FEEDBACK, RUS, true>(g, P, a, maps, grid, seglen)
-                            : launch_fused_z<HLL, THICK, CURVI, FEEDBACK, RUS, false>(g, P, a, maps, grid, seglen);
+    if (!RUS && a.fix != 0)
+        return g->dev.gh[2] > 0 ? launch_fused_z<HLL, THICK, CURVI, FEEDBACK, false, true, true>(g, P, a, maps, grid, seglen)
+                                : launch_fused_z<HLL, THICK, CURVI, FEEDBACK, false, false, true>(g, P, a, maps, grid, seglen);
+    return g->dev.gh[2] > 0 ? launch_fused_z<HLL, THICK, CURVI, FEEDBACK, RUS, true, false>(g, P, a, maps, grid, seglen)
+                            : launch_fused_z<HLL, THICK, CURVI, FEEDBACK, RUS, false, false>(g, P, a, maps, grid, seglen);
 }
 
 static cudaError_t launch_fused(rt_grid* g, bool hll, bool thick, bool curvi, bool feedback, const ParamsDev& P,
@@ -900,9 +913,9 @@ static int fused_segment_length(const rt_grid* g, int tiles) {
 
 static bool fused_eligible(const rt_grid* g) {
     const GridDev& D = g->dev;
-    // the comparison face fixes (rt_set_face_fix) exist in the per-direction kernels only
-    return g->fused_seg >= 0 && g->face_fix == RT_FIX_FPRESERVING && D.gh[0] > 0 && D.gh[1] > 0 &&
-           D.ntot < (1LL << 31);  // 32-bit element offsets inside the kernel
+    // the comparison face fixes (rt_set_face_fix) run in the fused kernel too, except with the Rusanov solver
+    return g->fused_seg >= 0 && (g->face_fix == RT_FIX_FPRESERVING || g->par.solver != RT_SOLVER_RUSANOV) && D.gh[0] > 0 &&
+           D.gh[1] > 0 && D.ntot < (1LL << 31);  // 32-bit element offsets inside the kernel
 }
 
 static int32_t fused_impl(rt_grid* g, double* dt_device, double cfl, const double* rho, double* T, double* const mom[3],
@@ -936,6 +949,7 @@ static int32_t fused_impl(rt_grid* g, double* dt_device, double cfl, const doubl
     a.src[4] = thick ? g->lim : nullptr;
     a.kpr = thick ? g->kpr : nullptr;
     a.chat = g->par.chat;
+    a.fix = g->face_fix;
     a.im.rho = rho;
     a.im.T = T;
     for (int q = 0; q < 3; ++q) a.im.mom[q] = feedback ? mom[q] : nullptr;

@@ -32,7 +32,7 @@ struct MetricOut {
     double* cot;
 };
 
-__global__ void k_metric_precompute(GridDev g, MetricOut m) {
+static __global__ void k_metric_precompute(GridDev g, MetricOut m) {
     const int tid = blockIdx.x * blockDim.x + threadIdx.x;
     const int nth = gridDim.x * blockDim.x;
     const int geo = g.geometry;
@@ -96,7 +96,7 @@ __global__ void k_metric_precompute(GridDev g, MetricOut m) {
 }
 
 // Test hook behind rt_grid_get_metrics: full 3-D volume and face areas from the separable factors.
-__global__ void k_metric_expand(GridDev g, double* vol, double* a1, double* a2, double* a3) {
+static __global__ void k_metric_expand(GridDev g, double* vol, double* a1, double* a2, double* a3) {
     const int n1 = g.n[0], n2 = g.n[1], n3 = g.n[2];
     const long long tot = (long long)(n1 + 1) * (n2 + 1) * (n3 + 1);
     for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < tot; t += (long long)gridDim.x * blockDim.x) {
@@ -116,7 +116,7 @@ __global__ void k_metric_expand(GridDev g, double* vol, double* a1, double* a2, 
 // (L291); fixed: untouched (L289).  Axes e < d run over their ghost-extended range.
 // One thread per (ghost layer, side, other-axis position).
 // ------------------------------------------------------------------------------------------------
-__global__ void k_fill_ghosts(GridDev g, Fields4 U, int d) {
+static __global__ void k_fill_ghosts(GridDev g, Fields4 U, int d) {
     int lo[3], ext[3];
     for (int e = 0; e < 3; ++e) {
         lo[e] = (e < d) ? -g.gh[e] : 0;
@@ -156,7 +156,7 @@ __global__ void k_fill_ghosts(GridDev g, Fields4 U, int d) {
 // a1 for the sub-step kernels, ONE launch: the face-normal ghosts of every active axis (other axes over their
 // interior range only).  The scheme never reads edge / corner ghosts — each direction's stencil leaves the
 // interior along its own axis only — so rt_substep does not need the axis-by-axis ordering of k_fill_ghosts.
-__global__ void k_fill_faces(GridDev g, Fields4 U) {
+static __global__ void k_fill_faces(GridDev g, Fields4 U) {
     long long cnt[3], tot = 0;
     for (int d = 0; d < 3; ++d) {
         const int ea = (d == 0) ? 1 : 0, eb = (d == 2) ? 1 : 2;
@@ -205,7 +205,7 @@ struct FiniteArgs {
     const double* f[5];
     int n;
 };
-__global__ void __launch_bounds__(128) k_check_finite(const __grid_constant__ GridDev g, const __grid_constant__ FiniteArgs v,
+static __global__ void __launch_bounds__(128) k_check_finite(const __grid_constant__ GridDev g, const __grid_constant__ FiniteArgs v,
                                                       unsigned long long* __restrict__ bad) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     bool b = false;
@@ -224,7 +224,7 @@ struct AvgArgs {
     const double* b[8];
     int n;
 };
-__global__ void __launch_bounds__(128) k_rk2_average(const __grid_constant__ GridDev g, const __grid_constant__ AvgArgs v) {
+static __global__ void __launch_bounds__(128) k_rk2_average(const __grid_constant__ GridDev g, const __grid_constant__ AvgArgs v) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= g.n[0]) return;
     const long long id = (i + g.gh[0]) + (blockIdx.y + g.gh[1]) * g.stride[1] + (blockIdx.z + g.gh[2]) * g.stride[2];
@@ -238,7 +238,7 @@ __global__ void __launch_bounds__(128) k_rk2_average(const __grid_constant__ Gri
 // (spherical: [A_+ F_+ - A_- F_-]/V of F = L0 e^{-tau}/r^2) or x 1/dx (Cartesian, plane-parallel rays along x1).
 // HBM: 8 B read + 8 B written per cell (+ 8 B with tau_hi).
 // ------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(128) k_irradiation_radial(const __grid_constant__ GridDev g, double L0, double kappa,
+static __global__ void __launch_bounds__(128) k_irradiation_radial(const __grid_constant__ GridDev g, double L0, double kappa,
                                                             double tau_in, const double* __restrict__ rho,
                                                             double* __restrict__ tau_hi, double* __restrict__ div) {
     const int lane = threadIdx.x & 31;
@@ -616,13 +616,13 @@ __device__ __forceinline__ void block_max_to_global(double v, CflScratch* scr, d
 }
 
 // dt = cfl / (running max of the rate), then re-arm the running max (fused-CFL path of k_implicit)
-__global__ void k_cfl_finalize(CflScratch* scr, double cfl, double* dt_out) {
+static __global__ void k_cfl_finalize(CflScratch* scr, double cfl, double* dt_out) {
     const unsigned long long bits = scr->rate_bits;
     scr->rate_bits = 0ull;
     *dt_out = cfl / __longlong_as_double((long long)bits);
 }
 
-__global__ void __launch_bounds__(256) k_cfl(GridDev g, double chat, const double* __restrict__ E, const double* __restrict__ F1,
+static __global__ void __launch_bounds__(256) k_cfl(GridDev g, double chat, const double* __restrict__ E, const double* __restrict__ F1,
                                              const double* __restrict__ F2, const double* __restrict__ F3, CflScratch* scr,
                                              double cfl, double* dt_out) {
     // a persistent-style grid (a few blocks per SM) walks the rows, so that only O(1000) atomics are issued

@@ -67,6 +67,7 @@ struct FusedArgs {
     ImplicitArgs im;           // U = U_out, rho, T, mom, dt / dt_dev, scratch, counters
     double chat;
     int use_tma;
+    int fix;                   // RT_FIX_* (read only by the VARFIX instantiations)
 };
 struct alignas(64) FusedMaps {
     CUtensorMap m[FNARR];      // ghosted (nt1, nt2, nt3) fp64 tensors, box 34 x FPH x 1
@@ -154,7 +155,9 @@ __device__ __forceinline__ void state_load(const double* buf, int t, State& s) {
 // RUS (with HLL = true): RT_SOLVER_RUSANOV, compile-time so that the HLL faces do not pay for the test
 // HASZ = false: 2-D grids (n3 = 1, x3 inactive): one staged plane, no x3 phase; the march degenerates to the steps
 // c = 0 (X, Y) and 1 (FIN, which reads nothing but the thick-limit value of plane 0).
-template <bool HLL, bool THICK, bool CURVI, bool FEEDBACK, bool RUS, bool HASZ>
+// VARFIX = true: the comparison face fixes of rt_set_face_fix (flat fallback L136 / clip Eq. 36-38) selected by the
+// launch-uniform a.fix; false: the paper's f-preserving scheme, compiled in (the default path carries no test for it)
+template <bool HLL, bool THICK, bool CURVI, bool FEEDBACK, bool RUS, bool HASZ, bool VARFIX = false>
 __global__ void __launch_bounds__(FNT, FUSED_MINB)
     k_substep_fused(const __grid_constant__ GridDev g, const __grid_constant__ ParamsDev par, const __grid_constant__ OpacDev oP,
                     const __grid_constant__ OpacDev oR, const __grid_constant__ OpacDev oS, const __grid_constant__ FusedArgs a,
@@ -180,6 +183,7 @@ __global__ void __launch_bounds__(FNT, FUSED_MINB)
     const int o = (ly + 2) * FPW + lx + 2;  // this thread's cell inside a staged plane
     const bool tma = a.use_tma != 0;
     constexpr bool rus = HLL && RUS;
+    const int fix = VARFIX ? a.fix : 0;
     const double dt = a.im.dt_dev ? __ldg(a.im.dt_dev) : a.im.dt;
     const double dtc = dt * a.chat;
 
@@ -266,8 +270,8 @@ __global__ void __launch_bounds__(FNT, FUSED_MINB)
                 dpb[q] = pe[q * FPS + ob + 1] - qb[q];
             }
             State loa, hia, lob, hib;
-            cell_faces<0, HLL>(qa, dma, dpa, false, true, loa, hia);
-            cell_faces<0, HLL>(qb, dpa, dpb, true, false, lob, hib);
+            cell_faces<0, HLL>(qa, dma, dpa, false, true, loa, hia, 0.0, 0.0, 0.0, fix);
+            cell_faces<0, HLL>(qb, dpa, dpb, true, false, lob, hib, 0.0, 0.0, 0.0, fix);
             const double limd = THICK ? dmax(pe[4 * FPS + ob - 1], pe[4 * FPS + ob]) : kInf;
             double fe[4];
             riemann<HLL>(hia, lob, limd, fe, rus);
@@ -334,7 +338,7 @@ __global__ void __launch_bounds__(FNT, FUSED_MINB)
             invEc = frcp(q0[0]);  // 1/E_c, E_c^2, |F_c|^2: shared by the three directions of this cell
             Ec2 = q0[0] * q0[0];
             F2c = fma(q0[3], q0[3], fma(q0[2], q0[2], q0[1] * q0[1]));
-            if (HASZ) cell_faces<2, HLL, true>(q0, dm, dp, true, true, lo, hi, invEc, Ec2, F2c);  // both always: one basic block, two independent chains
+            if (HASZ) cell_faces<2, HLL, true>(q0, dm, dp, true, true, lo, hi, invEc, Ec2, F2c, fix);  // both always: one basic block, two independent chains
             double flz[4] = {0.0, 0.0, 0.0, 0.0};
             if (HASZ && c >= ka) {
                 State L;
@@ -395,7 +399,7 @@ __global__ void __launch_bounds__(FNT, FUSED_MINB)
                 dp[q] = pc[q * FPS + o + 1] - qc[q];
             }
             State lo, hi;
-            cell_faces<0, HLL, true>(qc, dm, dp, true, true, lo, hi, invEc, Ec2, F2c);
+            cell_faces<0, HLL, true>(qc, dm, dp, true, true, lo, hi, invEc, Ec2, F2c, fix);
             State L;
 #pragma unroll
             for (int q = 0; q < 4; ++q) {
@@ -453,7 +457,7 @@ __global__ void __launch_bounds__(FNT, FUSED_MINB)
                 dp[q] = pc[q * FPS + o + FPW] - qc[q];
             }
             State hi;
-            cell_faces<1, HLL, true>(qc, dm, dp, true, true, ylo, hi, invEc, Ec2, F2c);
+            cell_faces<1, HLL, true>(qc, dm, dp, true, true, ylo, hi, invEc, Ec2, F2c, fix);
             if (ly < FTY - 1) {
                 state_store<HLL, FNT>(yex, tid, hi);
                 pair_arrive(1 + ly);
@@ -467,7 +471,7 @@ __global__ void __launch_bounds__(FNT, FUSED_MINB)
                     dpa[q] = pc[q * FPS + o + 2 * FPW] - qa[q];
                 }
                 State loa, hia;
-                cell_faces<1, HLL>(qa, dma, dpa, true, false, loa, hia);
+                cell_faces<1, HLL>(qa, dma, dpa, true, false, loa, hia, 0.0, 0.0, 0.0, fix);
                 const double limd = THICK ? dmax(pc[4 * FPS + o], pc[4 * FPS + o + FPW]) : kInf;
                 double fup[4];
                 riemann<HLL>(hi, loa, limd, fup, rus);
@@ -491,7 +495,7 @@ __global__ void __launch_bounds__(FNT, FUSED_MINB)
                     dpb[q] = qc[q] - qb[q];
                 }
                 State lob;
-                cell_faces<1, HLL>(qb, dmb, dpb, false, true, lob, L);
+                cell_faces<1, HLL>(qb, dmb, dpb, false, true, lob, L, 0.0, 0.0, 0.0, fix);
             }
             const double limd = THICK ? dmax(pc[4 * FPS + o - FPW], pc[4 * FPS + o]) : kInf;
             double fly[4];

@@ -557,9 +557,10 @@ TOL_CLIP = 1e-7  # Eq. 38 puts face states ON f = 1 up to rounding, where zeta (
 @pytest.mark.parametrize("case", ["cart3d", "sph3d", "cyl2d", "cart1d"])
 @pytest.mark.parametrize("fix", [W.FIX_PLUTO, W.FIX_CLIP])
 def test_face_fix_variants(rt, case, fix):
-    """rt_set_face_fix: the flat fallback of L136 and the clip of Eq. 36-38 in the per-direction kernels, 2 sub-steps on
-    random states with f up to 1 against the oracle; rt_substep falls back to the same kernels (bit-identical fields);
-    and the variant is not the default scheme (the fields differ by far more than the gate)."""
+    """rt_set_face_fix: the flat fallback of L136 and the clip of Eq. 36-38, 2 sub-steps on random states with f up to 1
+    against the oracle, through the per-direction kernels (rt_explicit_step) and through rt_substep (the VARFIX
+    instantiations of the fused kernel on 2-D / 3-D grids, k_substep_1d on the 1-D one; with the Rusanov solver the
+    per-direction kernels); and the variant is not the default scheme (the fields differ by far more than the gate)."""
     geometry, n, solver = {"cart3d": (W.CARTESIAN, (70, 33, 12), W.SOLVER_HLL), "sph3d": (W.SPHERICAL, (45, 20, 17), W.SOLVER_RUSANOV),
                            "cyl2d": (W.CYLINDRICAL, (64, 40, 1), W.SOLVER_GLF), "cart1d": (W.CARTESIAN, (300, 1, 1), W.SOLVER_HLL)}[case]
     w = random_workload(geometry, n, solver, 1, seed=90 + fix, fmax=1.0)
@@ -576,7 +577,7 @@ def test_face_fix_variants(rt, case, fix):
         it = w.interior
         e = np.abs(st.U[0].cpu().numpy()[it] - refU[0][it]) / np.abs(refU[0][it]).max()
         assert np.median(e) <= TOL1
-    # rt_substep with a variant selected: the split kernels, with the device-resident dt
+    # rt_substep with a variant selected (device-resident dt)
     g2 = drv.grid_from_workload(w)
     g2.set_face_fix(fix)
     st2, _, hist = drv.run_substeps_fused(g2, w, 2)
