@@ -43,6 +43,10 @@ enum { RT_FIX_FPRESERVING = 0 /* Eq. 19-21, the paper's scheme and the 
        RT_FIX_PLUTO = 1 /* flat fallback U_f = U_c whenever |R(F)| > R(E), L136 */,
        RT_FIX_CLIP = 2 /* Eq. 36-38: F_f = R(F) R(E)/|R(F)| whenever |R(F)| > R(E) */ };
 
+/* the "standard reconstruction method" R() of Sect. 2.5 (L132) */
+enum { RT_RECON_PLM = 0 /* piecewise linear, van Leer limiter (R-G3): the default */,
+       RT_RECON_LIMO3 = 1 /* compact third-order, Cada & Torrilhon 2009 (the scheme of the paper's Fig. 1-5; R-G22) */ };
+
 typedef struct rt_grid rt_grid; /* opaque */
 
 typedef struct {
@@ -113,6 +117,15 @@ int32_t rt_implicit_step(rt_grid* g, double dt, const double* rho, double* T,
  * combination with RT_SOLVER_RUSANOV makes rt_substep / rt_rk2_step take the per-direction kernels.  Unknown mode ->
  * RT_ERR_INVALID_ARG, state unchanged.  Host call, nothing enqueued. */
 int32_t rt_set_face_fix(rt_grid* g, int32_t mode);
+
+/* Reconstruction of the explicit half (step a2; L132).  RT_RECON_LIMO3 (DESIGN R-G22): with d- = u_i - u_{i-1},
+ * d+ = u_{i+1} - u_i, theta = d-/d+: u(upper face) = u_i + phi(theta) d+/2, u(lower face) = u_i - phi(1/theta) d-/2,
+ * phi_3 = (2 + theta)/3, phi_L = max(0, min(phi_3, max(-theta/2, min(2 theta, phi_3, 1.6)))); r > 0 switches the limiter
+ * off (phi = phi_3) where eta = (d-^2 + d+^2)/(r dl)^2 <= 1 (dl = the cell's length along the direction: smooth extrema keep
+ * third order), r <= 0 applies phi_L everywhere.  eta compares field differences with lengths, as in the original: choose r
+ * for the units of the fields.  LimO3 runs in the per-direction kernels and the 1-D kernel (rt_substep on 2-D / 3-D
+ * grids then takes the per-direction path).  Unknown kind / non-finite r -> RT_ERR_INVALID_ARG.  Host call. */
+int32_t rt_set_reconstruction(rt_grid* g, int32_t kind, double r);
 
 /* Irradiation (Sect. 2.9, Eq. 34-35): div_firr = DEVICE array (field layout, caller-owned, must stay valid)
  * of the divergence of a user-defined irradiation flux; every later implicit half adds Q = -div_firr dt to S_1 of

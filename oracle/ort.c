@@ -44,6 +44,8 @@ struct ort_grid {
     long long n_floor, n_clip;
     const double* div_firr; /* caller-owned, ghosted layout, or NULL (Sect. 2.9) */
     int face_fix;           /* ORT_FIX_* (zero-initialised: the f-preserving scheme of Eq. 19-21) */
+    int recon;              /* ORT_RECON_* (zero-initialised: PLM + van Leer) */
+    double limo3_r;         /* LimO3: radius of the asymptotic region in units of the cell length (<= 0: no switch) */
 };
 
 /* ------------------------------------------------------------------------------------------ */
@@ -103,6 +105,39 @@ double ort_vanleer_slope(double qm, double q0, double qp) {
     double dm = q0 - qm, dp = qp - q0;
     if (dm * dp > 0.0) return 2.0 * dm * dp / (dm + dp);
     return 0.0;
+}
+
+/* Compact third-order reconstruction LimO3 (L132: Cada & Torrilhon 2009, J. Comput. Phys. 228, 4118; the formula is not
+ * printed in PAPER.md: DESIGN R-G22 restates it).  With d- = u_i - u_{i-1}, d+ = u_{i+1} - u_i, theta = d-/d+:
+ *   u at the upper face = u_i + 1/2 phi(theta)   d+,      u at the lower face = u_i - 1/2 phi(1/theta) d-,
+ *   phi_3(theta)  = (2 + theta)/3                              (unlimited: the quadratic through the three cell averages)
+ *   phi_L(theta)  = max(0, min(phi_3, max(-theta/2, min(2 theta, phi_3, 1.6))))
+ *   eta = (d-^2 + d+^2)/(r dx)^2;  phi = phi_3 if eta <= 1 - eps, phi_L if eta >= 1 + eps, their linear blend in between,
+ *   eps = 1e-12; r <= 0 switches the smooth-extremum detector off (phi = phi_L).
+ * A vanishing denominator: phi(theta) d+ -> 0 as d+ -> 0 (phi_L is bounded by 1.6 and by 0 for theta -> -inf). */
+static double limo3_phi_times(double dnum, double dden, double eta_or_neg) {
+    /* returns phi(dnum/dden) * dden.  phi_3(theta) d+ = (2 d+ + d-)/3 needs no quotient; phi_L(theta) d+ -> 0 for d+ -> 0 */
+    double p3 = (2.0 * dden + dnum) / 3.0;
+    double pL = 0.0;
+    if (dden != 0.0) {
+        double theta = dnum / dden;
+        double phi3 = (2.0 + theta) / 3.0;
+        pL = fmax(0.0, fmin(phi3, fmax(-0.5 * theta, fmin(fmin(2.0 * theta, phi3), 1.6)))) * dden;
+    }
+    if (eta_or_neg < 0.0) return pL; /* no smoothness switch */
+    const double eps = 1.0e-12;
+    double eta = eta_or_neg;
+    if (eta <= 1.0 - eps) return p3;
+    if (eta >= 1.0 + eps) return pL;
+    return 0.5 * ((1.0 - (eta - 1.0) / eps) * p3 + (1.0 + (eta - 1.0) / eps) * pL);
+}
+
+void ort_limo3_faces(double um, double u0, double up, double dx, double r, double* lo, double* hi) {
+    double dm = u0 - um, dp = up - u0;
+    double eta = -1.0;
+    if (r > 0.0) eta = (dm * dm + dp * dp) / ((r * dx) * (r * dx));
+    *hi = u0 + 0.5 * limo3_phi_times(dm, dp, eta);   /* theta = d-/d+ */
+    *lo = u0 - 0.5 * limo3_phi_times(dp, dm, eta);   /* 1/theta = d+/d- */
 }
 
 /* Eq. 19-21 (L140-146), DESIGN R-G4.  E_f = R(E).  Keep F_f = R(F) iff ||R(F)||/R(E) <= 1 and
@@ -479,15 +514,19 @@ int32_t ort_fill_ghosts(ort_grid* g, double* const U[4]) {
  * or, on request, the flat fallback of L136 / the clip of Eq. 36-38: ort_set_face_fix)
  * for the cell's lower-face state (the RIGHT state of face i-1/2) and upper-face state (the LEFT
  * state of face i+1/2). */
-static void cell_face_states(const ort_grid* g, double* const U[4], long idx, long stride,
+static void cell_face_states(const ort_grid* g, double* const U[4], long idx, long stride, double dx,
                              double Ulo[4], double Uhi[4]) {
     double Uc[4], Rlo[4], Rhi[4];
     for (int q = 0; q < 4; ++q) {
         double qm = U[q][idx - stride], q0 = U[q][idx], qp = U[q][idx + stride];
-        double slope = ort_vanleer_slope(qm, q0, qp);
         Uc[q] = q0;
-        Rlo[q] = q0 - 0.5 * slope;
-        Rhi[q] = q0 + 0.5 * slope;
+        if (g->recon == ORT_RECON_LIMO3) {
+            ort_limo3_faces(qm, q0, qp, dx, g->limo3_r, &Rlo[q], &Rhi[q]);
+        } else {
+            double slope = ort_vanleer_slope(qm, q0, qp);
+            Rlo[q] = q0 - 0.5 * slope;
+            Rhi[q] = q0 + 0.5 * slope;
+        }
     }
     if (g->face_fix == ORT_FIX_PLUTO) {
         ort_pluto_face(Uc, Rlo, Ulo);
@@ -559,8 +598,16 @@ int32_t ort_explicit_step(ort_grid* g, double dt, const double* rho, const doubl
                     /* face between cell a = (i,j,k) - e_d and cell b = (i,j,k) */
                     long ib = IDX(g, i, j, k), ia = ib - stride[d];
                     double aLo[4], aHi[4], bLo[4], bHi[4];
-                    cell_face_states(g, U_in, ia, stride[d], aLo, aHi);
-                    cell_face_states(g, U_in, ib, stride[d], bLo, bHi);
+                    /* LimO3's smoothness switch wants the cell's length along d (ghost cells: that of the nearest
+                     * interior cell) */
+                    int ca[3] = {i, j, k}, cb[3] = {i, j, k};
+                    ca[d] -= 1;
+                    for (int e = 0; e < 3; ++e) {
+                        ca[e] = ca[e] < 0 ? 0 : (ca[e] > g->n[e] - 1 ? g->n[e] - 1 : ca[e]);
+                        cb[e] = cb[e] > g->n[e] - 1 ? g->n[e] - 1 : cb[e];
+                    }
+                    cell_face_states(g, U_in, ia, stride[d], cell_length(g, d, ca[0], ca[1], ca[2]), aLo, aHi);
+                    cell_face_states(g, U_in, ib, stride[d], cell_length(g, d, cb[0], cb[1], cb[2]), bLo, bHi);
                     double lim = INFINITY;
                     if (p->thick_limit) {
                         double tf = fmin(tau[ia], tau[ib]);
@@ -634,6 +681,14 @@ int32_t ort_explicit_step(ort_grid* g, double dt, const double* rho, const doubl
 int32_t ort_set_face_fix(ort_grid* g, int32_t mode) {
     if (!g || mode < ORT_FIX_FPRESERVING || mode > ORT_FIX_CLIP) return ORT_ERR_INVALID_ARG;
     g->face_fix = mode;
+    return ORT_OK;
+}
+
+/* L132: which standard reconstruction R() the explicit step applies */
+int32_t ort_set_reconstruction(ort_grid* g, int32_t kind, double r) {
+    if (!g || (kind != ORT_RECON_PLM && kind != ORT_RECON_LIMO3) || !isfinite(r)) return ORT_ERR_INVALID_ARG;
+    g->recon = kind;
+    g->limo3_r = r;
     return ORT_OK;
 }
 

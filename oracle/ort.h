@@ -27,6 +27,10 @@ enum { ORT_OPAC_PLANCK = 0, ORT_OPAC_ROSSELAND = 1, ORT_OPAC_SCATTER = 2 };
 /* how f <= 1 is enforced on the reconstructed face states (Sect. 2.5, Sect. 3.2 Eq. 36-38) */
 enum { ORT_FIX_FPRESERVING = 0 /* Eq. 19-21 */, ORT_FIX_PLUTO = 1 /* flat fallback, L136 */, ORT_FIX_CLIP = 2 /* Eq. 36-38 */ };
 
+/* the "standard reconstruction method" R() of Sect. 2.5 (L132): PLM with the van Leer limiter, or the compact third-order
+ * LimO3 of Cada & Torrilhon 2009 (the scheme of the paper's Fig. 1-5); DESIGN.md R-G22 */
+enum { ORT_RECON_PLM = 0, ORT_RECON_LIMO3 = 1 };
+
 typedef struct {
     double chat;    /* reduced speed of light, PAPER.md:L179 (Sect. 2.7) */
     double c;       /* speed of light in code units */
@@ -85,6 +89,12 @@ void ort_fpreserving_face(const double Uc[4], const double RU[4], double Uf[4]);
 void ort_pluto_face(const double Uc[4], const double RU[4], double Uf[4]);
 /* Eq. 36-38: E_f = R(E); F_f = R(F) if ||R(F)|| <= R(E), else R(F) R(E)/||R(F)|| */
 void ort_clip_face(const double RU[4], double Uf[4]);
+/* LimO3 (L132; Cada & Torrilhon 2009; DESIGN R-G22) for one field of one cell: values um, u0, up of the cells i-1, i, i+1,
+ * the cell's length dx along the direction and the radius r of the asymptotic region (r <= 0: the limiter alone, no
+ * smoothness switch) -> the values at the cell's lower and upper face */
+void ort_limo3_faces(double um, double u0, double up, double dx, double r, double* lo, double* hi);
+/* which reconstruction the explicit step applies (default ORT_RECON_PLM) and LimO3's r */
+int32_t ort_set_reconstruction(ort_grid* g, int32_t kind, double r);
 /* which of the three the explicit step applies (default ORT_FIX_FPRESERVING) */
 int32_t ort_set_face_fix(ort_grid* g, int32_t mode);
 /* L150 (R-G5,G6,G8): face flux from the two face states; lim = 4 chat/(3 tau_face) or +inf */

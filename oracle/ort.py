@@ -20,6 +20,7 @@ CARTESIAN, CYLINDRICAL, SPHERICAL = 0, 1, 2
 BC_PERIODIC, BC_OUTFLOW, BC_REFLECT, BC_FIXED = 0, 1, 2, 3
 SOLVER_HLL, SOLVER_GLF, SOLVER_RUSANOV = 0, 1, 2
 FIX_FPRESERVING, FIX_PLUTO, FIX_CLIP = 0, 1, 2
+RECON_PLM, RECON_LIMO3 = 0, 1
 OPAC_PLANCK, OPAC_ROSSELAND, OPAC_SCATTER = 0, 1, 2
 
 _dp = C.POINTER(C.c_double)
@@ -74,6 +75,10 @@ def lib():
         L.ort_pluto_face.argtypes = [_dp, _dp, _dp]
         L.ort_clip_face.restype = None
         L.ort_clip_face.argtypes = [_dp, _dp]
+        L.ort_limo3_faces.restype = None
+        L.ort_limo3_faces.argtypes = [C.c_double] * 5 + [_dp, _dp]
+        L.ort_set_reconstruction.restype = C.c_int32
+        L.ort_set_reconstruction.argtypes = [C.c_void_p, C.c_int32, C.c_double]
         L.ort_set_face_fix.restype = C.c_int32
         L.ort_set_face_fix.argtypes = [C.c_void_p, C.c_int32]
         L.ort_riemann_flux.restype = None
@@ -143,6 +148,13 @@ def wave_speeds(E, F, d):
 
 def vanleer_slope(qm, q0, qp):
     return lib().ort_vanleer_slope(float(qm), float(q0), float(qp))
+
+
+def limo3_faces(um, u0, up, dx=1.0, r=0.0):
+    """LimO3 (Cada & Torrilhon 2009) face values (lower, upper) of the middle cell"""
+    lo, hi = np.empty(1), np.empty(1)
+    lib().ort_limo3_faces(float(um), float(u0), float(up), float(dx), float(r), _p(lo), _p(hi))
+    return lo[0], hi[0]
 
 
 def fpreserving_face(Uc, RU):
@@ -284,6 +296,12 @@ class Grid:
                                      _ptrs(U))
         if rc != 0:
             raise ValueError("ort_implicit_step failed with status %d" % rc)
+
+    def set_reconstruction(self, kind, r=0.0):
+        """RECON_PLM (van Leer, default) or RECON_LIMO3 with its asymptotic-region radius r (<= 0: limiter alone)"""
+        rc = lib().ort_set_reconstruction(self._h, int(kind), float(r))
+        if rc != 0:
+            raise ValueError("ort_set_reconstruction failed with status %d" % rc)
 
     def set_face_fix(self, mode):
         """FIX_FPRESERVING (Eq. 19-21, default), FIX_PLUTO (flat fallback, L136) or FIX_CLIP (Eq. 36-38)"""

@@ -36,6 +36,8 @@ struct rt_grid {
     double* rk_dt;       // rt_rk2_step: the dt each stage reads (and overwrites)
     const double* divfirr;  // rt_set_irradiation: caller-owned device array or nullptr
     int face_fix;  // rt_set_face_fix: RT_FIX_*
+    int recon;     // rt_set_reconstruction: RT_RECON_*
+    double limo3_r;
     double* kpr;  // rho kappa_P per cell, written by the pre-pass of the fused sub-step (lazily allocated)
     CflScratch* scr;
     double* dt_dev;
@@ -224,6 +226,8 @@ extern "C" int32_t rt_grid_create(int32_t geometry, const int32_t n[3], int32_t 
     g->kpr = nullptr;
     g->divfirr = nullptr;
     g->face_fix = RT_FIX_FPRESERVING;
+    g->recon = RT_RECON_PLM;
+    g->limo3_r = 0.0;
     for (int q = 0; q < 4; ++q) g->rk_save[q] = nullptr;
     g->rk_dt = nullptr;
     g->scr = nullptr;
@@ -652,6 +656,8 @@ static int32_t explicit_impl(rt_grid* g, double dt, const double* dt_dev, const 
     a.chat = g->par.chat;
     a.rusanov = g->par.solver == RT_SOLVER_RUSANOV;
     a.fix = g->face_fix;
+    a.recon = g->recon;
+    a.limo3_r = g->limo3_r;
     const bool hll = g->par.solver != RT_SOLVER_GLF;  // HLL and Rusanov need the wave speeds
     const bool curvi = D.geometry != RT_CARTESIAN;
     if (D.gh[0] == 0) {
@@ -732,6 +738,16 @@ static int32_t implicit_impl(rt_grid* g, double dt, const double* dt_dev, const 
         }
         RT_LAUNCH_CHECK(g);
     }
+    return RT_OK;
+}
+
+extern "C" int32_t rt_set_reconstruction(rt_grid* g, int32_t kind, double r) {
+    DeviceGuard dg_(g);
+    if (!g) return RT_ERR_INVALID_ARG;
+    if ((kind != RT_RECON_PLM && kind != RT_RECON_LIMO3) || !isfinite(r))
+        return fail(g, RT_ERR_INVALID_ARG, "rt_set_reconstruction: unknown kind %d or non-finite r", kind);
+    g->recon = kind;
+    g->limo3_r = r;
     return RT_OK;
 }
 
@@ -914,7 +930,9 @@ static int fused_segment_length(const rt_grid* g, int tiles) {
 static bool fused_eligible(const rt_grid* g) {
     const GridDev& D = g->dev;
     // the comparison face fixes (rt_set_face_fix) run in the fused kernel too, except with the Rusanov solver
-    return g->fused_seg >= 0 && (g->face_fix == RT_FIX_FPRESERVING || g->par.solver != RT_SOLVER_RUSANOV) && D.gh[0] > 0 &&
+    // LimO3 (rt_set_reconstruction) exists in the per-direction kernels and the 1-D kernel only
+    return g->fused_seg >= 0 && g->recon == RT_RECON_PLM &&
+           (g->face_fix == RT_FIX_FPRESERVING || g->par.solver != RT_SOLVER_RUSANOV) && D.gh[0] > 0 &&
            D.gh[1] > 0 && D.ntot < (1LL << 31);  // 32-bit element offsets inside the kernel
 }
 
@@ -1050,6 +1068,8 @@ static int32_t oned_impl(rt_grid* g, double* dt_device, double cfl, const double
     sw.chat = g->par.chat;
     sw.rusanov = g->par.solver == RT_SOLVER_RUSANOV;
     sw.fix = g->face_fix;
+    sw.recon = g->recon;
+    sw.limo3_r = g->limo3_r;
     ImplicitArgs a;
     for (int q = 0; q < 4; ++q) a.U[q] = U_out[q];
     a.rho = rho;

@@ -26,7 +26,24 @@ struct SweepArgs {
     double chat;
     int rusanov;  // RT_SOLVER_RUSANOV (the HLL instantiation computes the wave speeds it needs)
     int fix;      // RT_FIX_* (rt_set_face_fix): 0 = f-preserving (Eq. 19-21), 1 = flat fallback (L136), 2 = clip (Eq. 36-38)
+    int recon;    // RT_RECON_* (rt_set_reconstruction): 0 = PLM + van Leer, 1 = LimO3 (L132)
+    double limo3_r;  // LimO3: radius of the asymptotic region in cell lengths (<= 0: no smoothness switch)
 };
+
+// both face states of one cell with the reconstruction the launch selected (a uniform branch: two code copies)
+template <int D, bool HLL>
+__device__ __forceinline__ void cell_faces_sel(const SweepArgs& a, const double q0[4], const double dm[4], const double dp[4],
+                                               bool want_lo, bool want_hi, State& lo, State& hi, double dx) {
+    if (a.recon) cell_faces<D, HLL, false, true>(q0, dm, dp, want_lo, want_hi, lo, hi, 0.0, 0.0, 0.0, a.fix, a.limo3_r * dx);
+    else cell_faces<D, HLL>(q0, dm, dp, want_lo, want_hi, lo, hi, 0.0, 0.0, 0.0, a.fix);
+}
+// the cell's length along D (LimO3's smoothness switch); ghost cells take the nearest interior cell's
+__device__ __forceinline__ double cell_len(const GridDev& g, int D, int i, int j, int k) {
+    i = min(max(i, 0), g.n[0] - 1);
+    j = min(max(j, 0), g.n[1] - 1);
+    k = min(max(k, 0), g.n[2] - 1);
+    return g.len[D][0][i] * g.len[D][1][j] * g.len[D][2][k];
+}
 
 __device__ __forceinline__ double sweep_dtc(const SweepArgs& a) { return a.dt_dev ? __ldg(a.dt_dev) * a.chat : a.dtc; }
 
@@ -68,7 +85,7 @@ __global__ void __launch_bounds__(128) k_sweep_x(const __grid_constant__ GridDev
     if (THICK) limd = dmax(a.lim[id - 1], a.lim[id]);
 
     State lo, hi;
-    cell_faces<0, HLL>(q0, dm, dp, true, true, lo, hi, 0.0, 0.0, 0.0, a.fix);
+    cell_faces_sel<0, HLL>(a, q0, dm, dp, true, true, lo, hi, a.recon ? cell_len(g, 0, i, j, k) : 0.0);
 
     // left state of this lane's lower face = upper-face state of the lane below
     State L;
@@ -177,7 +194,11 @@ __global__ void __launch_bounds__(128) k_sweep_march(const __grid_constant__ Gri
 #pragma unroll
         for (int q = 0; q < 4; ++q) dp[q] = qn[q] - qc[q];
         State lo, hi;
-        cell_faces<D, HLL>(qc, dm, dp, c >= ca, c < cb, lo, hi, 0.0, 0.0, 0.0, a.fix);
+        {
+            double dxc = 0.0;
+            if (a.recon) dxc = D == 1 ? cell_len(g, 1, i, c, o) : cell_len(g, 2, i, o, c);
+            cell_faces_sel<D, HLL>(a, qc, dm, dp, c >= ca, c < cb, lo, hi, dxc);
+        }
         if (c >= ca) {
             double fl[4];
             riemann<HLL>(hiPrev, lo, THICK ? dmax(limp, limc) : kInf, fl, a.rusanov != 0);
@@ -396,8 +417,8 @@ __global__ void __launch_bounds__(K1D_NT) k_substep_1d(const __grid_constant__ G
             dpb[q] = sU[q][i + 3] - qb[q];
         }
         State loa, hia, lob, hib;
-        cell_faces<0, HLL>(qa, dma, dpa, false, true, loa, hia, 0.0, 0.0, 0.0, sw.fix);
-        cell_faces<0, HLL>(qb, dpa, dpb, true, false, lob, hib, 0.0, 0.0, 0.0, sw.fix);
+        cell_faces_sel<0, HLL>(sw, qa, dma, dpa, false, true, loa, hia, sw.recon ? cell_len(g, 0, i - 1, 0, 0) : 0.0);
+        cell_faces_sel<0, HLL>(sw, qb, dpa, dpb, true, false, lob, hib, sw.recon ? cell_len(g, 0, i, 0, 0) : 0.0);
         const double limd = THICK ? dmax(sLim[i], sLim[i + 1]) : kInf;
         double fe[4];
         riemann<HLL>(hia, lob, limd, fe, sw.rusanov != 0);

@@ -197,6 +197,29 @@ __device__ __forceinline__ double half_slope(double dm, double dp) {
     return pr > 0.0 ? h : 0.0;
 }
 
+// LimO3 (L132; Cada & Torrilhon 2009; DESIGN R-G22): phi(dnum/dden) dden without the quotient.  With s = sign(dden),
+// a = |dden|, b = s dnum and P = s (2 dden + dnum)/3 = a phi_3:  a phi_L = max(0, min(P, max(-b/2, min(2b, P, 1.6a)))),
+// which is 0 for dden = 0 as the limit demands.  eta < 0: no smoothness switch (phi = phi_L); else phi_3 below
+// eta = 1 - eps, phi_L above 1 + eps, their blend in between (eps = 1e-12).
+__device__ __forceinline__ double limo3_times(double dnum, double dden, double eta) {
+    const double p3 = (2.0 * dden + dnum) * (1.0 / 3.0);
+    const bool neg = dden < 0.0;
+    const double a = fabs(dden), b = neg ? -dnum : dnum, P = neg ? -p3 : p3;
+    const double inner = dmin(dmin(b + b, P), 1.6 * a);
+    const double pl = dmax(0.0, dmin(P, dmax(-0.5 * b, inner)));
+    const double pL = neg ? -pl : pl;
+    if (eta < 0.0) return pL;
+    constexpr double eps = 1.0e-12;
+    if (eta <= 1.0 - eps) return p3;
+    if (eta >= 1.0 + eps) return pL;
+    return 0.5 * ((1.0 - (eta - 1.0) / eps) * p3 + (1.0 + (eta - 1.0) / eps) * pL);
+}
+// the smoothness indicator (d-^2 + d+^2)/(r dx)^2, rounded operation by operation: it DECIDES which branch a face
+// takes, so it is evaluated exactly as the oracle evaluates it (no contraction into fused multiply-adds)
+__device__ __forceinline__ double limo3_eta(double dm, double dp, double rdx) {
+    return __ddiv_rn(__dadd_rn(__dmul_rn(dm, dm), __dmul_rn(dp, dp)), __dmul_rn(rdx, rdx));
+}
+
 // f-preserving face state (Eq. 19-21; R-G4).  Uc = cell value, invEc = 1/E_c,
 // Ec2 = E_c^2, F2c = |F_c|^2; on entry st.U holds the reconstructed R(U) = Uc + sh (sh = the signed half slope, of
 // which dE = sh[0] is passed in); on exit the face state.  Returns through E2f/F2f the squares of the final face state.
@@ -284,30 +307,40 @@ __device__ __forceinline__ void riemann(const State& L, const State& R, double l
 // (LEFT state of face c+1/2).  WANT_LO / WANT_HI are warp-uniform run-time flags.
 // KNOWN: the caller passes 1/E_c, E_c^2 and |F_c|^2 (the three directions of one cell share them).
 // fix (launch-uniform; RT_FIX_*): 0 = the f-preserving scheme; the fused kernel never passes anything else.
-template <int D, bool HLL, bool KNOWN = false>
+// LIMO3: the compact third-order reconstruction instead of PLM; rdx = r x the cell's length along D (<= 0: no
+// smoothness switch).  The per-direction kernels and the 1-D kernel only.
+template <int D, bool HLL, bool KNOWN = false, bool LIMO3 = false>
 __device__ __forceinline__ void cell_faces(const double q0[4], const double dm[4], const double dp[4], bool want_lo,
                                            bool want_hi, State& lo, State& hi, double invEc_known = 0.0,
-                                           double Ec2_known = 0.0, double F2c_known = 0.0, int fix = 0) {
-    double h[4];
+                                           double Ec2_known = 0.0, double F2c_known = 0.0, int fix = 0, double rdx = 0.0) {
+    double hlo[4], hhi[4];  // U at the lower face = q0 - hlo, at the upper face = q0 + hhi
 #pragma unroll
-    for (int q = 0; q < 4; ++q) h[q] = half_slope(dm[q], dp[q]);
+    for (int q = 0; q < 4; ++q) {
+        if (LIMO3) {
+            const double eta = rdx > 0.0 ? limo3_eta(dm[q], dp[q], rdx) : -1.0;
+            hhi[q] = 0.5 * limo3_times(dm[q], dp[q], eta);
+            hlo[q] = 0.5 * limo3_times(dp[q], dm[q], eta);
+        } else {
+            hlo[q] = hhi[q] = half_slope(dm[q], dp[q]);
+        }
+    }
     const double Ec = q0[0];
     const double Ec2 = KNOWN ? Ec2_known : Ec * Ec;
     const double F2c = KNOWN ? F2c_known : fma(q0[3], q0[3], fma(q0[2], q0[2], q0[1] * q0[1]));
     const double invEc = KNOWN ? invEc_known : frcp(Ec);
     if (want_lo) {
 #pragma unroll
-        for (int q = 0; q < 4; ++q) lo.U[q] = q0[q] - h[q];
+        for (int q = 0; q < 4; ++q) lo.U[q] = q0[q] - hlo[q];
         double E2f, F2f;
-        if (fix == 0) fpreserve(lo, q0, -h[0], invEc, Ec2, F2c, E2f, F2f);
+        if (fix == 0) fpreserve(lo, q0, -hlo[0], invEc, Ec2, F2c, E2f, F2f);
         else facefix_variant(fix, lo, q0, Ec2, F2c, E2f, F2f);
         flux_and_speeds<D, HLL>(lo, E2f, F2f);
     }
     if (want_hi) {
 #pragma unroll
-        for (int q = 0; q < 4; ++q) hi.U[q] = q0[q] + h[q];
+        for (int q = 0; q < 4; ++q) hi.U[q] = q0[q] + hhi[q];
         double E2f, F2f;
-        if (fix == 0) fpreserve(hi, q0, h[0], invEc, Ec2, F2c, E2f, F2f);
+        if (fix == 0) fpreserve(hi, q0, hhi[0], invEc, Ec2, F2c, E2f, F2f);
         else facefix_variant(fix, hi, q0, Ec2, F2c, E2f, F2f);
         flux_and_speeds<D, HLL>(hi, E2f, F2f);
     }

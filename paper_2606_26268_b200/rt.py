@@ -18,6 +18,7 @@ CARTESIAN, CYLINDRICAL, SPHERICAL = 0, 1, 2
 BC_PERIODIC, BC_OUTFLOW, BC_REFLECT, BC_FIXED = 0, 1, 2, 3
 SOLVER_HLL, SOLVER_GLF, SOLVER_RUSANOV = 0, 1, 2
 FIX_FPRESERVING, FIX_PLUTO, FIX_CLIP = 0, 1, 2
+RECON_PLM, RECON_LIMO3 = 0, 1
 OPAC_PLANCK, OPAC_ROSSELAND, OPAC_SCATTER = 0, 1, 2
 OK, ERR_INVALID_ARG, ERR_BAD_STATE, ERR_CUDA, ERR_NOT_FINITE = 0, 1, 2, 3, 4
 NGHOST = 2
@@ -67,6 +68,7 @@ _SIGNATURES = {
                                C.POINTER(C.c_void_p), C.POINTER(C.c_void_p)]),
     "rt_set_irradiation": (C.c_int32, [C.c_void_p, C.c_void_p]),
     "rt_set_face_fix": (C.c_int32, [C.c_void_p, C.c_int32]),
+    "rt_set_reconstruction": (C.c_int32, [C.c_void_p, C.c_int32, C.c_double]),
     "rt_irradiation_radial": (C.c_int32, [C.c_void_p, C.c_double, C.c_double, C.c_double, C.c_void_p, C.c_void_p, C.c_void_p]),
     "rt_rk2_step": (C.c_int32, [C.c_void_p, C.c_void_p, C.c_double, C.c_void_p, C.c_void_p, C.POINTER(C.c_void_p),
                                 C.POINTER(C.c_void_p), C.POINTER(C.c_void_p), C.POINTER(C.c_void_p)]),
@@ -314,6 +316,11 @@ class Grid:
                               _ptr_array(mom) if mom is not None else None, _ptr_array(U_in), _ptr_array(U_out))
         if rc != OK:
             self._raise("rt_substep", rc)
+
+    def set_reconstruction(self, kind, r=0.0):
+        rc = lib().rt_set_reconstruction(self._h, int(kind), float(r))
+        if rc != OK:
+            self._raise("rt_set_reconstruction", rc)
 
     def set_face_fix(self, mode):
         rc = lib().rt_set_face_fix(self._h, int(mode))

@@ -18,6 +18,7 @@ SEED0 = 2606_26268
 CARTESIAN, CYLINDRICAL, SPHERICAL = 0, 1, 2
 BC_PERIODIC, BC_OUTFLOW, BC_REFLECT, BC_FIXED = 0, 1, 2, 3
 SOLVER_HLL, SOLVER_GLF, SOLVER_RUSANOV = 0, 1, 2
+RECON_PLM, RECON_LIMO3 = 0, 1  # reconstruction of the explicit half (rt_set_reconstruction / ort_set_reconstruction)
 FIX_FPRESERVING, FIX_PLUTO, FIX_CLIP = 0, 1, 2  # face fix of the explicit half (rt_set_face_fix / ort_set_face_fix)
 OPAC_PLANCK, OPAC_ROSSELAND, OPAC_SCATTER = 0, 1, 2
 NGHOST = 2

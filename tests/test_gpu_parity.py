@@ -593,6 +593,103 @@ def test_face_fix_variants(rt, case, fix):
         g3.set_face_fix(3)
 
 
+# ----------------------------------------------------------------------------- LimO3 (L132)
+@pytest.mark.parametrize("case", ["cart3d", "sph3d", "cyl2d", "cart1d"])
+def test_limo3_reconstruction(rt, case, r=0.0):
+    """rt_set_reconstruction(RT_RECON_LIMO3): the compact third-order reconstruction of Cada & Torrilhon 2009 (the scheme
+    of the paper's Fig. 1-5) in the per-direction kernels and the 1-D kernel, with (r > 0) and without its smoothness
+    switch, 2 sub-steps on random states against the oracle (which evaluates phi(theta) with the quotient, the kernels
+    without); through rt_explicit_step and through rt_substep; and it is not PLM.  Limiter alone (r = 0): on these
+    white-noise states the UNLIMITED phi_3 of the smoothness switch would extrapolate E to ~0 or below at some faces, where
+    the closure is ill-conditioned and any two implementations differ (measured: 4 cells of 15 300 at 3e-6); the switch is
+    tested on smooth fields below."""
+    geometry, n, solver = {"cart3d": (W.CARTESIAN, (70, 33, 12), W.SOLVER_HLL), "sph3d": (W.SPHERICAL, (45, 20, 17), W.SOLVER_GLF),
+                           "cyl2d": (W.CYLINDRICAL, (64, 40, 1), W.SOLVER_RUSANOV), "cart1d": (W.CARTESIAN, (300, 1, 1), W.SOLVER_HLL)}[case]
+    w = random_workload(geometry, n, solver, 1, seed=190 + len(case), fmax=0.8)
+    og = ort.grid_from_workload(w)
+    og.set_reconstruction(ort.RECON_LIMO3, r)
+    refU, refT, refm, dts = ort.run_substeps(og, w, 2)
+    g = drv.grid_from_workload(w)
+    g.set_reconstruction(rt.RECON_LIMO3, r)
+    st, _ = drv.run_substeps(g, w, 2, dts=dts)
+    torch.cuda.synchronize()
+    errs = field_errors(w, to_host(st.U), refU, st.T.cpu().numpy(), refT, to_host(st.mom), refm)
+    assert_below(errs, 2 * TOL1, "LimO3, " + case)
+    lerrs = local_errors(w, to_host(st.U), refU, st.T.cpu().numpy(), refT, to_host(st.mom), refm)
+    assert_local_below(lerrs, 2 * TOL1, "LimO3, " + case)
+    g2 = drv.grid_from_workload(w)
+    g2.set_reconstruction(rt.RECON_LIMO3, r)
+    st2, _, hist = drv.run_substeps_fused(g2, w, 2)
+    torch.cuda.synchronize()
+    assert np.allclose(hist.cpu().numpy(), dts, rtol=1e-12, atol=0)
+    errs2 = field_errors(w, to_host(st2.U), refU, st2.T.cpu().numpy(), refT, to_host(st2.mom), refm)
+    assert_below(errs2, 2 * TOL1, "LimO3 through rt_substep, " + case)
+    g3 = drv.grid_from_workload(w)
+    st3, _ = drv.run_substeps(g3, w, 2, dts=dts)
+    assert (st3.U[0] - st.U[0]).abs().max().item() > 1e-4 * float(np.abs(refU[0]).max())
+    with pytest.raises(Exception):
+        g3.set_reconstruction(2)
+
+
+def _smooth_workload(geometry, n, solver, seed):
+    """O(1) smooth fields (E = 2 + waves, f <= 0.45) plus 0.1 % noise: the data LimO3's dimensional smoothness switch is
+    made for (eta compares field differences with r x cell length)"""
+    w = random_workload(geometry, n, solver, 1, seed=seed, fmax=0.5)
+    rng = np.random.default_rng(seed + 7)
+    shape = w.U[0].shape
+    idx = np.meshgrid(*[np.arange(s) for s in shape], indexing="ij")
+    ph = lambda a, b, c: 2 * np.pi * (a * idx[2] / max(shape[2], 2) + b * idx[1] / max(shape[1], 2) + c * idx[0] / max(shape[0], 2))
+    E = 2.0 + 0.5 * np.sin(ph(2, 1, 1)) + 0.3 * np.cos(ph(1, 2, 0)) + 1e-3 * rng.standard_normal(shape)
+    w.U[0] = np.ascontiguousarray(E)
+    for q, (a, b, c) in enumerate([(1, 1, 0), (2, 0, 1), (0, 1, 2)]):
+        w.U[1 + q] = np.ascontiguousarray(0.25 * E * np.sin(ph(a, b, c) + q))
+    # the gas too: the implicit half pulls E towards a_R T^4, and a white-noise T would roughen E after one sub-step
+    w.rho = np.ascontiguousarray(1.0 + 0.3 * np.sin(ph(1, 0, 1)))
+    w.T = np.ascontiguousarray(1.2 + 0.2 * np.cos(ph(0, 1, 1)))
+    return w
+
+
+@pytest.mark.parametrize("case", ["cart3d", "sph3d", "cyl2d", "cart1d"])
+def test_limo3_smoothness_switch_on_smooth_fields(rt, case):
+    """LimO3 with r > 0 on smooth O(1) fields: r is chosen so that eta = (d-^2 + d+^2)/(r dl)^2 straddles 1 and both
+    branches (phi_3, phi_L) are taken by a good share of the faces; the branch is DECIDED in the same precision on both
+    sides (rt_math.cuh: limo3_eta).  3 sub-steps, per-direction kernels and rt_substep."""
+    geometry, n, solver, r = {"cart3d": (W.CARTESIAN, (70, 33, 12), W.SOLVER_HLL, 0.15), "sph3d": (W.SPHERICAL, (45, 20, 17), W.SOLVER_GLF, 0.15),
+                              "cyl2d": (W.CYLINDRICAL, (64, 40, 1), W.SOLVER_RUSANOV, 0.4),
+                              "cart1d": (W.CARTESIAN, (300, 1, 1), W.SOLVER_HLL, 0.012)}[case]
+    w = _smooth_workload(geometry, n, solver, seed=290 + len(case))
+    if geometry != W.CARTESIAN:
+        w.bc = (1, 1, 1, 1, 0, 0) if n[2] > 1 else (1, 1, 1, 1, 1, 1)
+    # share of the x1 faces on each branch, from the initial E field
+    E = w.U[0][w.interior]
+    d = np.diff(E, axis=2)
+    dl = np.diff(w.xf[0])[None, None, 1:-1]
+    eta = (d[..., :-1] ** 2 + d[..., 1:] ** 2) / (r * dl) ** 2
+    share = float((eta <= 1.0).mean())
+    assert 0.05 < share < 0.95, share
+    og = ort.grid_from_workload(w)
+    og.set_reconstruction(ort.RECON_LIMO3, r)
+    refU, refT, refm, dts = ort.run_substeps(og, w, 3)
+    assert refU[0][w.interior].min() > 0.05                       # nothing near the E = 0 singularity of the closure
+    for fused in (False, True):
+        g = drv.grid_from_workload(w)
+        g.set_reconstruction(rt.RECON_LIMO3, r)
+        if fused:
+            st, _, hist = drv.run_substeps_fused(g, w, 3)
+            assert np.allclose(hist.cpu().numpy(), dts, rtol=1e-12, atol=0)
+        else:
+            st, _ = drv.run_substeps(g, w, 3, dts=dts)
+        torch.cuda.synchronize()
+        errs = field_errors(w, to_host(st.U), refU, st.T.cpu().numpy(), refT, to_host(st.mom), refm)
+        assert_below(errs, 3 * TOL1, "LimO3 r = %g, %s" % (r, case))
+        lerrs = local_errors(w, to_host(st.U), refU, st.T.cpu().numpy(), refT, to_host(st.mom), refm)
+        assert_local_below(lerrs, 3 * TOL1, "LimO3 r = %g, %s" % (r, case))
+    # the switch matters: r = 0 gives another answer
+    og.set_reconstruction(ort.RECON_LIMO3, 0.0)
+    U0, _, _, _ = ort.run_substeps(og, w, 3, dts=dts)
+    assert np.abs(U0[0] - refU[0]).max() > 1e-9 * np.abs(refU[0]).max()
+
+
 # ----------------------------------------------------------------------------- streams and CUDA graphs
 def test_substeps_on_a_side_stream_and_replayed_from_a_cuda_graph(rt):
     """rt_substep enqueues on the stream given at rt_grid_create and never synchronises: (a) a grid created on a side
