@@ -715,6 +715,11 @@ static int32_t implicit_impl(rt_grid* g, double dt, const double* dt_dev, const 
     a.ichat = 1.0 / g->par.chat;
     a.counters = g->counters;
     a.divfirr = g->divfirr;
+    for (int q = 0; q < 4; ++q) a.avgU[q] = nullptr;
+    a.avgT = nullptr;
+    for (int q = 0; q < 3; ++q) a.avgm[q] = nullptr;
+    a.Tout = a.T;
+    for (int q = 0; q < 3; ++q) a.mout[q] = a.mom[q];
     ParamsDev P = {g->par.chat, g->par.c, g->par.a_R, g->par.c_v, g->par.E_floor, g->par.solver, g->par.thick_limit,
                    g->par.feedback_momentum};
     const int bx = D.n[0] >= 128 ? 128 : ((D.n[0] + 31) / 32) * 32;
@@ -852,7 +857,7 @@ static cudaError_t launch_fused_z(rt_grid* g, const ParamsDev& P, const FusedArg
 // x3 active (3-D) or not (2-D); the comparison face fixes (a.fix != 0; never with the Rusanov solver: fused_eligible)
 template <bool HLL, bool THICK, bool CURVI, bool FEEDBACK, bool RUS = false>
 static cudaError_t launch_fused_t(rt_grid* g, const ParamsDev& P, const FusedArgs& a, const FusedMaps& maps, dim3 grid, int seglen) {
-    if (!RUS && a.fix != 0)
+    if (!RUS && (a.fix != 0 || a.im.avgU[0] != nullptr))
         return g->dev.gh[2] > 0 ? launch_fused_z<HLL, THICK, CURVI, FEEDBACK, false, true, true>(g, P, a, maps, grid, seglen)
                                 : launch_fused_z<HLL, THICK, CURVI, FEEDBACK, false, false, true>(g, P, a, maps, grid, seglen);
     return g->dev.gh[2] > 0 ? launch_fused_z<HLL, THICK, CURVI, FEEDBACK, RUS, true, false>(g, P, a, maps, grid, seglen)
@@ -936,8 +941,18 @@ static bool fused_eligible(const rt_grid* g) {
            D.gh[1] > 0 && D.ntot < (1LL << 31);  // 32-bit element offsets inside the kernel
 }
 
+// RK2: what the second stage averages its result with (fused into its stores), and where the new time step goes
+struct RkAvg {
+    const double* U[4];   // average the result with these (nullptr: no average: first stage)
+    const double* T;
+    const double* m[3];
+    double* Tout;         // updated T, m go here instead of in place (nullptr: in place)
+    double* mout[3];
+    double* dt_out;       // the new time step (nullptr: dt_device)
+};
+
 static int32_t fused_impl(rt_grid* g, double* dt_device, double cfl, const double* rho, double* T, double* const mom[3],
-                          double* const U_in[4], double* const U_out[4]) {
+                          double* const U_in[4], double* const U_out[4], const RkAvg* avg = nullptr) {
     ProfScope::trim(g);
     if (!U_in || !U_out) return fail(g, RT_ERR_INVALID_ARG, "rt_substep: null argument");
     if (!g->have_par) return fail(g, RT_ERR_BAD_STATE, "rt_substep: rt_set_params has not been called");
@@ -983,6 +998,11 @@ static int32_t fused_impl(rt_grid* g, double* dt_device, double cfl, const doubl
     a.im.ichat = 1.0 / g->par.chat;
     a.im.counters = g->counters;
     a.im.divfirr = g->divfirr;
+    for (int q = 0; q < 4; ++q) a.im.avgU[q] = avg ? avg->U[q] : nullptr;
+    a.im.avgT = avg ? avg->T : nullptr;
+    for (int q = 0; q < 3; ++q) a.im.avgm[q] = (avg && feedback) ? avg->m[q] : nullptr;
+    a.im.Tout = (avg && avg->Tout) ? avg->Tout : T;
+    for (int q = 0; q < 3; ++q) a.im.mout[q] = feedback ? ((avg && avg->mout[q]) ? avg->mout[q] : mom[q]) : nullptr;
     ParamsDev P = {g->par.chat, g->par.c, g->par.a_R, g->par.c_v, g->par.E_floor, g->par.solver, g->par.thick_limit,
                    g->par.feedback_momentum};
     const int tx = (D.n[0] + FTX - 1) / FTX, ty = (D.n[1] + FTY - 1) / FTY;
@@ -1024,7 +1044,7 @@ static int32_t fused_impl(rt_grid* g, double* dt_device, double cfl, const doubl
     RT_LAUNCH_CHECK(g);
     {
         ProfScope ps(g, RT_K_CFL);
-        k_cfl_finalize<<<1, 1, 0, g->stream>>>(g->scr, cfl, dt_device);
+        k_cfl_finalize<<<1, 1, 0, g->stream>>>(g->scr, cfl, (avg && avg->dt_out) ? avg->dt_out : dt_device);
     }
     RT_LAUNCH_CHECK(g);
     return RT_OK;
@@ -1087,6 +1107,11 @@ static int32_t oned_impl(rt_grid* g, double* dt_device, double cfl, const double
     a.ichat = 1.0 / g->par.chat;
     a.counters = g->counters;
     a.divfirr = g->divfirr;
+    for (int q = 0; q < 4; ++q) a.avgU[q] = nullptr;
+    a.avgT = nullptr;
+    for (int q = 0; q < 3; ++q) a.avgm[q] = nullptr;
+    a.Tout = a.T;
+    for (int q = 0; q < 3; ++q) a.mout[q] = a.mom[q];
     ParamsDev P = {g->par.chat, g->par.c, g->par.a_R, g->par.c_v, g->par.E_floor, g->par.solver, g->par.thick_limit,
                    g->par.feedback_momentum};
     const bool hll = g->par.solver != RT_SOLVER_GLF, thick = g->par.thick_limit != 0, curvi = D.geometry != RT_CARTESIAN;
@@ -1151,12 +1176,34 @@ extern "C" int32_t rt_rk2_step(rt_grid* g, double* dt_device, double cfl, const 
     for (int q = 0; q < nsave; ++q)
         if (!g->rk_save[q]) RT_CUDA(g, cudaMalloc(&g->rk_save[q], bytes));
     if (!g->rk_dt) RT_CUDA(g, cudaMalloc(&g->rk_dt, 2 * sizeof(double)));
-    // T^n, m^n (the sub-steps update them in place) and two copies of dt (each stage overwrites the one it reads)
+    RT_CUDA(g, cudaMemcpyAsync(g->rk_dt, dt_device, sizeof(double), cudaMemcpyDeviceToDevice, g->stream));
+    RT_CUDA(g, cudaMemcpyAsync(g->rk_dt + 1, dt_device, sizeof(double), cudaMemcpyDeviceToDevice, g->stream));
+    if (fused_eligible(g) && g->par.solver != RT_SOLVER_RUSANOV) {
+        // Both stages in the fused kernel, nothing copied.  Stage 1 reads T^n, m^n and writes T_1, m_1 into the handle's
+        // scratch arrays; stage 2 reads those (in place) and stores the averages (U + U_2)/2 into U, (T^n + T_2)/2 into T,
+        // (m^n + m_2)/2 into m, and reduces the CFL rate of the AVERAGED state: no save copies, no averaging pass, no
+        // separate CFL pass, W2 untouched.
+        RkAvg s1;
+        memset(&s1, 0, sizeof(s1));
+        s1.Tout = g->rk_save[0];
+        for (int q = 0; q < 3; ++q) s1.mout[q] = feedback ? g->rk_save[1 + q] : nullptr;
+        int32_t rc1 = fused_impl(g, g->rk_dt, cfl, rho, T, mom, U, W1, &s1);
+        if (rc1 != RT_OK) return rc1;
+        RkAvg s2;
+        memset(&s2, 0, sizeof(s2));
+        for (int q = 0; q < 4; ++q) s2.U[q] = U[q];
+        s2.T = T;
+        for (int q = 0; q < 3; ++q) s2.m[q] = feedback ? mom[q] : nullptr;
+        s2.Tout = T;
+        for (int q = 0; q < 3; ++q) s2.mout[q] = feedback ? mom[q] : nullptr;
+        s2.dt_out = dt_device;
+        double* m1[3] = {g->rk_save[1], g->rk_save[2], g->rk_save[3]};
+        return fused_impl(g, g->rk_dt + 1, cfl, rho, g->rk_save[0], feedback ? m1 : nullptr, W1, U, &s2);
+    }
+    // T^n, m^n (the sub-steps update them in place)
     RT_CUDA(g, cudaMemcpyAsync(g->rk_save[0], T, bytes, cudaMemcpyDeviceToDevice, g->stream));
     for (int q = 0; q < 3 && feedback; ++q)
         RT_CUDA(g, cudaMemcpyAsync(g->rk_save[1 + q], mom[q], bytes, cudaMemcpyDeviceToDevice, g->stream));
-    RT_CUDA(g, cudaMemcpyAsync(g->rk_dt, dt_device, sizeof(double), cudaMemcpyDeviceToDevice, g->stream));
-    RT_CUDA(g, cudaMemcpyAsync(g->rk_dt + 1, dt_device, sizeof(double), cudaMemcpyDeviceToDevice, g->stream));
     int32_t rc = substep_impl(g, g->rk_dt, cfl, rho, T, mom, U, W1);
     if (rc != RT_OK) return rc;
     rc = substep_impl(g, g->rk_dt + 1, cfl, rho, T, mom, W1, W2);

@@ -155,8 +155,9 @@ __device__ __forceinline__ void state_load(const double* buf, int t, State& s) {
 // RUS (with HLL = true): RT_SOLVER_RUSANOV, compile-time so that the HLL faces do not pay for the test
 // HASZ = false: 2-D grids (n3 = 1, x3 inactive): one staged plane, no x3 phase; the march degenerates to the steps
 // c = 0 (X, Y) and 1 (FIN, which reads nothing but the thick-limit value of plane 0).
-// VARFIX = true: the comparison face fixes of rt_set_face_fix (flat fallback L136 / clip Eq. 36-38) selected by the
-// launch-uniform a.fix; false: the paper's f-preserving scheme, compiled in (the default path carries no test for it)
+// VARFIX = true: the instantiations with run-time options: the comparison face fixes of rt_set_face_fix (flat fallback
+// L136 / clip Eq. 36-38) selected by the launch-uniform a.fix, and the RK2 average of the second stage (a.im.avgU ...);
+// false: the paper's f-preserving scheme, compiled in, plain stores (the default path carries no test for either)
 template <bool HLL, bool THICK, bool CURVI, bool FEEDBACK, bool RUS, bool HASZ, bool VARFIX = false>
 __global__ void __launch_bounds__(FNT, FUSED_MINB)
     k_substep_fused(const __grid_constant__ GridDev g, const __grid_constant__ ParamsDev par, const __grid_constant__ OpacDev oP,
@@ -375,8 +376,8 @@ __global__ void __launch_bounds__(FNT, FUSED_MINB)
                         const double ilmin = HASZ ? dmin(il[0], dmin(il[1], il[2])) : dmin(il[0], il[1]);  // active directions
                         rhochi = lim > 1.0e300 ? 0.0 : (4.0 / 3.0) * ilmin * frcp(lim);
                     }
-                    const double r = implicit_cell<FEEDBACK, true, THICK>(g, par, oP, oR, oS, a.im, dt, (long long)id, il, U4[0], F, rho,
-                                                                          T0, m, floored, clipped, rhochi, kpr_f);
+                    const double r = implicit_cell<FEEDBACK, true, THICK, VARFIX>(g, par, oP, oR, oS, a.im, dt, (long long)id, il, U4[0],
+                                                                                  F, rho, T0, m, floored, clipped, rhochi, kpr_f);
                     rate = dmax(rate, r);
                     nfloor += floored ? 1 : 0;
                     nclip += clipped ? 1 : 0;

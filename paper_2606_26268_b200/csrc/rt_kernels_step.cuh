@@ -248,6 +248,16 @@ struct ImplicitArgs {
     double ichat; // 1 / chat
     unsigned long long* counters;  // [0] floor activations, [1] clip activations
     const double* divfirr;         // div F_irr per cell (Sect. 2.9, Eq. 34-35) or nullptr
+    // RK2 (L107, L256): the second stage stores the average of its result with the state the step started from (AVG
+    // instantiations only; nullptr: off).  avgU may be the output arrays themselves (each cell is read, then written, by
+    // its own thread); the CFL rate is then that of the averaged state
+    const double* avgU[4];
+    const double* avgT;
+    const double* avgm[3];
+    // where the updated T and m go: the arrays they were read from (in place), or, for the first RK2 stage, scratch
+    // arrays, so that T^n and m^n survive for the average without being copied first
+    double* Tout;
+    double* mout[3];
 };
 
 // CFL = true additionally evaluates the step-10 rate (R-G15) of the UPDATED state of each cell and folds it
@@ -259,7 +269,7 @@ struct ImplicitArgs {
 // CHIGIVEN: rho chi and rho kappa_P of the cell are passed in (the fused kernel recovers the first from the
 // thick-limit array of the SAME sub-step, lim = 4/(3 rho chi dx), and gets the second from the same pre-pass): no
 // opacity is evaluated here.
-template <bool FEEDBACK, bool CFL, bool CHIGIVEN = false>
+template <bool FEEDBACK, bool CFL, bool CHIGIVEN = false, bool AVG = false>
 __device__ __forceinline__ double implicit_cell(const GridDev& g, const ParamsDev& par, const OpacDev& oP, const OpacDev& oR,
                                                 const OpacDev& oS, const ImplicitArgs& a, double dt, long long id,
                                                 const double il[3] /* 1/dl_d of the cell (CFL only) */, double E, double F[3],
@@ -311,16 +321,26 @@ __device__ __forceinline__ double implicit_cell(const GridDev& g, const ParamsDe
         Tn_ = fma(1.0 + gr, qd, Tn_);
         asm volatile("");
     }
-    const double En = En_, Tn = Tn_;
+    double En = En_, Tn = Tn_;
     const double idamp = frcp(fma(dt * par.chat, rhochi, 1.0));
+    const bool avg = AVG && a.avgU[0] != nullptr;  // launch-uniform
+    if (avg) {
+        En = 0.5 * (En + a.avgU[0][id]);
+        Tn = 0.5 * (Tn + a.avgT[id]);
+    }
     a.U[0][id] = En;
-    a.T[id] = Tn;
+    a.Tout[id] = Tn;
     const double ichat = a.ichat;
     double Fn[3];
 #pragma unroll
     for (int q = 0; q < 3; ++q) {
         Fn[q] = F[q] * idamp;
-        if (FEEDBACK) a.mom[q][id] = fma(-(Fn[q] - F[q]), ichat, m[q]);
+        if (FEEDBACK) {
+            double mn = fma(-(Fn[q] - F[q]), ichat, m[q]);
+            if (avg) mn = 0.5 * (mn + a.avgm[q][id]);
+            a.mout[q][id] = mn;
+        }
+        if (avg) Fn[q] = 0.5 * (Fn[q] + a.avgU[1 + q][id]);
         a.U[1 + q][id] = Fn[q];
     }
     return CFL ? cell_rate_il(par.chat, En, Fn[0], Fn[1], Fn[2], il) : 0.0;
