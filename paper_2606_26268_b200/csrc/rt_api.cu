@@ -614,10 +614,27 @@ static int32_t launch_thick_limit(rt_grid* g, const double* rho, const double* T
                 L.same_ab = (oP.n2a == oR.n2a && oP.n2b == oR.n2b) ? 1 : 0;
             }
         }
+        // two 2-D tables on the same axes and units (or one), no scattering: the table-pair path
+        TablePair tp;
+        memset(&tp, 0, sizeof(tp));
+        bool pair = !lean && oR.set && oR.kind == 1 && oR.n_lrho > 1 && !oS.set;
+        if (pair && second)
+            pair = oP.set && oP.kind == 1 && oP.n_lrho == oR.n_lrho && oP.n_lT == oR.n_lT && oP.lrho_min == oR.lrho_min &&
+                   oP.lrho_max == oR.lrho_max && oP.lT_min == oR.lT_min && oP.lT_max == oR.lT_max && oP.rho_unit == oR.rho_unit &&
+                   oP.T_unit == oR.T_unit;
+        if (pair) {
+            tp.tabR = oR.tab;
+            tp.tabP = second ? oP.tab : nullptr;
+            tp.n_lrho = oR.n_lrho; tp.n_lT = oR.n_lT;
+            tp.lrho_min = oR.lrho_min; tp.lrho_max = oR.lrho_max; tp.lT_min = oR.lT_min; tp.lT_max = oR.lT_max;
+            tp.su = oR.su; tp.sv = oR.sv; tp.rho_unit = oR.rho_unit; tp.T_unit = oR.T_unit;
+        }
         if (lean)
-            k_thick_limit<true><<<grid, bx, 0, g->stream>>>(D, oR, oS, os, rho, T, g->lim, oP, g->same_PR, kpr, L);
+            k_thick_limit<1><<<grid, bx, 0, g->stream>>>(D, oR, oS, os, rho, T, g->lim, oP, g->same_PR, kpr, L, tp);
+        else if (pair)
+            k_thick_limit<2><<<grid, bx, 0, g->stream>>>(D, oR, oS, os, rho, T, g->lim, oP, g->same_PR, kpr, L, tp);
         else
-            k_thick_limit<false><<<grid, bx, 0, g->stream>>>(D, oR, oS, os, rho, T, g->lim, oP, g->same_PR, kpr, L);
+            k_thick_limit<0><<<grid, bx, 0, g->stream>>>(D, oR, oS, os, rho, T, g->lim, oP, g->same_PR, kpr, L, tp);
     }
     RT_LAUNCH_CHECK(g);
     return RT_OK;

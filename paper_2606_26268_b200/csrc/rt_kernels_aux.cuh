@@ -472,16 +472,47 @@ __device__ __forceinline__ void lean_eval(const LeanLaws& L, double rho, double 
 // the same rho0, T0.  Otherwise the general evaluation (tables share their log10 inputs: OpacSet).
 // One thread per x1 column of a block of kThickRows x2 rows; the loads of the next row are issued before the
 // arithmetic of the current one.
-template <bool LEAN>
+// MODE 2: kappa_R (and kappa_P, when asked for and not the same law) are 2-D tables on the SAME axes and units, no
+// scattering: the two log10, the cell of the table and the interpolation weights are found once, then one 2 x 2 gather
+// and one 10^x per table (C5).  Same arithmetic as table_eval, without the per-opacity tests of the general path.
+struct TablePair {
+    const double* tabR;
+    const double* tabP;  // nullptr: kappa_P is not wanted or is the same table
+    int n_lrho, n_lT;
+    double lrho_min, lrho_max, lT_min, lT_max, su, sv, rho_unit, T_unit;
+};
+__device__ __forceinline__ void table_pair_eval(const TablePair& tp, double rho, double T, double& kR, double& kP) {
+    const double x = dmin(dmax(flog10(rho * tp.rho_unit), tp.lrho_min), tp.lrho_max);
+    const double y = dmin(dmax(flog10(T * tp.T_unit), tp.lT_min), tp.lT_max);
+    const double u = (x - tp.lrho_min) * tp.su, v = (y - tp.lT_min) * tp.sv;
+    const int i0 = max(0, min((int)u, tp.n_lrho - 2)), j0 = max(0, min((int)v, tp.n_lT - 2));
+    const double tu = u - (double)i0, tv = v - (double)j0;
+    const int off = j0 * tp.n_lrho + i0;
+    {
+        const double* p = tp.tabR + off;
+        const double v00 = __ldg(p), v01 = __ldg(p + 1), v10 = __ldg(p + tp.n_lrho), v11 = __ldg(p + tp.n_lrho + 1);
+        kR = fexp10((1.0 - tv) * ((1.0 - tu) * v00 + tu * v01) + tv * ((1.0 - tu) * v10 + tu * v11));
+    }
+    kP = kR;
+    if (tp.tabP) {
+        const double* p = tp.tabP + off;
+        const double v00 = __ldg(p), v01 = __ldg(p + 1), v10 = __ldg(p + tp.n_lrho), v11 = __ldg(p + tp.n_lrho + 1);
+        kP = fexp10((1.0 - tv) * ((1.0 - tu) * v00 + tu * v01) + tv * ((1.0 - tu) * v10 + tu * v11));
+    }
+}
+
+template <int MODE>
 __global__ void __launch_bounds__(256) k_thick_limit(const __grid_constant__ GridDev g, const __grid_constant__ OpacDev oR,
                                                      const __grid_constant__ OpacDev oS, const __grid_constant__ OpacSet os,
                                                      const double* __restrict__ rho, const double* __restrict__ T,
                                                      double* __restrict__ lim, const __grid_constant__ OpacDev oP,
-                                                     int same_PR, double* __restrict__ kpr, const __grid_constant__ LeanLaws laws) {
+                                                     int same_PR, double* __restrict__ kpr, const __grid_constant__ LeanLaws laws,
+                                                     const __grid_constant__ TablePair tp) {
+    constexpr bool LEAN = MODE == 1;
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     const int k = blockIdx.z;
     if (i >= g.n[0]) return;
-    const bool share = os.share != 0;
+    const bool share = MODE == 0 && os.share != 0;
     const int s1 = (int)g.stride[1], s2 = (int)g.stride[2];
     const int n0 = g.n[0], n1 = g.n[1], n2 = g.n[2];
     const bool act1 = g.gh[1] > 0, act2 = g.gh[2] > 0;
@@ -519,6 +550,8 @@ __global__ void __launch_bounds__(256) k_thick_limit(const __grid_constant__ Gri
         double chi, kP;
         if (LEAN) {
             lean_eval(laws, rc, tc, chi, kP);
+        } else if (MODE == 2) {
+            table_pair_eval(tp, rc, tc, chi, kP);
         } else {
             LogRT l = {0.0, 0.0};
             if (share) l = log_inputs(os.src == RT_OPAC_SCATTER_IDX ? oS : (os.src == 1 ? oR : oP), rc, tc);
