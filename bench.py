@@ -390,6 +390,20 @@ def run_native(args):
                                "gpu_launches": m2["launches"], "roofline": r2}}
         del m2, w2
         torch.cuda.empty_cache()
+        # the two launch-latency-bound configs ("report cell-updates/s and us per sub-step only"), replayed from
+        # a CUDA graph of two sub-steps, 200 sub-steps per region
+        import copy
+        lat = {}
+        for name in ("C1a", "C2"):
+            a2 = copy.copy(args)
+            a2.graph = True
+            w3 = make_workload(name)
+            m3 = measure_workload(a2, rt, drv, w3, dev, world, 200, 4, 3, barrier)
+            lat[name] = {"us_per_substep": round(m3["ms_per_step"] * 1e3, 2), "value": m3["value"], "unit": UNIT,
+                         "cells": w3.ncells, "cuda_graph": True, "launches_per_substep": m3["launches"] / m3["K"]}
+            del m3, w3
+        out["also"]["latency_bound"] = lat
+        torch.cuda.empty_cache()
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         out["cpu_baseline"] = cpu_baseline(w)
     if world > 1:
