@@ -33,6 +33,7 @@ FUSED_KERNEL = True   # rt_substep runs k_substep_fused (2-D / 3-D grids, --fuse
 
 # fp64-pipe roof by formula, kept beside the MEASURED one (rt_measure_fp64, same process): 148 SMs x 64 lanes/clk x 1.965 GHz
 FP64_FORMULA_TINST = 148 * 64 * 1.965e9 / 1e12
+N_SM = 148
 REGIONS = 5           # timed regions of K steps each; the line reports the median (SURVEY 8(d) "Timing")
 
 
@@ -201,13 +202,23 @@ def load_fp64_counts(workload):
 
 
 def measure_fp64_peak(rt, dev):
-    """DFMA microbenchmark in this process (rt_measure_fp64): 8 independent chains per thread, 8 warps per SM
-    sub-partition, ~10 ms.  Thread instructions per second."""
-    best = 0.0
-    for _ in range(3):
-        ms, n = rt.measure_fp64(148 * 4, 256, 8, 20000, device=dev)
-        best = max(best, n / (ms * 1e-3))
-    return best / 1e12
+    """DFMA microbenchmark in this process (rt_measure_fp64), 8 warps per SM sub-partition, ~10 ms per launch, best of 3,
+    in 1e12 DFMA thread instructions per second:
+      chains8      8 chains x = fma(x, a, b), a and b shared by the chains (the operand reuse cache serves them)
+      two_reg      4 chains x = fma(x, y_c, const): two register operands, like DMUL / DADD  -> the pipe's own rate
+      three_reg    4 chains x = fma(x, y_c, z_c): three different register pairs -> the register file's rate (3 cycles)
+      *_plus_fmul  the same with 4 independent fp32 multiplies per 4 DFMAs: what an instruction of another pipe costs
+                   while the fp64 pipe is busy (DESIGN.md Sect. 5)
+    The roof bench.py divides by is the best of the first two."""
+    out = {}
+    for key, code in (("chains8", 8), ("two_reg", 204), ("three_reg", 304), ("two_reg_plus_fmul", 214), ("three_reg_plus_fmul", 314)):
+        best = 0.0
+        for _ in range(3):
+            ms, n = rt.measure_fp64(148 * 4, 256, code, 20000 if code == 8 else 40000, device=dev)
+            best = max(best, n / (ms * 1e-3))
+        out[key] = best / 1e12
+    out["peak"] = max(out["chains8"], out["two_reg"])
+    return out
 
 
 def measure_workload(args, rt, drv, w, dev, world, K, Wm, regions, barrier):
@@ -319,8 +330,12 @@ def roofline_block(w, m, K, world, peaks, fp64_peak):
                         "alg_frac": round(sub_GBps / peaks["hbm_gbs"], 4)}}
     # fp64 pipe: the roof that binds the fused kernel (DESIGN.md Sect. 5).  Peak MEASURED in this process; executed
     # instructions per cell from the committed ncu capture of the same sources (refused when stale)
+    probes = fp64_peak
+    fp64_peak = probes["peak"]
     alu = {"peak_measured_Tinst": round(fp64_peak, 3), "peak_formula_Tinst": round(FP64_FORMULA_TINST, 3),
-           "peak_source": "rt_measure_fp64 in this run: DFMA chains, 8 per thread, 8 warps per SM sub-partition"}
+           "peak_source": "rt_measure_fp64 in this run: the better of DFMA chains with shared operands (8 per thread) and"
+                          " with two register operands (4 per thread), 8 warps per SM sub-partition",
+           "probes_Tinst": {k: round(v, 3) for k, v in probes.items() if k != "peak"}}
     cnt = load_fp64_counts(w.name) if dom == "fused" else None
     if cnt and not cnt.get("stale"):
         inst = cnt["fp64_thread_inst_per_cell"]
@@ -328,6 +343,17 @@ def roofline_block(w, m, K, world, peaks, fp64_peak):
         alu.update({"executed_fp64_thread_inst_per_cell": inst, "achieved_Tinst": round(ach, 3),
                     "frac_of_measured": round(ach / fp64_peak, 4), "ncu_pipe_fp64_active_pct": cnt.get("pipe_fp64_active_pct"),
                     "counts_source": "profiles/fp64_counts.txt (bench_ncu_counts.py; same csrc hash as the tree)"})
+        # the issue slot: every executed warp instruction holds it for max(pipe, even source registers, odd source
+        # registers) cycles (2 for the fp64 pipe, 3 for a DFMA with three register operands, 1 otherwise), one after the
+        # other; the sum over the kernel's instruction stream is its own lower bound on this device
+        ic = cnt.get("issue_cycles_per_warp_of_cells")
+        sm_mhz = (m.get("clocks") or {}).get("sm_mhz")
+        if ic and sm_mhz:
+            bound_ms = ic * (w.ncells / 32.0) / (N_SM * 4) / (sm_mhz * 1e6) * 1e3
+            alu["issue"] = {"cycles_per_warp_of_cells": ic, "bound_ms": round(bound_ms, 4), "frac": round(bound_ms / avg_ms, 4),
+                            "sm_mhz": sm_mhz,
+                            "note": "issue cycles of the executed instruction stream (ncu capture) / (148 SMs x 4 schedulers x"
+                                    " the SM clock sampled during the timed region) over the measured launch time"}
     elif cnt:
         alu.update(cnt)
     roof["alu"] = alu

@@ -12,6 +12,12 @@ per workload and averaged over the captured launches of k_substep_fused (C4 alte
   pipe_fp64_active_pct        sm__inst_executed_pipe_fp64.avg.pct_of_peak_sustained_active
   dram_bytes_per_launch       dram__bytes_read.sum + dram__bytes_write.sum
   warp_inst_per_launch, time_ms_under_ncu, issue_active_pct
+  issue_cycles_per_warp_of_cells   sum over the executed warp instructions of the cycles each holds the issue slot of its
+                              SM sub-partition, per 32 cells: max(pipe, distinct even source registers, distinct odd
+                              source registers) with pipe = 2 for the fp64 instructions and 1 for the rest (the register
+                              file delivers one even and one odd register per cycle; a 64-bit operand is one of each).
+                              rt_measure_fp64's 204/304/214/314 modes measure exactly these charges (DESIGN.md Sect. 5).
+                              The operand reuse cache and the MUFU / shared-memory rates are left out.
 
 together with the sha256 of the CUDA sources in the tree: bench.py refuses the numbers when the sources have changed
 since (a kernel edit must be followed by a new capture)."""
@@ -19,6 +25,7 @@ import argparse
 import csv
 import json
 import os
+import re
 import sys
 
 ROOT = os.path.dirname(os.path.abspath(__file__))
@@ -27,15 +34,42 @@ FP64_OPS = ("DFMA", "DMUL", "DADD", "DSETP")
 UNIT = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9, "Tbyte": 1e12, "ns": 1e-6, "us": 1e-3, "ms": 1.0, "s": 1e3}
 
 
+def issue_cycles(sass):
+    """cycles one warp instruction holds the issue slot (see the module docstring)"""
+    t = sass.strip().split(None, 1)
+    if t and t[0].startswith("@"):
+        t = t[1].split(None, 1) if len(t) > 1 else []
+    if not t:
+        return 1
+    opc = t[0].split(".")[0]
+    parts = [p.strip() for p in (t[1] if len(t) > 1 else "").rstrip(" ;").split(",")]
+    if opc == "DSETP":
+        srcs = parts[2:]
+    elif opc in ("STS", "STG", "ST", "STL", "RED", "ATOMS", "ATOMG", "BRA", "BAR", "SYNCS", "UTMALDG", "CCTL"):
+        srcs = parts
+    else:
+        srcs = parts[1:]
+    wide = opc in FP64_OPS
+    even, odd = set(), set()
+    for p in srcs:
+        for r in re.findall(r"(?<![A-Za-z])R(\d+)", p):
+            n = int(r)
+            (even if n % 2 == 0 else odd).add(n)
+            if wide:
+                (odd if n % 2 == 0 else even).add(n + 1)
+    return max(2 if wide else 1, len(even), len(odd))
+
+
 def parse_source(path, kernel="k_substep_fused"):
-    """[(kernel name, fp64 thread instructions, warp instructions)] per captured launch (duplicate sections dropped)"""
+    """[(kernel name, fp64 thread instructions, warp instructions, issue cycles)] per captured launch (duplicate
+    sections dropped)"""
     out, seen = [], set()
-    name, hdr, fp64, warp = None, None, 0, 0
+    name, hdr, fp64, warp, cyc = None, None, 0, 0, 0
 
     def flush():
         if name and kernel in name and (name, fp64, warp) not in seen:
             seen.add((name, fp64, warp))
-            out.append((name, fp64, warp))
+            out.append((name, fp64, warp, cyc))
 
     with open(path, newline="") as fh:
         for r in csv.reader(fh):
@@ -43,7 +77,7 @@ def parse_source(path, kernel="k_substep_fused"):
                 continue
             if r[0] == "Kernel Name":
                 flush()
-                name, hdr, fp64, warp = r[1], None, 0, 0
+                name, hdr, fp64, warp, cyc = r[1], None, 0, 0, 0
                 continue
             if r[0] == "Address":
                 hdr = {h: i for i, h in enumerate(r)}
@@ -55,6 +89,7 @@ def parse_source(path, kernel="k_substep_fused"):
                 op = op[1:]
             opc = op[0].split(".")[0] if op else ""
             warp += int(r[hdr["Instructions Executed"]])
+            cyc += int(r[hdr["Instructions Executed"]]) * issue_cycles(r[hdr["Source"]])
             if opc in FP64_OPS:
                 fp64 += int(r[hdr["Predicated-On Thread Instructions Executed"]])
     flush()
@@ -101,6 +136,8 @@ def main():
              "fp64_thread_inst_per_cell": round(mean([s[1] for s in src]) / w.ncells, 1),
              "fp64_thread_inst_per_cell_each": [round(s[1] / w.ncells, 1) for s in src],
              "warp_inst_per_launch": mean([s[2] for s in src]),
+             "issue_cycles_per_warp_of_cells": round(mean([s[3] for s in src]) / (w.ncells / 32.0), 1),
+             "issue_cycles_per_warp_of_cells_each": [round(s[3] / (w.ncells / 32.0), 1) for s in src],
              "pipe_fp64_active_pct": round(mean([r["pipe_fp64"] for r in raw]), 2),
              "issue_active_pct": round(mean([r["issue"] for r in raw]), 2),
              "dram_bytes_per_launch": mean([r["dram_bytes"] for r in raw]),

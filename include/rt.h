@@ -209,6 +209,11 @@ int32_t rt_set_tuning(rt_grid* g, int32_t march_len, int32_t fused_seg);
  * handle.  Launches `blocks` x `threads` threads, each running `chains` (1, 2, 4 or 8) independent chains of
  * 8 * iters dependent DFMAs, twice (the first launch warms up), and writes the CUDA-event duration of the second launch
  * in milliseconds to *ms_host (HOST).  Thread instructions of that launch = blocks * threads * chains * 8 * iters.
+ * chains = 101, 102, 104: 1, 2, 4 chains with 64 instead of 8 DFMAs per chain between loop branches (x 64 * iters).
+ * chains = 204 / 304: four chains whose DFMA reads two / three DIFFERENT register pairs (x = fma(x, y_c, const) /
+ * fma(x, y_c, z_c)); 214 / 314: the same plus four independent fp32 multiplies per four DFMAs.  DFMA count of these
+ * four = blocks * threads * 4 * 8 * iters.  They measure what the issue slot charges per instruction (DESIGN.md
+ * Sect. 5: 2 cycles per fp64 warp instruction, 3 with three register operands, 1 per other instruction, not overlapped).
  * Synchronises the stream.  Bad argument -> RT_ERR_INVALID_ARG; no device / launch failure -> RT_ERR_CUDA. */
 int32_t rt_measure_fp64(void* cuda_stream, int32_t blocks, int32_t threads, int32_t chains, int32_t iters, double* ms_host);
 

@@ -1328,7 +1328,9 @@ extern "C" int32_t rt_get_floor_counts(rt_grid* g, int64_t* n_floor, int64_t* n_
 extern "C" int32_t rt_measure_fp64(void* cuda_stream, int32_t blocks, int32_t threads, int32_t chains, int32_t iters,
                                    double* ms_host) {
     if (!ms_host || blocks < 1 || threads < 32 || threads > 1024 || (threads & 31) || iters < 1) return RT_ERR_INVALID_ARG;
-    if (chains != 1 && chains != 2 && chains != 4 && chains != 8 && chains != 101 && chains != 102 && chains != 104) return RT_ERR_INVALID_ARG;
+    if (chains != 1 && chains != 2 && chains != 4 && chains != 8 && chains != 101 && chains != 102 && chains != 104 &&
+        chains != 204 && chains != 304 && chains != 214 && chains != 314)
+        return RT_ERR_INVALID_ARG;
     cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
     double* sink = nullptr;
     cudaEvent_t e0 = nullptr, e1 = nullptr;
@@ -1345,6 +1347,10 @@ extern "C" int32_t rt_measure_fp64(void* cuda_stream, int32_t blocks, int32_t th
                 case 101: k_dfma_chains<1, 64><<<blocks, threads, 0, st>>>(sink, iters, a, b); break;
                 case 102: k_dfma_chains<2, 64><<<blocks, threads, 0, st>>>(sink, iters, a, b); break;
                 case 104: k_dfma_chains<4, 64><<<blocks, threads, 0, st>>>(sink, iters, a, b); break;
+                case 204: k_dfma_operands<2, 0><<<blocks, threads, 0, st>>>(sink, iters, a, b, 1.0f, 0.0f); break;
+                case 304: k_dfma_operands<3, 0><<<blocks, threads, 0, st>>>(sink, iters, a, b, 1.0f, 0.0f); break;
+                case 214: k_dfma_operands<2, 4><<<blocks, threads, 0, st>>>(sink, iters, a, b, 1.0f, 0.0f); break;
+                case 314: k_dfma_operands<3, 4><<<blocks, threads, 0, st>>>(sink, iters, a, b, 1.0f, 0.0f); break;
                 default: k_dfma_chains<8><<<blocks, threads, 0, st>>>(sink, iters, a, b); break;
             }
             cudaEventRecord(e1, st);

@@ -160,7 +160,9 @@ def opacity_from_spec(spec):
 
 
 def measure_fp64(blocks, threads, chains, iters, device="cuda:0"):
-    """rt_measure_fp64: milliseconds of one launch of the DFMA-chain microbenchmark and its thread-instruction count"""
+    """rt_measure_fp64: milliseconds of one launch of the DFMA microbenchmark and its DFMA thread-instruction count
+    (chains: 1, 2, 4, 8 chains of 8 * iters; 101, 102, 104: 1, 2, 4 chains of 64 * iters; 204, 304, 214, 314: 4 chains of
+    8 * iters with two / three register operands, without / with four fp32 multiplies per four DFMAs; include/rt.h)"""
     if not torch.cuda.is_available():
         raise RuntimeError("no CUDA device: paper_2606_26268_b200 has no CPU path")
     ms = C.c_double()
@@ -169,7 +171,8 @@ def measure_fp64(blocks, threads, chains, iters, device="cuda:0"):
         rc = lib().rt_measure_fp64(C.c_void_p(st.cuda_stream), int(blocks), int(threads), int(chains), int(iters), C.byref(ms))
     if rc != OK:
         raise RtError("rt_measure_fp64", rc)
-    return ms.value, float(blocks) * threads * chains * 8 * iters
+    nch, per = (chains, 8) if chains < 100 else (chains - 100, 64) if chains < 200 else (4, 8)
+    return ms.value, float(blocks) * threads * nch * per * iters
 
 
 class Grid:

@@ -1106,3 +1106,26 @@ def test_argument_errors_are_reported_not_computed(rt):
     with pytest.raises(RuntimeError):
         g.explicit_step(0.1, None, None, [t.cpu() for t in U], V)                      # host tensors: no CPU path
     assert all(torch.all(v == 0.0) for v in V), "a rejected call must not enqueue work"
+
+
+def test_fp64_probe_modes_and_what_they_charge(rt):
+    """rt_measure_fp64 (include/rt.h): bad arguments are refused; the operand-count modes order as DESIGN.md Sect. 5
+    states: a DFMA with three register operands runs at about 2/3 of the rate of one with two, and four fp32
+    multiplies per four DFMAs cost time of their own (they do not hide behind the fp64 pipe)."""
+    for bad in (3, 16, 205, 0):
+        with pytest.raises(rt.RtError) as ei:
+            rt.measure_fp64(148, 256, bad, 100)
+        assert ei.value.status == rt.ERR_INVALID_ARG
+    with pytest.raises(rt.RtError):
+        rt.measure_fp64(148, 100, 8, 100)          # threads not a multiple of 32
+
+    def rate(code):
+        best = 0.0
+        for _ in range(3):
+            ms, n = rt.measure_fp64(148 * 4, 256, code, 4000)
+            best = max(best, n / ms)
+        return best
+    two, three, two_f, three_f = rate(204), rate(304), rate(214), rate(314)
+    assert 0.60 < three / two < 0.75, (two, three)
+    assert two_f < 0.85 * two and three_f < 0.9 * three, (two, two_f, three, three_f)
+    assert rate(8) > 0.85 * two
