@@ -503,7 +503,7 @@ static int32_t launch_fill_faces(rt_grid* g, double* const U[4], cudaStream_t st
     long long tot = 0;
     for (int d = 0; d < 3; ++d) {
         if (D.gh[d] == 0 || (D.bc[2 * d] == RT_BC_FIXED && D.bc[2 * d + 1] == RT_BC_FIXED)) continue;
-        long long c = 4;
+        long long c = 2;  // work items: (transverse cell, side), both layers each
         for (int e = 0; e < 3; ++e)
             if (e != d) c *= D.n[e];
         tot += c;

@@ -157,11 +157,13 @@ static __global__ void k_fill_ghosts(GridDev g, Fields4 U, int d) {
 // interior range only).  The scheme never reads edge / corner ghosts — each direction's stencil leaves the
 // interior along its own axis only — so rt_substep does not need the axis-by-axis ordering of k_fill_ghosts.
 static __global__ void k_fill_faces(GridDev g, Fields4 U) {
+    // one work item = both ghost layers of one (transverse cell, side) of one axis; along x1 the two layers are one
+    // 16-byte store (they share a 32-byte sector: item-per-layer traffic was twice the sectors)
     long long cnt[3], tot = 0;
     for (int d = 0; d < 3; ++d) {
         const int ea = (d == 0) ? 1 : 0, eb = (d == 2) ? 1 : 2;
         const bool skip = g.gh[d] == 0 || (g.bc[2 * d] == 3 && g.bc[2 * d + 1] == 3);
-        cnt[d] = skip ? 0 : 4LL * g.n[ea] * g.n[eb];
+        cnt[d] = skip ? 0 : 2LL * g.n[ea] * g.n[eb];
         tot += cnt[d];
     }
     for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < tot; t += (long long)gridDim.x * blockDim.x) {
@@ -175,27 +177,48 @@ static __global__ void k_fill_faces(GridDev g, Fields4 U) {
         const long long na = g.n[ea], nb = g.n[eb];
         const int a = (int)(r % na);
         const int b = (int)((r / na) % nb);
-        const int ls = (int)(r / (na * nb));  // 0..3
-        const int gl = ls & 1, side = ls >> 1;
+        const int side = (int)(r / (na * nb));  // 0..1
         const int kind = g.bc[2 * d + side];
         if (kind == 3) continue;
         const int nd = g.n[d];
-        const int dst = side == 0 ? -1 - gl : nd + gl;
-        int src;
-        if (kind == 0) src = side == 0 ? nd - 1 - gl : gl;
-        else if (kind == 1) src = side == 0 ? 0 : nd - 1;
-        else src = side == 0 ? gl : nd - 1 - gl;
+        // the two ghost cells in address order: index dlo and dlo + 1 along d, filled from slo and shi
+        const int dlo = side == 0 ? -2 : nd;
+        int slo, shi;
+        if (kind == 0) {
+            slo = side == 0 ? nd - 2 : 0;
+            shi = slo + 1;
+        } else if (kind == 1) {
+            slo = shi = side == 0 ? 0 : nd - 1;
+        } else {
+            slo = side == 0 ? 1 : nd - 1;
+            shi = side == 0 ? 0 : nd - 2;
+        }
         int c[3];
         c[ea] = a;
         c[eb] = b;
         c[d] = 0;
         const long long base = (c[0] + g.gh[0]) * g.stride[0] + (c[1] + g.gh[1]) * g.stride[1] + (c[2] + g.gh[2]) * g.stride[2];
-        const long long id = base + dst * g.stride[d], is = base + src * g.stride[d];
+        const long long id = base + dlo * g.stride[d];
+        const long long is0 = base + slo * g.stride[d], is1 = base + shi * g.stride[d];
+        double v0[4], v1[4];
 #pragma unroll
         for (int q = 0; q < 4; ++q) {
-            double v = U.q[q][is];
-            if (kind == 2 && q == 1 + d) v = -v;
-            U.q[q][id] = v;
+            v0[q] = U.q[q][is0];
+            v1[q] = U.q[q][is1];
+            if (kind == 2 && q == 1 + d) {
+                v0[q] = -v0[q];
+                v1[q] = -v1[q];
+            }
+        }
+        const bool pair = d == 0 && (id & 1) == 0;  // the fields are 16-byte aligned (include/rt.h)
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            if (pair) {
+                *reinterpret_cast<double2*>(U.q[q] + id) = make_double2(v0[q], v1[q]);
+            } else {
+                U.q[q][id] = v0[q];
+                U.q[q][id + g.stride[d]] = v1[q];
+            }
         }
     }
 }
