@@ -3,8 +3,8 @@
     python -m paper_2606_26268_b200.build [--force] [--verbose]
 
 nvcc cross-compiles without a GPU.  The library links the static CUDA runtime, so it depends only on
-the driver at run time.  The fused sub-step kernel has 80 instantiations (solver x thick limit x geometry x
-feedback x 2-D/3-D x face fix); they are compiled as RT_FUSED_PARTS translation units side by side with the
+the driver at run time.  The fused sub-step kernel has 112 instantiations (solver x thick limit x geometry x
+feedback x 2-D/3-D x {plain, RK2 average, run-time face fix}); they are compiled as RT_FUSED_PARTS translation units side by side with the
 API unit, then linked.
 """
 import os

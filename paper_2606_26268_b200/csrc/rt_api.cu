@@ -856,9 +856,9 @@ static bool fused_make_maps(const rt_grid* g, const FusedArgs& a, int narr, Fuse
     return true;
 }
 
-template <bool HLL, bool THICK, bool CURVI, bool FEEDBACK, bool RUS, bool HASZ, bool VARFIX>
+template <bool HLL, bool THICK, bool CURVI, bool FEEDBACK, bool RUS, bool HASZ, int VMODE>
 static cudaError_t launch_fused_z(rt_grid* g, const ParamsDev& P, const FusedArgs& a, const FusedMaps& maps, dim3 grid, int seglen) {
-    auto kern = k_substep_fused<HLL, THICK, CURVI, FEEDBACK, RUS, HASZ, VARFIX>;
+    auto kern = k_substep_fused<HLL, THICK, CURVI, FEEDBACK, RUS, HASZ, VMODE>;
     // the attribute is per device (and per instantiation: this function is a template)
     static bool attr_done[64] = {false};
     const int dev = g->device >= 0 && g->device < 64 ? g->device : 0;
@@ -874,11 +874,15 @@ static cudaError_t launch_fused_z(rt_grid* g, const ParamsDev& P, const FusedArg
 // x3 active (3-D) or not (2-D); the comparison face fixes (a.fix != 0; never with the Rusanov solver: fused_eligible)
 template <bool HLL, bool THICK, bool CURVI, bool FEEDBACK, bool RUS = false>
 static cudaError_t launch_fused_t(rt_grid* g, const ParamsDev& P, const FusedArgs& a, const FusedMaps& maps, dim3 grid, int seglen) {
-    if (!RUS && (a.fix != 0 || a.im.avgU[0] != nullptr))
-        return g->dev.gh[2] > 0 ? launch_fused_z<HLL, THICK, CURVI, FEEDBACK, false, true, true>(g, P, a, maps, grid, seglen)
-                                : launch_fused_z<HLL, THICK, CURVI, FEEDBACK, false, false, true>(g, P, a, maps, grid, seglen);
-    return g->dev.gh[2] > 0 ? launch_fused_z<HLL, THICK, CURVI, FEEDBACK, RUS, true, false>(g, P, a, maps, grid, seglen)
-                            : launch_fused_z<HLL, THICK, CURVI, FEEDBACK, RUS, false, false>(g, P, a, maps, grid, seglen);
+    // VMODE (rt_kernels_fused.cuh): 2 = run-time face fix (+ RK2 options), 1 = RK2 average, 0 = neither
+    if (!RUS && a.fix != 0)
+        return g->dev.gh[2] > 0 ? launch_fused_z<HLL, THICK, CURVI, FEEDBACK, false, true, 2>(g, P, a, maps, grid, seglen)
+                                : launch_fused_z<HLL, THICK, CURVI, FEEDBACK, false, false, 2>(g, P, a, maps, grid, seglen);
+    if (!RUS && a.im.avgU[0] != nullptr)
+        return g->dev.gh[2] > 0 ? launch_fused_z<HLL, THICK, CURVI, FEEDBACK, false, true, 1>(g, P, a, maps, grid, seglen)
+                                : launch_fused_z<HLL, THICK, CURVI, FEEDBACK, false, false, 1>(g, P, a, maps, grid, seglen);
+    return g->dev.gh[2] > 0 ? launch_fused_z<HLL, THICK, CURVI, FEEDBACK, RUS, true, 0>(g, P, a, maps, grid, seglen)
+                            : launch_fused_z<HLL, THICK, CURVI, FEEDBACK, RUS, false, 0>(g, P, a, maps, grid, seglen);
 }
 
 static cudaError_t launch_fused(rt_grid* g, bool hll, bool thick, bool curvi, bool feedback, const ParamsDev& P,

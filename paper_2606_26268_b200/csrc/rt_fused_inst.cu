@@ -1,6 +1,6 @@
 // rt_fused_inst.cu — explicit instantiations of k_substep_fused, one part per translation unit:
 //   nvcc -DRT_FUSED_PART=<0 .. RT_FUSED_PARTS-1> -c rt_fused_inst.cu
-// (80 instantiations of a 128-register kernel take minutes in one unit; the parts compile side by side).
+// (112 instantiations of a 128-register kernel take minutes in one unit; the parts compile side by side).
 #include "rt_kernels_fused.cuh"
 #include "rt_fused_inst.cuh"
 

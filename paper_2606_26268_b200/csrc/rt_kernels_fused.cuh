@@ -67,7 +67,7 @@ struct FusedArgs {
     ImplicitArgs im;           // U = U_out, rho, T, mom, dt / dt_dev, scratch, counters
     double chat;
     int use_tma;
-    int fix;                   // RT_FIX_* (read only by the VARFIX instantiations)
+    int fix;                   // RT_FIX_* (read only by the VMODE = 2 instantiations)
 };
 struct alignas(64) FusedMaps {
     CUtensorMap m[FNARR];      // ghosted (nt1, nt2, nt3) fp64 tensors, box 34 x FPH x 1
@@ -155,10 +155,12 @@ __device__ __forceinline__ void state_load(const double* buf, int t, State& s) {
 // RUS (with HLL = true): RT_SOLVER_RUSANOV, compile-time so that the HLL faces do not pay for the test
 // HASZ = false: 2-D grids (n3 = 1, x3 inactive): one staged plane, no x3 phase; the march degenerates to the steps
 // c = 0 (X, Y) and 1 (FIN, which reads nothing but the thick-limit value of plane 0).
-// VARFIX = true: the instantiations with run-time options: the comparison face fixes of rt_set_face_fix (flat fallback
-// L136 / clip Eq. 36-38) selected by the launch-uniform a.fix, and the RK2 average of the second stage (a.im.avgU ...);
-// false: the paper's f-preserving scheme, compiled in, plain stores (the default path carries no test for either)
-template <bool HLL, bool THICK, bool CURVI, bool FEEDBACK, bool RUS, bool HASZ, bool VARFIX = false>
+// VMODE = 0: the paper's f-preserving scheme compiled in, T and m updated through a.im.Tout / mout, no other option
+// (the path of rt_substep).  1: the same plus the RK2 average of the second stage (rt_rk2_step) behind one
+// launch-uniform test per cell (a.im.avgU[0] != nullptr); the values to average with are prefetched into L2 one plane
+// ahead.  2: 1 plus the comparison face fixes of rt_set_face_fix (flat fallback L136 / clip Eq. 36-38) selected by
+// the launch-uniform a.fix.
+template <bool HLL, bool THICK, bool CURVI, bool FEEDBACK, bool RUS, bool HASZ, int VMODE = 0>
 __global__ void __launch_bounds__(FNT, FUSED_MINB)
     k_substep_fused(const __grid_constant__ GridDev g, const __grid_constant__ ParamsDev par, const __grid_constant__ OpacDev oP,
                     const __grid_constant__ OpacDev oR, const __grid_constant__ OpacDev oS, const __grid_constant__ FusedArgs a,
@@ -184,7 +186,7 @@ __global__ void __launch_bounds__(FNT, FUSED_MINB)
     const int o = (ly + 2) * FPW + lx + 2;  // this thread's cell inside a staged plane
     const bool tma = a.use_tma != 0;
     constexpr bool rus = HLL && RUS;
-    const int fix = VARFIX ? a.fix : 0;
+    const int fix = VMODE == 2 ? a.fix : 0;
     const double dt = a.im.dt_dev ? __ldg(a.im.dt_dev) : a.im.dt;
     const double dtc = dt * a.chat;
 
@@ -308,6 +310,15 @@ __global__ void __launch_bounds__(FNT, FUSED_MINB)
 #pragma unroll
                 for (int q = 0; q < 3; ++q) prefetch_l2(a.im.mom[q] + idn);
             }
+            if (VMODE != 0 && a.im.avgU[0] != nullptr) {  // launch-uniform: the second RK2 stage averages with U^n, T^n, m^n
+#pragma unroll
+                for (int q = 0; q < 4; ++q) prefetch_l2(a.im.avgU[q] + idn);
+                prefetch_l2(a.im.avgT + idn);
+                if (FEEDBACK) {
+#pragma unroll
+                    for (int q = 0; q < 3; ++q) prefetch_l2(a.im.avgm[q] + idn);
+                }
+            }
         }
         // gas state of cell c-1 for FIN: issued here so that the x3 phase hides what is left of its latency
         double rho_f = 1.0, T_f = 1.0, kpr_f = 0.0;
@@ -376,7 +387,7 @@ __global__ void __launch_bounds__(FNT, FUSED_MINB)
                         const double ilmin = HASZ ? dmin(il[0], dmin(il[1], il[2])) : dmin(il[0], il[1]);  // active directions
                         rhochi = lim > 1.0e300 ? 0.0 : (4.0 / 3.0) * ilmin * frcp(lim);
                     }
-                    const double r = implicit_cell<FEEDBACK, true, THICK, VARFIX>(g, par, oP, oR, oS, a.im, dt, (long long)id, il, U4[0],
+                    const double r = implicit_cell<FEEDBACK, true, THICK, VMODE != 0>(g, par, oP, oR, oS, a.im, dt, (long long)id, il, U4[0],
                                                                                   F, rho, T0, m, floored, clipped, rhochi, kpr_f);
                     rate = dmax(rate, r);
                     nfloor += floored ? 1 : 0;

@@ -275,6 +275,19 @@ __device__ __forceinline__ double implicit_cell(const GridDev& g, const ParamsDe
                                                 const double il[3] /* 1/dl_d of the cell (CFL only) */, double E, double F[3],
                                                 double rho, double T0, const double m[3], bool& floored, bool& clipped,
                                                 double rhochi_given = 0.0, double rhokp_given = 0.0) {
+    // second RK2 stage (launch-uniform): the values to average with, loaded first so that the arithmetic below covers
+    // their latency
+    const bool avg = AVG && a.avgU[0] != nullptr;
+    double avE = 0.0, avT = 0.0, avF[3] = {0.0, 0.0, 0.0}, avm[3] = {0.0, 0.0, 0.0};
+    if (avg) {
+        avE = a.avgU[0][id];
+        avT = a.avgT[id];
+#pragma unroll
+        for (int q = 0; q < 3; ++q) {
+            avF[q] = a.avgU[1 + q][id];
+            if (FEEDBACK) avm[q] = a.avgm[q][id];
+        }
+    }
     // irradiation (Eq. 34-35): Q = -div F_irr dt joins S_1 of Eq. 33; a launch-uniform branch
     const bool irr = a.divfirr != nullptr;
     double Q = 0.0;
@@ -323,10 +336,9 @@ __device__ __forceinline__ double implicit_cell(const GridDev& g, const ParamsDe
     }
     double En = En_, Tn = Tn_;
     const double idamp = frcp(fma(dt * par.chat, rhochi, 1.0));
-    const bool avg = AVG && a.avgU[0] != nullptr;  // launch-uniform
     if (avg) {
-        En = 0.5 * (En + a.avgU[0][id]);
-        Tn = 0.5 * (Tn + a.avgT[id]);
+        En = 0.5 * (En + avE);
+        Tn = 0.5 * (Tn + avT);
     }
     a.U[0][id] = En;
     a.Tout[id] = Tn;
@@ -337,10 +349,10 @@ __device__ __forceinline__ double implicit_cell(const GridDev& g, const ParamsDe
         Fn[q] = F[q] * idamp;
         if (FEEDBACK) {
             double mn = fma(-(Fn[q] - F[q]), ichat, m[q]);
-            if (avg) mn = 0.5 * (mn + a.avgm[q][id]);
+            if (avg) mn = 0.5 * (mn + avm[q]);
             a.mout[q][id] = mn;
         }
-        if (avg) Fn[q] = 0.5 * (Fn[q] + a.avgU[1 + q][id]);
+        if (avg) Fn[q] = 0.5 * (Fn[q] + avF[q]);
         a.U[1 + q][id] = Fn[q];
     }
     return CFL ? cell_rate_il(par.chat, En, Fn[0], Fn[1], Fn[2], il) : 0.0;
