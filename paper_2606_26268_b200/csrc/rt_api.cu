@@ -494,12 +494,8 @@ static int32_t launch_fill_ghosts(rt_grid* g, double* const U[4]) {
     return RT_OK;
 }
 
-// face-normal ghosts of all active axes in one launch (the sub-step kernels read nothing else)
-static int32_t launch_fill_faces(rt_grid* g, double* const U[4], cudaStream_t st = nullptr) {
-    if (!st) st = g->stream;
-    const GridDev& D = g->dev;
-    Fields4 F;
-    for (int q = 0; q < 4; ++q) F.q[q] = U[q];
+// blocks of 256 threads for the face-normal ghost fill (0: nothing to fill)
+static int fill_faces_blocks(const GridDev& D) {
     long long tot = 0;
     for (int d = 0; d < 3; ++d) {
         if (D.gh[d] == 0 || (D.bc[2 * d] == RT_BC_FIXED && D.bc[2 * d + 1] == RT_BC_FIXED)) continue;
@@ -508,8 +504,17 @@ static int32_t launch_fill_faces(rt_grid* g, double* const U[4], cudaStream_t st
             if (e != d) c *= D.n[e];
         tot += c;
     }
-    if (tot == 0) return RT_OK;
-    const int nb = (int)((tot + 255) / 256 > 8192 ? 8192 : (tot + 255) / 256);
+    return (int)((tot + 255) / 256 > 8192 ? 8192 : (tot + 255) / 256);
+}
+
+// face-normal ghosts of all active axes in one launch (the sub-step kernels read nothing else)
+static int32_t launch_fill_faces(rt_grid* g, double* const U[4], cudaStream_t st = nullptr) {
+    if (!st) st = g->stream;
+    const GridDev& D = g->dev;
+    Fields4 F;
+    for (int q = 0; q < 4; ++q) F.q[q] = U[q];
+    const int nb = fill_faces_blocks(D);
+    if (nb == 0) return RT_OK;
     {
         ProfScope ps(g, RT_K_GHOST, st);
         k_fill_faces<<<nb, 256, 0, st>>>(D, F);
@@ -568,7 +573,9 @@ static void launch_sweep(rt_grid* g, int d, bool hll, bool thick, bool curvi, co
 }
 
 // with_kp: also write rho kappa_P per cell into g->kpr (fused sub-step: the implicit half then evaluates no opacity)
-static int32_t launch_thick_limit(rt_grid* g, const double* rho, const double* T, bool with_kp = false) {
+// Ufill: also fill the face-normal ghosts of these four fields, in the same launch (k_thick_limit_faces)
+static int32_t launch_thick_limit(rt_grid* g, const double* rho, const double* T, bool with_kp = false,
+                                  double* const* Ufill = nullptr) {
     const GridDev& D = g->dev;
     // ghosts the kernel never writes (beyond the first face-normal layer) are never used either: zero them once
     if (!g->lim) {
@@ -592,6 +599,13 @@ static int32_t launch_thick_limit(rt_grid* g, const double* rho, const double* T
         }
     }
     dim3 grid((D.n[0] + bx - 1) / bx, (D.n[1] + kThickRows - 1) / kThickRows, D.n[2]);
+    int nbg = Ufill ? fill_faces_blocks(D) : 0;
+    const long long nthick = (long long)grid.x * grid.y * grid.z;
+    if (nbg > 0 && nthick + nbg >= (1LL << 31)) {  // too many blocks for one 1-D grid: two launches
+        const int32_t rcf = launch_fill_faces(g, Ufill);
+        if (rcf != RT_OK) return rcf;
+        nbg = 0;
+    }
     {
         ProfScope ps(g, RT_K_THICK);
         const OpacDev &oP = g->opac[RT_OPAC_PLANCK], &oR = g->opac[RT_OPAC_ROSSELAND], &oS = g->opac[RT_OPAC_SCATTER];
@@ -629,12 +643,27 @@ static int32_t launch_thick_limit(rt_grid* g, const double* rho, const double* T
             tp.lrho_min = oR.lrho_min; tp.lrho_max = oR.lrho_max; tp.lT_min = oR.lT_min; tp.lT_max = oR.lT_max;
             tp.su = oR.su; tp.sv = oR.sv; tp.rho_unit = oR.rho_unit; tp.T_unit = oR.T_unit;
         }
-        if (lean)
-            k_thick_limit<1><<<grid, bx, 0, g->stream>>>(D, oR, oS, os, rho, T, g->lim, oP, g->same_PR, kpr, L, tp);
-        else if (pair)
-            k_thick_limit<2><<<grid, bx, 0, g->stream>>>(D, oR, oS, os, rho, T, g->lim, oP, g->same_PR, kpr, L, tp);
-        else
-            k_thick_limit<0><<<grid, bx, 0, g->stream>>>(D, oR, oS, os, rho, T, g->lim, oP, g->same_PR, kpr, L, tp);
+        if (nbg > 0) {
+            // the ghost fill rides in the same launch (its blocks are sized for 256 threads; bx <= 256 of them only makes
+            // their grid-stride loops a little longer)
+            Fields4 F;
+            for (int q = 0; q < 4; ++q) F.q[q] = Ufill[q];
+            const unsigned nblk = (unsigned)(nthick + nbg);
+            const int gx = (int)grid.x, gy = (int)grid.y;
+            if (lean)
+                k_thick_limit_faces<1><<<nblk, bx, 0, g->stream>>>(D, oR, oS, os, rho, T, g->lim, oP, g->same_PR, kpr, L, tp, F, nbg, gx, gy);
+            else if (pair)
+                k_thick_limit_faces<2><<<nblk, bx, 0, g->stream>>>(D, oR, oS, os, rho, T, g->lim, oP, g->same_PR, kpr, L, tp, F, nbg, gx, gy);
+            else
+                k_thick_limit_faces<0><<<nblk, bx, 0, g->stream>>>(D, oR, oS, os, rho, T, g->lim, oP, g->same_PR, kpr, L, tp, F, nbg, gx, gy);
+        } else {
+            if (lean)
+                k_thick_limit<1><<<grid, bx, 0, g->stream>>>(D, oR, oS, os, rho, T, g->lim, oP, g->same_PR, kpr, L, tp);
+            else if (pair)
+                k_thick_limit<2><<<grid, bx, 0, g->stream>>>(D, oR, oS, os, rho, T, g->lim, oP, g->same_PR, kpr, L, tp);
+            else
+                k_thick_limit<0><<<grid, bx, 0, g->stream>>>(D, oR, oS, os, rho, T, g->lim, oP, g->same_PR, kpr, L, tp);
+        }
     }
     RT_LAUNCH_CHECK(g);
     return RT_OK;
@@ -987,14 +1016,9 @@ static int32_t fused_impl(rt_grid* g, double* dt_device, double cfl, const doubl
     const GridDev& D = g->dev;
     const bool thick = g->par.thick_limit != 0;
 
-    int32_t rc = launch_fill_faces(g, U_in);
+    // the ghost fill and, with the thick limit, the pre-pass: one launch (k_thick_limit_faces)
+    int32_t rc = thick ? launch_thick_limit(g, rho, T, true, U_in) : launch_fill_faces(g, U_in);
     if (rc != RT_OK) return rc;
-    if (thick) {
-        // (running the ghost fill beside the pre-pass on a second stream was measured: no gain, both are short and
-        // memory-bound)
-        rc = launch_thick_limit(g, rho, T, true);
-        if (rc != RT_OK) return rc;
-    }
     FusedArgs a;
     for (int q = 0; q < 4; ++q) {
         a.src[q] = U_in[q];

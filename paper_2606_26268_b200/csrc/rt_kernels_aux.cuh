@@ -156,7 +156,8 @@ static __global__ void k_fill_ghosts(GridDev g, Fields4 U, int d) {
 // a1 for the sub-step kernels, ONE launch: the face-normal ghosts of every active axis (other axes over their
 // interior range only).  The scheme never reads edge / corner ghosts — each direction's stencil leaves the
 // interior along its own axis only — so rt_substep does not need the axis-by-axis ordering of k_fill_ghosts.
-static __global__ void k_fill_faces(GridDev g, Fields4 U) {
+// block `block` of `nblocks` blocks of blockDim.x threads
+__device__ __forceinline__ void fill_faces_body(const GridDev& g, const Fields4& U, int block, int nblocks) {
     // one work item = both ghost layers of one (transverse cell, side) of one axis; along x1 the two layers are one
     // 16-byte store (they share a 32-byte sector: item-per-layer traffic was twice the sectors)
     long long cnt[3], tot = 0;
@@ -166,7 +167,7 @@ static __global__ void k_fill_faces(GridDev g, Fields4 U) {
         cnt[d] = skip ? 0 : 2LL * g.n[ea] * g.n[eb];
         tot += cnt[d];
     }
-    for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < tot; t += (long long)gridDim.x * blockDim.x) {
+    for (long long t = block * (long long)blockDim.x + threadIdx.x; t < tot; t += (long long)nblocks * blockDim.x) {
         long long r = t;
         int d = 0;
         while (r >= cnt[d]) {
@@ -221,6 +222,10 @@ static __global__ void k_fill_faces(GridDev g, Fields4 U) {
             }
         }
     }
+}
+
+static __global__ void k_fill_faces(const __grid_constant__ GridDev g, const __grid_constant__ Fields4 U) {
+    fill_faces_body(g, U, (int)blockIdx.x, (int)gridDim.x);
 }
 
 // Debug aid (SURVEY.md Sect. 5 "failure detection"): count the interior cells in which any of up to five fields is not finite.
@@ -524,16 +529,16 @@ __device__ __forceinline__ void table_pair_eval(const TablePair& tp, double rho,
     }
 }
 
+// block (bxi, byi, bzi) of the pre-pass: x1 columns bxi * blockDim.x ..., x2 rows byi * kThickRows ..., x3 plane bzi
 template <int MODE>
-__global__ void __launch_bounds__(256) k_thick_limit(const __grid_constant__ GridDev g, const __grid_constant__ OpacDev oR,
-                                                     const __grid_constant__ OpacDev oS, const __grid_constant__ OpacSet os,
-                                                     const double* __restrict__ rho, const double* __restrict__ T,
-                                                     double* __restrict__ lim, const __grid_constant__ OpacDev oP,
-                                                     int same_PR, double* __restrict__ kpr, const __grid_constant__ LeanLaws laws,
-                                                     const __grid_constant__ TablePair tp) {
+__device__ __forceinline__ void thick_limit_body(const GridDev& g, const OpacDev& oR, const OpacDev& oS, const OpacSet& os,
+                                                 const double* __restrict__ rho, const double* __restrict__ T,
+                                                 double* __restrict__ lim, const OpacDev& oP, int same_PR,
+                                                 double* __restrict__ kpr, const LeanLaws& laws, const TablePair& tp, int bxi,
+                                                 int byi, int bzi) {
     constexpr bool LEAN = MODE == 1;
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    const int k = blockIdx.z;
+    const int i = bxi * blockDim.x + threadIdx.x;
+    const int k = bzi;
     if (i >= g.n[0]) return;
     const bool share = MODE == 0 && os.share != 0;
     const int s1 = (int)g.stride[1], s2 = (int)g.stride[2];
@@ -556,7 +561,7 @@ __global__ void __launch_bounds__(256) k_thick_limit(const __grid_constant__ Gri
         if (k == n2 - 1) goff2 = (per ? -n2 : 1) * s2;
     }
     const bool per1 = g.bc[2] == 0;
-    const int j0 = blockIdx.y * kThickRows;
+    const int j0 = byi * kThickRows;
     const int j1 = min(j0 + kThickRows, n1);
     const double* __restrict__ len01 = g.len[0][1];
     const double* __restrict__ len11 = g.len[1][1];
@@ -599,6 +604,39 @@ __global__ void __launch_bounds__(256) k_thick_limit(const __grid_constant__ Gri
             if (j == n1 - 1) lim[id + (per1 ? -n1 : 1) * s1] = v;
         }
     }
+}
+
+template <int MODE>
+__global__ void __launch_bounds__(256) k_thick_limit(const __grid_constant__ GridDev g, const __grid_constant__ OpacDev oR,
+                                                     const __grid_constant__ OpacDev oS, const __grid_constant__ OpacSet os,
+                                                     const double* __restrict__ rho, const double* __restrict__ T,
+                                                     double* __restrict__ lim, const __grid_constant__ OpacDev oP,
+                                                     int same_PR, double* __restrict__ kpr, const __grid_constant__ LeanLaws laws,
+                                                     const __grid_constant__ TablePair tp) {
+    thick_limit_body<MODE>(g, oR, oS, os, rho, T, lim, oP, same_PR, kpr, laws, tp, (int)blockIdx.x, (int)blockIdx.y, (int)blockIdx.z);
+}
+
+// The pre-pass and the ghost fill of a sub-step in ONE launch (rt_substep on 2-D / 3-D grids): they touch different
+// arrays (lim, rho kappa_P from rho, T | the ghosts of U), so nbg blocks of the 1-D grid, spread evenly over it, do the
+// ghost fill -- short, bound by the sector traffic of the x1 ghosts -- beside the issue-bound pre-pass blocks (the l-th
+// of which is block bxi + gx (byi + gy bzi) of the pre-pass); one launch gap less per sub-step.
+template <int MODE>
+__global__ void __launch_bounds__(256) k_thick_limit_faces(const __grid_constant__ GridDev g, const __grid_constant__ OpacDev oR,
+                                                           const __grid_constant__ OpacDev oS, const __grid_constant__ OpacSet os,
+                                                           const double* __restrict__ rho, const double* __restrict__ T,
+                                                           double* __restrict__ lim, const __grid_constant__ OpacDev oP,
+                                                           int same_PR, double* __restrict__ kpr,
+                                                           const __grid_constant__ LeanLaws laws, const __grid_constant__ TablePair tp,
+                                                           const __grid_constant__ Fields4 U, int nbg, int gx, int gy) {
+    // ghost-fill blocks are every stride-th block of the grid, so that they are resident beside pre-pass blocks
+    const int tot = (int)gridDim.x, stride = tot / nbg, b = (int)blockIdx.x;
+    if (b % stride == 0 && b / stride < nbg) {
+        fill_faces_body(g, U, b / stride, nbg);
+        return;
+    }
+    const int l = b - min(nbg, (b + stride - 1) / stride);
+    const int bxi = l % gx, t = l / gx;
+    thick_limit_body<MODE>(g, oR, oS, os, rho, T, lim, oP, same_PR, kpr, laws, tp, bxi, t % gy, t / gy);
 }
 
 // ------------------------------------------------------------------------------------------------
