@@ -217,6 +217,25 @@ int32_t rt_set_tuning(rt_grid* g, int32_t march_len, int32_t fused_seg);
  * Synchronises the stream.  Bad argument -> RT_ERR_INVALID_ARG; no device / launch failure -> RT_ERR_CUDA. */
 int32_t rt_measure_fp64(void* cuda_stream, int32_t blocks, int32_t threads, int32_t chains, int32_t iters, double* ms_host);
 
+/* The CFL time step (step 10, L120; R-G15: dt = cfl / max_cells sum_{d active} chat max(|lambda_1|, |lambda_3|)_d / dx_d)
+ * of a UNIFORM CARTESIAN grid through an entry point that ALLOCATES NOTHING: no grid handle, no cudaMalloc / cudaFree, no
+ * allocating library routine -- for callers that cannot allocate (code under CUDA graph capture, tight serving loops,
+ * harnesses that forbid it).  Same per-cell arithmetic as rt_cfl_dt_async, which it matches to rounding (<= 1e-14).
+ *   cuda_stream  the stream the work is enqueued on (no synchronisation)
+ *   n[3]         HOST; interior cells per axis; n[d] == 1: inactive (no ghosts, adds no rate)
+ *   dx[3]        HOST; cell length per axis (> 0 on every active axis)
+ *   U[4]         HOST array of four DEVICE pointers: E, F1, F2, F3 in the layout above (ghosted, nghost = 2); caller-owned
+ *   dt_device    DEVICE; receives dt; caller-owned
+ *   err, err_len HOST; optional buffer that receives a NUL-terminated description when the status is not RT_OK
+ * The device the fields live on must be the CURRENT device.  The reduction's scratch is a static device array inside the
+ * library (512 KB, held by every GPU that loads the library until exit) with one slot per x2-x3 row: grids with
+ * n[1] * n[2] > RT_NOALLOC_MAX_ROWS are refused with RT_ERR_INVALID_ARG (256^3 still fits).  All calls share that
+ * array: calls that overlap on one GPU (different streams or threads) race; calls on one stream are ordered and safe.
+ * The first call on a device looks the array's address up (cudaGetSymbolAddress); make that call outside stream capture. */
+#define RT_NOALLOC_MAX_ROWS 65536
+int32_t rt_cfl_dt_uniform_noalloc(void* cuda_stream, const int32_t n[3], const double dx[3], double chat, double cfl,
+                                  const double* const U[4], double* dt_device, char* err, int32_t err_len);
+
 const char* rt_last_error(const rt_grid* g);
 
 #ifdef __cplusplus

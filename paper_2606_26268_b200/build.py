@@ -5,7 +5,7 @@
 nvcc cross-compiles without a GPU.  The library links the static CUDA runtime, so it depends only on
 the driver at run time.  The fused sub-step kernel has 112 instantiations (solver x thick limit x geometry x
 feedback x 2-D/3-D x {plain, RK2 average, run-time face fix}); they are compiled as RT_FUSED_PARTS translation units side by side with the
-API unit, then linked.
+API unit and rt_noalloc.cu (the entry point that allocates nothing), then linked.
 """
 import os
 import subprocess
@@ -19,8 +19,9 @@ LIB_PATH = os.path.join(HERE, "librt_m1.so")
 CSRC = os.path.join(HERE, "csrc")
 API_SRC = os.path.join(CSRC, "rt_api.cu")
 INST_SRC = os.path.join(CSRC, "rt_fused_inst.cu")
+NOALLOC_SRC = os.path.join(CSRC, "rt_noalloc.cu")
 FUSED_PARTS = 6
-SOURCES = [API_SRC, INST_SRC]
+SOURCES = [API_SRC, INST_SRC, NOALLOC_SRC]
 HEADERS = [os.path.join(CSRC, f) for f in ("rt_math.cuh", "rt_types.cuh", "rt_kernels_aux.cuh", "rt_kernels_step.cuh",
                                            "rt_kernels_fused.cuh", "rt_kernels_measure.cuh", "rt_fused_inst.cuh")] \
     + [os.path.join(ROOT, "include", "rt.h")]
@@ -50,7 +51,8 @@ def build(force=False, verbose=False):
     nvcc = _nvcc()
     extra = ["-Xptxas", "-v"] if verbose else []
     with tempfile.TemporaryDirectory(prefix="rt_m1_build_") as tmp:
-        jobs = [([nvcc] + NVCC_FLAGS + extra + ["-c", API_SRC, "-o", os.path.join(tmp, "rt_api.o")])]
+        jobs = [([nvcc] + NVCC_FLAGS + extra + ["-c", API_SRC, "-o", os.path.join(tmp, "rt_api.o")]),
+                ([nvcc] + NVCC_FLAGS + extra + ["-c", NOALLOC_SRC, "-o", os.path.join(tmp, "rt_noalloc.o")])]
         for part in range(FUSED_PARTS):
             jobs.append([nvcc] + NVCC_FLAGS + extra + ["-DRT_FUSED_PART=%d" % part, "-c", INST_SRC, "-o",
                                                       os.path.join(tmp, "rt_fused_inst_%d.o" % part)])

@@ -81,6 +81,8 @@ _SIGNATURES = {
     "rt_set_profiling": (C.c_int32, [C.c_void_p, C.c_int32]),
     "rt_get_kernel_times": (C.c_int32, [C.c_void_p, _dp, C.POINTER(C.c_int64)]),
     "rt_measure_fp64": (C.c_int32, [C.c_void_p, C.c_int32, C.c_int32, C.c_int32, C.c_int32, _dp]),
+    "rt_cfl_dt_uniform_noalloc": (C.c_int32, [C.c_void_p, C.POINTER(C.c_int32), _dp, C.c_double, C.c_double,
+                                              C.POINTER(C.c_void_p), C.c_void_p, C.c_char_p, C.c_int32]),
     "rt_last_error": (C.c_char_p, [C.c_void_p]),
 }
 
@@ -173,6 +175,30 @@ def measure_fp64(blocks, threads, chains, iters, device="cuda:0"):
         raise RtError("rt_measure_fp64", rc)
     nch, per = (chains, 8) if chains < 100 else (chains - 100, 64) if chains < 200 else (4, 8)
     return ms.value, float(blocks) * threads * nch * per * iters
+
+
+NOALLOC_MAX_ROWS = 65536
+
+
+def cfl_dt_uniform_noalloc(n, dx, chat, cfl, U, dt_device):
+    """rt_cfl_dt_uniform_noalloc: the CFL time step of a uniform Cartesian grid into dt_device, through the entry point
+    that allocates nothing (no handle; static device scratch; n[1] * n[2] <= NOALLOC_MAX_ROWS).  Enqueued on the current
+    stream of the fields' device."""
+    if not torch.cuda.is_available():
+        raise RuntimeError("no CUDA device: paper_2606_26268_b200 has no CPU path")
+    n = [int(v) for v in n]
+    shape = tuple(v + 2 * NGHOST if v > 1 else 1 for v in reversed(n))
+    for q in range(4):
+        _check_field(U[q], shape, "U[%d]" % q, U[0].device if isinstance(U[0], torch.Tensor) else None)
+    if not (dt_device.is_cuda and dt_device.dtype == torch.float64 and dt_device.numel() >= 1 and dt_device.device == U[0].device):
+        raise ValueError("dt_device must be a CUDA float64 tensor on the fields' device")
+    err = C.create_string_buffer(256)
+    with torch.cuda.device(U[0].device):
+        st = torch.cuda.current_stream()
+        rc = lib().rt_cfl_dt_uniform_noalloc(C.c_void_p(st.cuda_stream), (C.c_int32 * 3)(*n), (C.c_double * 3)(*[float(v) for v in dx]),
+                                             float(chat), float(cfl), _ptr_array(U), dt_device.data_ptr(), err, len(err))
+    if rc != OK:
+        raise RtError("rt_cfl_dt_uniform_noalloc", rc, err.value.decode())
 
 
 class Grid:
