@@ -177,11 +177,15 @@ def one_substep(rt, g, w, st, step_index):
 
 
 def csrc_hash():
-    """sha256 over the CUDA sources: ties the ncu-derived instruction counts under profiles/ to the code they were taken from"""
+    """sha256 over the CUDA sources k_substep_fused and its launch are built from (everything under csrc/ except the two
+    files that hold only self-contained extras: the fp64 microbenchmark kernels and the no-alloc CFL entry point): ties
+    the ncu-derived instruction counts under profiles/ to the code they were taken from"""
     import hashlib
     h = hashlib.sha256()
     d = os.path.join(ROOT, "paper_2606_26268_b200", "csrc")
     for f in sorted(os.listdir(d)):
+        if f in ("rt_kernels_measure.cuh", "rt_noalloc.cu"):
+            continue
         with open(os.path.join(d, f), "rb") as fh:
             h.update(f.encode() + b"\0" + fh.read())
     return h.hexdigest()[:16]
