@@ -572,6 +572,15 @@ static void launch_sweep(rt_grid* g, int d, bool hll, bool thick, bool curvi, co
     }
 }
 
+// chi is ONE half-integer power law (kappa_R fast, no scattering) and kappa_P, when asked for, is the same law or another
+// fast law with the same rho0, T0: the pre-pass takes its lean path (k_thick_limit<1>)
+static bool lean_laws(const rt_grid* g, bool with_kp) {
+    const OpacDev &oP = g->opac[RT_OPAC_PLANCK], &oR = g->opac[RT_OPAC_ROSSELAND], &oS = g->opac[RT_OPAC_SCATTER];
+    bool lean = oR.set && oR.kind == 0 && oR.fast && !oS.set;
+    if (with_kp && !g->same_PR) lean = lean && oP.set && oP.kind == 0 && oP.fast && oP.irho0 == oR.irho0 && oP.iT0 == oR.iT0;
+    return lean;
+}
+
 // with_kp: also write rho kappa_P per cell into g->kpr (fused sub-step: the implicit half then evaluates no opacity)
 // Ufill: also fill the face-normal ghosts of these four fields, in the same launch (k_thick_limit_faces)
 static int32_t launch_thick_limit(rt_grid* g, const double* rho, const double* T, bool with_kp = false,
@@ -598,7 +607,14 @@ static int32_t launch_thick_limit(rt_grid* g, const double* rho, const double* T
             }
         }
     }
-    dim3 grid((D.n[0] + bx - 1) / bx, (D.n[1] + kThickRows - 1) / kThickRows, D.n[2]);
+    // x2 rows per block: kThickRows, or (lean power laws: register batches of kThickRows rows, the next batch prefetched
+    // into L2) four times as many where that still leaves >= 16 blocks per SM
+    int rpb = kThickRows;
+    if (lean_laws(g, with_kp)) {
+        rpb = 4 * kThickRows;
+        while (rpb > kThickRows && (long long)((D.n[0] + bx - 1) / bx) * ((D.n[1] + rpb - 1) / rpb) * D.n[2] < 16LL * 148) rpb /= 2;
+    }
+    dim3 grid((D.n[0] + bx - 1) / bx, (D.n[1] + rpb - 1) / rpb, D.n[2]);
     int nbg = Ufill ? fill_faces_blocks(D) : 0;
     const long long nthick = (long long)grid.x * grid.y * grid.z;
     if (nbg > 0 && nthick + nbg >= (1LL << 31)) {  // too many blocks for one 1-D grid: two launches
@@ -612,9 +628,8 @@ static int32_t launch_thick_limit(rt_grid* g, const double* rho, const double* T
         const int m2[2] = {RT_OPAC_ROSSELAND, RT_OPAC_SCATTER};
         const int m3[3] = {RT_OPAC_PLANCK, RT_OPAC_ROSSELAND, RT_OPAC_SCATTER};
         const OpacSet os = with_kp ? opac_set(g, m3, 3) : opac_set(g, m2, 2);
-        bool lean = oR.set && oR.kind == 0 && oR.fast && !oS.set;
+        const bool lean = lean_laws(g, with_kp);
         const bool second = with_kp && !g->same_PR;
-        if (second) lean = lean && oP.set && oP.kind == 0 && oP.fast && oP.irho0 == oR.irho0 && oP.iT0 == oR.iT0;
         double* kpr = with_kp ? g->kpr : nullptr;
         LeanLaws L;
         memset(&L, 0, sizeof(L));
@@ -650,19 +665,23 @@ static int32_t launch_thick_limit(rt_grid* g, const double* rho, const double* T
             for (int q = 0; q < 4; ++q) F.q[q] = Ufill[q];
             const unsigned nblk = (unsigned)(nthick + nbg);
             const int gx = (int)grid.x, gy = (int)grid.y;
-            if (lean)
-                k_thick_limit_faces<1><<<nblk, bx, 0, g->stream>>>(D, oR, oS, os, rho, T, g->lim, oP, g->same_PR, kpr, L, tp, F, nbg, gx, gy);
+            if (lean && rpb > kThickRows)
+                k_thick_limit_faces<3><<<nblk, bx, 0, g->stream>>>(D, oR, oS, os, rho, T, g->lim, oP, g->same_PR, kpr, L, tp, F, nbg, gx, gy, rpb);
+            else if (lean)
+                k_thick_limit_faces<1><<<nblk, bx, 0, g->stream>>>(D, oR, oS, os, rho, T, g->lim, oP, g->same_PR, kpr, L, tp, F, nbg, gx, gy, rpb);
             else if (pair)
-                k_thick_limit_faces<2><<<nblk, bx, 0, g->stream>>>(D, oR, oS, os, rho, T, g->lim, oP, g->same_PR, kpr, L, tp, F, nbg, gx, gy);
+                k_thick_limit_faces<2><<<nblk, bx, 0, g->stream>>>(D, oR, oS, os, rho, T, g->lim, oP, g->same_PR, kpr, L, tp, F, nbg, gx, gy, rpb);
             else
-                k_thick_limit_faces<0><<<nblk, bx, 0, g->stream>>>(D, oR, oS, os, rho, T, g->lim, oP, g->same_PR, kpr, L, tp, F, nbg, gx, gy);
+                k_thick_limit_faces<0><<<nblk, bx, 0, g->stream>>>(D, oR, oS, os, rho, T, g->lim, oP, g->same_PR, kpr, L, tp, F, nbg, gx, gy, rpb);
         } else {
-            if (lean)
-                k_thick_limit<1><<<grid, bx, 0, g->stream>>>(D, oR, oS, os, rho, T, g->lim, oP, g->same_PR, kpr, L, tp);
+            if (lean && rpb > kThickRows)
+                k_thick_limit<3><<<grid, bx, 0, g->stream>>>(D, oR, oS, os, rho, T, g->lim, oP, g->same_PR, kpr, L, tp, rpb);
+            else if (lean)
+                k_thick_limit<1><<<grid, bx, 0, g->stream>>>(D, oR, oS, os, rho, T, g->lim, oP, g->same_PR, kpr, L, tp, rpb);
             else if (pair)
-                k_thick_limit<2><<<grid, bx, 0, g->stream>>>(D, oR, oS, os, rho, T, g->lim, oP, g->same_PR, kpr, L, tp);
+                k_thick_limit<2><<<grid, bx, 0, g->stream>>>(D, oR, oS, os, rho, T, g->lim, oP, g->same_PR, kpr, L, tp, rpb);
             else
-                k_thick_limit<0><<<grid, bx, 0, g->stream>>>(D, oR, oS, os, rho, T, g->lim, oP, g->same_PR, kpr, L, tp);
+                k_thick_limit<0><<<grid, bx, 0, g->stream>>>(D, oR, oS, os, rho, T, g->lim, oP, g->same_PR, kpr, L, tp, rpb);
         }
     }
     RT_LAUNCH_CHECK(g);

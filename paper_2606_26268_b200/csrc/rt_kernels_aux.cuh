@@ -495,6 +495,54 @@ __device__ __forceinline__ void lean_eval(const LeanLaws& L, double rho, double 
     }
 }
 
+// The same for R cells of one thread at a time: the launch-uniform multi-way branches are taken once per batch instead
+// of once per cell (per cell they were a quarter of the pre-pass's instructions).
+template <int R>
+__device__ __forceinline__ void pow_half_batch(const double (&x)[R], int n, double (&out)[R]) {
+    switch (n) {
+#define RT_PH(N)                                                                       \
+    case N:                                                                            \
+        _Pragma("unroll") for (int r = 0; r < R; ++r) out[r] = pow_half_ct<N>(x[r]);   \
+        break;
+        RT_PH(-15) RT_PH(-14) RT_PH(-13) RT_PH(-12) RT_PH(-11) RT_PH(-10) RT_PH(-9) RT_PH(-8) RT_PH(-7) RT_PH(-6) RT_PH(-5)
+        RT_PH(-4) RT_PH(-3) RT_PH(-2) RT_PH(-1) RT_PH(1) RT_PH(2) RT_PH(3) RT_PH(4) RT_PH(5) RT_PH(6) RT_PH(7) RT_PH(8)
+        RT_PH(9) RT_PH(10) RT_PH(11) RT_PH(12) RT_PH(13) RT_PH(14) RT_PH(15)
+#undef RT_PH
+        default:
+#pragma unroll
+            for (int r = 0; r < R; ++r) out[r] = 1.0;
+    }
+}
+template <int R>
+__device__ __forceinline__ void lean_eval_batch(const LeanLaws& L, const double (&rho)[R], const double (&T)[R],
+                                                double (&k_first)[R], double (&k_second)[R]) {
+    double xr[R], xt[R], pr[R], pt[R];
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        xr[r] = rho[r] * L.irho0;
+        xt[r] = T[r] * L.iT0;
+    }
+    pow_half_batch<R>(xr, L.na[0], pr);
+    pow_half_batch<R>(xt, L.nb[0], pt);
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        pr[r] *= pt[r];
+        k_first[r] = dmin(dmax(L.k0[0] * pr[r], L.kmin[0]), L.kmax[0]);
+        k_second[r] = k_first[r];
+    }
+    if (L.two) {
+        if (!L.same_ab) {
+            pow_half_batch<R>(xr, L.na[1], pr);
+            pow_half_batch<R>(xt, L.nb[1], pt);
+#pragma unroll
+            for (int r = 0; r < R; ++r) pr[r] *= pt[r];
+        }
+#pragma unroll
+        for (int r = 0; r < R; ++r) k_second[r] = dmin(dmax(L.k0[1] * pr[r], L.kmin[1]), L.kmax[1]);
+    }
+}
+__device__ __forceinline__ void prefetch_global_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
+
 // LEAN: chi is ONE half-integer power law (kappa_R fast, no scattering) and kappa_P, when asked for (kpr != nullptr:
 // the fused sub-step, whose implicit half then evaluates no opacity at all), is the same law or another fast law with
 // the same rho0, T0.  Otherwise the general evaluation (tables share their log10 inputs: OpacSet).
@@ -529,14 +577,14 @@ __device__ __forceinline__ void table_pair_eval(const TablePair& tp, double rho,
     }
 }
 
-// block (bxi, byi, bzi) of the pre-pass: x1 columns bxi * blockDim.x ..., x2 rows byi * kThickRows ..., x3 plane bzi
+// block (bxi, byi, bzi) of the pre-pass: x1 columns bxi * blockDim.x ..., x2 rows byi * rows_per_block ..., x3 plane bzi
 template <int MODE>
 __device__ __forceinline__ void thick_limit_body(const GridDev& g, const OpacDev& oR, const OpacDev& oS, const OpacSet& os,
                                                  const double* __restrict__ rho, const double* __restrict__ T,
                                                  double* __restrict__ lim, const OpacDev& oP, int same_PR,
                                                  double* __restrict__ kpr, const LeanLaws& laws, const TablePair& tp, int bxi,
-                                                 int byi, int bzi) {
-    constexpr bool LEAN = MODE == 1;
+                                                 int byi, int bzi, int rows_per_block) {
+    constexpr bool LEAN = MODE == 1 || MODE == 3;  // 3: the register-batch form (large grids)
     const int i = bxi * blockDim.x + threadIdx.x;
     const int k = bzi;
     if (i >= g.n[0]) return;
@@ -561,12 +609,59 @@ __device__ __forceinline__ void thick_limit_body(const GridDev& g, const OpacDev
         if (k == n2 - 1) goff2 = (per ? -n2 : 1) * s2;
     }
     const bool per1 = g.bc[2] == 0;
-    const int j0 = byi * kThickRows;
-    const int j1 = min(j0 + kThickRows, n1);
+    const int j0 = byi * rows_per_block;  // rows_per_block: a multiple of kThickRows
+    const int j1 = min(j0 + rows_per_block, n1);
     const double* __restrict__ len01 = g.len[0][1];
     const double* __restrict__ len11 = g.len[1][1];
     const double* __restrict__ len21 = g.len[2][1];
     int id = (i + g.gh[0]) + (j0 + g.gh[1]) * s1 + (k + g.gh[2]) * s2;
+    // what follows the opacities of one cell: rho kappa_P, tau, lim and the ghost copies of lim
+    auto finish = [&](int j, int idc, double rc, double chi, double kP) {
+        if (kpr) kpr[idc] = kP * rc;
+        double dx = l02[0] * __ldg(len01 + j);
+        if (act1) dx = dmax(dx, l02[1] * __ldg(len11 + j));
+        if (act2) dx = dmax(dx, l02[2] * __ldg(len21 + j));
+        const double tau = rc * chi * dx;
+        // any value >= 1 means "no limit" (|lambda| <= 1, L167): tau -> 0 maps to +inf without a division by zero
+        const double v = tau > 1.0e-100 ? 4.0 * frcp(3.0 * tau) : __builtin_huge_val();
+        lim[idc] = v;
+        if (goff0 | goff2) {
+            if (goff0) lim[idc + goff0] = v;
+            if (goff2) lim[idc + goff2] = v;
+        }
+        if (act1 && (j == 0 || j == n1 - 1)) {
+            if (j == 0) lim[idc + (per1 ? n1 : -1) * s1] = v;
+            if (j == n1 - 1) lim[idc + (per1 ? -n1 : 1) * s1] = v;
+        }
+    };
+    if (MODE == 3) {
+        // kThickRows cells at a time as one register batch (the plan's launch-uniform branches once per batch); the next
+        // batch's rho, T are on their way into L2 while this one is computed (a prefetch holds no registers)
+        constexpr int R = kThickRows;
+#pragma unroll 1
+        for (int jb = j0; jb < j1; jb += R, id += R * s1) {
+            double rb[R], tb[R], chi[R], kP[R];
+#pragma unroll
+            for (int q = 0; q < R; ++q) {
+                const int idq = id + min(q, j1 - 1 - jb) * s1;  // rows past the end repeat the last one (not stored)
+                rb[q] = __ldg(rho + idq);
+                tb[q] = __ldg(T + idq);
+            }
+            if (jb + R < j1) {
+#pragma unroll
+                for (int q = 0; q < R; ++q) {
+                    const int idq = id + min(R + q, j1 - 1 - jb) * s1;
+                    prefetch_global_l2(rho + idq);
+                    prefetch_global_l2(T + idq);
+                }
+            }
+            lean_eval_batch<R>(laws, rb, tb, chi, kP);
+#pragma unroll
+            for (int q = 0; q < R; ++q)
+                if (jb + q < j1) finish(jb + q, id + q * s1, rb[q], chi[q], kP[q]);
+        }
+        return;
+    }
     double r = __ldg(rho + id), t = __ldg(T + id);
 #pragma unroll 1
     for (int j = j0; j < j1; ++j, id += s1) {
@@ -587,22 +682,7 @@ __device__ __forceinline__ void thick_limit_body(const GridDev& g, const OpacDev
             chi = kR + opacity_eval_shared(oS, rc, tc, share, l);
             kP = !kpr ? 0.0 : (same_PR ? kR : opacity_eval_shared(oP, rc, tc, share, l));
         }
-        if (kpr) kpr[id] = kP * rc;
-        double dx = l02[0] * __ldg(len01 + j);
-        if (act1) dx = dmax(dx, l02[1] * __ldg(len11 + j));
-        if (act2) dx = dmax(dx, l02[2] * __ldg(len21 + j));
-        const double tau = rc * chi * dx;
-        // any value >= 1 means "no limit" (|lambda| <= 1, L167): tau -> 0 maps to +inf without a division by zero
-        const double v = tau > 1.0e-100 ? 4.0 * frcp(3.0 * tau) : __builtin_huge_val();
-        lim[id] = v;
-        if (goff0 | goff2) {
-            if (goff0) lim[id + goff0] = v;
-            if (goff2) lim[id + goff2] = v;
-        }
-        if (act1 && (j == 0 || j == n1 - 1)) {
-            if (j == 0) lim[id + (per1 ? n1 : -1) * s1] = v;
-            if (j == n1 - 1) lim[id + (per1 ? -n1 : 1) * s1] = v;
-        }
+        finish(j, id, rc, chi, kP);
     }
 }
 
@@ -612,8 +692,9 @@ __global__ void __launch_bounds__(256) k_thick_limit(const __grid_constant__ Gri
                                                      const double* __restrict__ rho, const double* __restrict__ T,
                                                      double* __restrict__ lim, const __grid_constant__ OpacDev oP,
                                                      int same_PR, double* __restrict__ kpr, const __grid_constant__ LeanLaws laws,
-                                                     const __grid_constant__ TablePair tp) {
-    thick_limit_body<MODE>(g, oR, oS, os, rho, T, lim, oP, same_PR, kpr, laws, tp, (int)blockIdx.x, (int)blockIdx.y, (int)blockIdx.z);
+                                                     const __grid_constant__ TablePair tp, int rows_per_block) {
+    thick_limit_body<MODE>(g, oR, oS, os, rho, T, lim, oP, same_PR, kpr, laws, tp, (int)blockIdx.x, (int)blockIdx.y, (int)blockIdx.z,
+                           rows_per_block);
 }
 
 // The pre-pass and the ghost fill of a sub-step in ONE launch (rt_substep on 2-D / 3-D grids): they touch different
@@ -627,7 +708,7 @@ __global__ void __launch_bounds__(256) k_thick_limit_faces(const __grid_constant
                                                            double* __restrict__ lim, const __grid_constant__ OpacDev oP,
                                                            int same_PR, double* __restrict__ kpr,
                                                            const __grid_constant__ LeanLaws laws, const __grid_constant__ TablePair tp,
-                                                           const __grid_constant__ Fields4 U, int nbg, int gx, int gy) {
+                                                           const __grid_constant__ Fields4 U, int nbg, int gx, int gy, int rows_per_block) {
     // ghost-fill blocks are every stride-th block of the grid, so that they are resident beside pre-pass blocks
     const int tot = (int)gridDim.x, stride = tot / nbg, b = (int)blockIdx.x;
     if (b % stride == 0 && b / stride < nbg) {
@@ -636,7 +717,7 @@ __global__ void __launch_bounds__(256) k_thick_limit_faces(const __grid_constant
     }
     const int l = b - min(nbg, (b + stride - 1) / stride);
     const int bxi = l % gx, t = l / gx;
-    thick_limit_body<MODE>(g, oR, oS, os, rho, T, lim, oP, same_PR, kpr, laws, tp, bxi, t % gy, t / gy);
+    thick_limit_body<MODE>(g, oR, oS, os, rho, T, lim, oP, same_PR, kpr, laws, tp, bxi, t % gy, t / gy, rows_per_block);
 }
 
 // ------------------------------------------------------------------------------------------------

@@ -1108,6 +1108,21 @@ def test_argument_errors_are_reported_not_computed(rt):
     assert all(torch.all(v == 0.0) for v in V), "a rejected call must not enqueue work"
 
 
+@pytest.mark.parametrize("fused", [False, True])
+@pytest.mark.parametrize("same_law", [False, True])
+def test_lean_prepass_register_batches_on_a_ragged_grid(rt, fused, same_law):
+    """the thick-limit pre-pass in its register-batch form (k_thick_limit<3>: half-integer power laws, no scattering,
+    grids large enough for two batches of 4 rows per block): 1030 rows = 128 blocks of 8 + one of 6 (a full batch and
+    a ragged one); fused: inside the launch it shares with the ghost fill, with rho kappa_P from a second law"""
+    w = random_workload(W.CARTESIAN, (40, 1030, 35), W.SOLVER_HLL, 1, seed=771, bc=(1, 1, 0, 0, 2, 1))
+    kP = W.power_law(1.0 if same_law else 2.0, a=1.0, b=-3.5 if same_law else -3.0, kmin=1e-4, kmax=1e6)
+    w.opacities = {W.OPAC_PLANCK: kP, W.OPAC_ROSSELAND: W.power_law(1.0, a=1.0, b=-3.5, kmin=1e-4, kmax=1e6)}
+    errs, counts, _ = run_both(rt, w, 1, fused=fused, local=True)
+    assert_below(errs[0], TOL1, "lean pre-pass, batches")
+    assert_local_below(errs[1], TOL1, "lean pre-pass, batches")
+    assert counts[0] == counts[1]
+
+
 def test_fp64_probe_modes_and_what_they_charge(rt):
     """rt_measure_fp64 (include/rt.h): bad arguments are refused; the operand-count modes order as DESIGN.md Sect. 5
     states: a DFMA with three register operands runs at about 2/3 of the rate of one with two, and four fp32
