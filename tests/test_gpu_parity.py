@@ -690,6 +690,38 @@ def test_limo3_smoothness_switch_on_smooth_fields(rt, case):
     assert np.abs(U0[0] - refU[0]).max() > 1e-9 * np.abs(refU[0]).max()
 
 
+@pytest.mark.parametrize("case", ["cart3d-hll", "cyl2d-hll", "sph3d-glf-rk2"])
+def test_limo3_through_substep_and_rk2(rt, case):
+    """LimO3 through rt_substep on a 2-D grid with HLL and through rt_rk2_step (the composition the paper's Fig. 1-3 runs
+    use): smooth fields with the smoothness switch on both branches, curvilinear lengths in the switch, against the oracle.
+    (LimO3 takes the per-direction kernels: as an instantiation of the fused kernel it was measured SLOWER, DESIGN.md
+    Sect. 6.)"""
+    geometry, n, solver, r = {"cart3d-hll": (W.CARTESIAN, (70, 33, 12), W.SOLVER_HLL, 0.15),
+                              "cyl2d-hll": (W.CYLINDRICAL, (64, 40, 1), W.SOLVER_HLL, 0.4),
+                              "sph3d-glf-rk2": (W.SPHERICAL, (45, 20, 17), W.SOLVER_GLF, 0.15)}[case]
+    w = _smooth_workload(geometry, n, solver, seed=390 + len(case))
+    if geometry != W.CARTESIAN:
+        w.bc = (1, 1, 1, 1, 0, 0) if n[2] > 1 else (1, 1, 1, 1, 1, 1)
+    og = ort.grid_from_workload(w)
+    og.set_reconstruction(ort.RECON_LIMO3, r)
+    g = drv.grid_from_workload(w)
+    g.set_reconstruction(rt.RECON_LIMO3, r)
+    if case.endswith("rk2"):
+        refU, refT, refm, dts = ort.run_rk2(og, w, 2)
+        st, hist = drv.run_rk2(g, w, 2)
+        tol = 8 * TOL1
+    else:
+        refU, refT, refm, dts = ort.run_substeps(og, w, 3)
+        st, _, hist = drv.run_substeps_fused(g, w, 3)
+        tol = 3 * TOL1
+    torch.cuda.synchronize()
+    assert np.allclose(hist.cpu().numpy(), dts, rtol=1e-12, atol=0)
+    errs = field_errors(w, to_host(st.U), refU, st.T.cpu().numpy(), refT, to_host(st.mom), refm)
+    assert_below(errs, tol, "LimO3, " + case)
+    lerrs = local_errors(w, to_host(st.U), refU, st.T.cpu().numpy(), refT, to_host(st.mom), refm)
+    assert_local_below(lerrs, tol, "LimO3, " + case)
+
+
 # ----------------------------------------------------------------------------- streams and CUDA graphs
 def test_substeps_on_a_side_stream_and_replayed_from_a_cuda_graph(rt):
     """rt_substep enqueues on the stream given at rt_grid_create and never synchronises: (a) a grid created on a side
