@@ -203,11 +203,18 @@ __device__ __forceinline__ double half_slope(double dm, double dp) {
 // eta = 1 - eps, phi_L above 1 + eps, their blend in between (eps = 1e-12).
 __device__ __forceinline__ double limo3_times(double dnum, double dden, double eta) {
     const double p3 = (2.0 * dden + dnum) * (1.0 / 3.0);
-    const bool neg = dden < 0.0;
-    const double a = fabs(dden), b = neg ? -dnum : dnum, P = neg ? -p3 : p3;
-    const double inner = dmin(dmin(b + b, P), 1.6 * a);
-    const double pl = dmax(0.0, dmin(P, dmax(-0.5 * b, inner)));
-    const double pL = neg ? -pl : pl;
+    // the sign folds are multiplications by s = +-1 (exact) instead of selects, and the min / max chain is split by the
+    // sign of b, which leaves three of its five: for b >= 0 every candidate is >= 0 and P >= the others' minimum, so
+    // a phi_L = min(P, 2b, 1.6a); for b < 0 the inner minimum is <= 2b < 0 < -b/2, so a phi_L = max(0, min(P, -b/2)).
+    // Both are max(0, min(P, c, d)) with (c, d) = (2b, 1.6a) or (-b/2, +inf): the same VALUE as the chain, bit for bit
+    // (min and max round nothing; 2b and -b/2 are exact).
+    const double s = __hiloint2double((__double2hiint(dden) & (int)0x80000000) | 0x3ff00000, 0);
+    const double a = fabs(dden), b = s * dnum, P = s * p3;
+    const bool pos = b >= 0.0;
+    const double c = b * (pos ? 2.0 : -0.5);
+    const double d = pos ? 1.6 * a : __builtin_huge_val();
+    const double pl = dmax(0.0, dmin(dmin(P, c), d));
+    const double pL = s * pl;
     if (eta < 0.0) return pL;
     constexpr double eps = 1.0e-12;
     if (eta <= 1.0 - eps) return p3;
