@@ -13,8 +13,9 @@
 // 8-byte cp.async loop instead.  Thread (lx, ly) owns cell (i0+lx, j0+ly): every lane owns an output cell.  The
 // fluxes through the two OUTER x1 faces of a row (lower face of lane 0, upper face of lane 31) need the face states of
 // the cells i0-1 and i0+32: the 2 x FTY such faces of a plane are one half-filled warp task ("edge task": both face
-// states + Riemann flux of the face), done one step ahead by the warp whose turn it is (rows take turns, so the extra
-// work averages out) and handed over through shared memory.  That costs 3.6 % more warp instructions than the rows
+// states + Riemann flux of the face), done one step ahead by the warp whose turn it is (rows 1, 2, 5, 6 take turns:
+// rows 0 and FTY-1 already carry the tile's extra x2 face work, and rows 4 and 3 share their schedulers) and handed
+// over through shared memory.  That costs 3.6 % more warp instructions than the rows
 // alone; halo lanes (30 useful lanes of 32, and a ragged ninth tile on a 256-cell row) cost 12.5 %.
 // Per plane c, every thread:
 //   Z  : both x3 face states of cell c (Eq. 17-21 + closure + speeds), Riemann flux at face c-1/2 against
@@ -296,7 +297,9 @@ __global__ void __launch_bounds__(FNT, FUSED_MINB)
         if (HASZ) {
             // outer x1 faces of plane c+1, consumed by the X phase of the next step (behind its barrier); the buffer
             // written here was last read in the X phase of step c-1, before this step's barrier
-            if (c + 1 < kb && ly == ((c + 1) & (FNY - 1))) edge_task(c + 1, planes + ((c + 5) & 3) * (FNARR * FPS));
+            // the task rotates over the warps of rows 1, 2, 5, 6: rows 0 and FTY-1 carry the extra x2 face work of the tile's
+            // edge and share their schedulers (warp id mod 4) with rows 4 and 3
+            if (c + 1 < kb && ly == (((c + 1) & 1) + 1 + ((c + 1) & 2) * 2)) edge_task(c + 1, planes + ((c + 5) & 3) * (FNARR * FPS));
         } else if (c == 0) {
             if (ly == 0) edge_task(0, pc);   // 2-D: the only plane; one extra barrier
             __syncthreads();
